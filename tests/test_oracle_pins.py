@@ -1,0 +1,342 @@
+"""Pins for the CPU oracle (no GPU): the oracle is checked against what the paper and the mathematics fix,
+never against itself.  Each test says which mistake it is meant to catch."""
+import numpy as np
+import pytest
+
+from oracle import banded, dense, residual, stepwise
+from paper_1812_01396_b200 import inputs
+
+
+# --------------------------------------------------------------------------------------------
+# independent helpers (hand-written, no LAPACK)
+# --------------------------------------------------------------------------------------------
+def gauss_solve(A, B):
+    """Textbook Gaussian elimination with partial pivoting + back substitution, python loops."""
+    A = np.array(A, dtype=np.complex128)
+    B = np.array(B, dtype=np.complex128)
+    n = A.shape[0]
+    for k in range(n):
+        p = k + int(np.argmax(np.abs(A[k:, k])))
+        if p != k:
+            A[[k, p]] = A[[p, k]]
+            B[[k, p]] = B[[p, k]]
+        for i in range(k + 1, n):
+            f = A[i, k] / A[k, k]
+            A[i, k:] -= f * A[k, k:]
+            B[i] -= f * B[k]
+    X = np.zeros_like(B)
+    for i in range(n - 1, -1, -1):
+        X[i] = (B[i] - A[i, i + 1:] @ X[i + 1:]) / A[i, i]
+    return X
+
+
+def tiny(bs, nb, n_e=2, nrhs=3, seed=7, eta=1e-3, inj_last=False):
+    return inputs.random_problem(bs, nb, n_e, nrhs, seed=seed, eta=eta, inj_last=inj_last)
+
+
+def args(p, e):
+    il = None if p.Inj_last is None else p.Inj_last[e]
+    return (p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], il)
+
+
+# --------------------------------------------------------------------------------------------
+# assembly: element-by-element definition (catches wrong block placement / missing conj / conj(E))
+# --------------------------------------------------------------------------------------------
+def test_assemble_T_elementwise_definition():
+    p = tiny(3, 4)
+    E = p.E[0]
+    T = dense.assemble_T(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[0], p.Sigma_R[0])
+    bs, nb = 3, 4
+    n = bs * nb
+    for r in range(n):
+        for c in range(n):
+            I, a = divmod(r, bs)
+            J, b = divmod(c, bs)
+            if I == J:
+                v = E * p.S_diag[I][a, b] - p.H_diag[I][a, b]
+                if I == 0:
+                    v -= p.Sigma_L[0][a, b]
+                if I == nb - 1:
+                    v -= p.Sigma_R[0][a, b]
+            elif J == I + 1:
+                v = E * p.S_upper[I][a, b] - p.H_upper[I][a, b]
+            elif J == I - 1:
+                # lower block = conj-transpose of the MATRICES, E itself not conjugated (reading c8)
+                v = E * np.conj(p.S_upper[J][b, a]) - np.conj(p.H_upper[J][b, a])
+            else:
+                v = 0.0
+            assert T[r, c] == pytest.approx(v, abs=1e-15)
+
+
+def test_A_is_hermitian_only_at_real_E():
+    p = tiny(4, 3, eta=0.0)
+    A = dense.assemble_A(p.E[0].real, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    assert np.allclose(A, A.conj().T, atol=1e-14)
+    A2 = dense.assemble_A(p.E[0].real + 0.1j, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    assert not np.allclose(A2, A2.conj().T, atol=1e-6)
+    # A(E) - A(E)^H = 2i Im(E) S exactly
+    S = dense.assemble_A(1.0, np.zeros_like(p.H_diag), np.zeros_like(p.H_upper), p.S_diag, p.S_upper)
+    assert np.allclose(A2 - A2.conj().T, 2j * 0.1 * S, atol=1e-13)
+
+
+# --------------------------------------------------------------------------------------------
+# solve: brute force, hand-written elimination, residual
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb", [(1, 2), (2, 2), (3, 3), (2, 5), (16, 8)])
+def test_solve_vs_bruteforce_inverse_and_gauss(bs, nb):
+    p = tiny(bs, nb, inj_last=True)
+    for e in range(p.n_energy):
+        r = dense.solve_energy(*args(p, e))
+        T = dense.assemble_T(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e])
+        Tinv = np.linalg.inv(T)
+        b = dense.pad_injection(p.Inj_first[e], p.Inj_last[e], nb)
+        assert np.allclose(r["X"], Tinv @ b, rtol=1e-10, atol=1e-12)
+        assert np.allclose(r["G_1N"], Tinv[:bs, -bs:], rtol=1e-10, atol=1e-12)
+        assert np.allclose(r["G_N1"], Tinv[-bs:, :bs], rtol=1e-10, atol=1e-12)
+        if bs * nb <= 12:
+            assert np.allclose(r["X"], gauss_solve(T, b), rtol=1e-10, atol=1e-12)
+        # invariant T X = Inj (north_star)
+        assert np.linalg.norm(T @ r["X"] - b) <= 1e-13 * (np.linalg.norm(T) * np.linalg.norm(r["X"]) + np.linalg.norm(b))
+
+
+def test_transmission_formula_written_out():
+    """T = sum_{abcd} GL[a,b] G[b,c] GR[c,d] conj(G[a,d]) with Gamma = i(Sigma - Sigma^H) -- index loops."""
+    p = tiny(3, 3)
+    r = dense.solve_energy(*args(p, 0))
+    G = r["G_1N"]
+    SL, SR = p.Sigma_L[0], p.Sigma_R[0]
+    bs = 3
+    GL = np.array([[1j * (SL[a, b] - np.conj(SL[b, a])) for b in range(bs)] for a in range(bs)])
+    GR = np.array([[1j * (SR[a, b] - np.conj(SR[b, a])) for b in range(bs)] for a in range(bs)])
+    t = 0.0
+    for a in range(bs):
+        for b in range(bs):
+            for c in range(bs):
+                for d in range(bs):
+                    t += GL[a, b] * G[b, c] * GR[c, d] * np.conj(G[a, d])
+    assert r["T_LR"] == pytest.approx(t.real, rel=1e-12)
+    assert abs(r["T_LR_complex"].imag) <= 1e-12 * max(1.0, abs(t.real))     # reading c6
+
+
+# --------------------------------------------------------------------------------------------
+# closed forms
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb,n_e", [(1, 6, 5), (4, 10, 6)])
+def test_perfect_chain_closed_form_dense(bs, nb, n_e):
+    """BASELINE.json config 1 (small): X_j = e^{ikj} 1, T(E) = bs exactly (number of channels in band)."""
+    p = inputs.perfect_chain_problem(bs, nb, n_e)
+    k = inputs.chain_wavevector(p.E, -1.0)
+    for e in range(n_e):
+        r = dense.solve_energy(*args(p, e))
+        expect = np.concatenate([np.exp(1j * k[e] * j) * np.eye(bs) for j in range(1, nb + 1)])
+        assert np.allclose(r["X"], expect, atol=1e-12)
+        assert r["T_LR"] == pytest.approx(bs, abs=1e-11)
+        assert r["T_RL"] == pytest.approx(bs, abs=1e-11)
+
+
+def test_perfect_chain_config1_banded_full_size():
+    """BASELINE.json config 1 at full size (bs=64, nb=256), Tier B, a subset of the 64 energies."""
+    cfg = inputs.CONFIGS["C1"]
+    p = inputs.make_problem(cfg)
+    k = inputs.chain_wavevector(p.E, -1.0)
+    for e in (0, 31, 63):
+        r = banded.solve_energy(*args(p, e))
+        assert r["T_LR"] == pytest.approx(64.0, abs=1e-9)
+        j = np.arange(1, cfg.nb + 1)
+        Xb = r["X"].reshape(cfg.nb, cfg.bs, cfg.bs)
+        expect = np.exp(1j * k[e] * j)[:, None, None] * np.eye(cfg.bs)[None]
+        assert np.abs(Xb - expect).max() <= 1e-10
+
+
+def test_single_impurity_textbook_transmission():
+    """1-D tight-binding chain (bs = 1), one site with on-site energy V: textbook result
+    T(E) = (2 t sin k)^2 / ((2 t sin k)^2 + V^2), E = 2 t cos k.  Catches errors in where Sigma sits,
+    in Gamma, in the off-diagonal sign and in the trace formula."""
+    t, V, nb = -1.0, 0.7, 9
+    p = inputs.perfect_chain_problem(1, nb, 7, t=t)
+    p.H_diag[4, 0, 0] = V
+    k = inputs.chain_wavevector(p.E, t)
+    for e in range(p.n_energy):
+        r = dense.solve_energy(*args(p, e))
+        v2 = (2 * t * np.sin(k[e])) ** 2
+        assert r["T_LR"] == pytest.approx(v2 / (v2 + V * V), rel=1e-12)
+        assert r["T_RL"] == pytest.approx(v2 / (v2 + V * V), rel=1e-12)
+
+
+def test_scalar_chain_surface_greens_function():
+    """bs = 1, nb = 2 dimer with analytic 2x2 inverse: G_12 = -A_12 / det."""
+    p = tiny(1, 2)
+    E = p.E[0]
+    r = dense.solve_energy(*args(p, 0))
+    a = E * p.S_diag[0][0, 0] - p.H_diag[0][0, 0] - p.Sigma_L[0][0, 0]
+    d = E * p.S_diag[1][0, 0] - p.H_diag[1][0, 0] - p.Sigma_R[0][0, 0]
+    u = E * p.S_upper[0][0, 0] - p.H_upper[0][0, 0]
+    l = E * np.conj(p.S_upper[0][0, 0]) - np.conj(p.H_upper[0][0, 0])
+    det = a * d - u * l
+    assert r["G_1N"][0, 0] == pytest.approx(-u / det, rel=1e-12)
+    assert r["G_N1"][0, 0] == pytest.approx(-l / det, rel=1e-12)
+    gl = -2 * p.Sigma_L[0][0, 0].imag
+    gr = -2 * p.Sigma_R[0][0, 0].imag
+    assert r["T_LR"] == pytest.approx(gl * gr * abs(u / det) ** 2, rel=1e-12)
+
+
+# --------------------------------------------------------------------------------------------
+# invariants
+# --------------------------------------------------------------------------------------------
+def test_T_LR_equals_T_RL_at_real_energy():
+    """Exact only at Im E = 0 (reading c10)."""
+    p = tiny(6, 5, n_e=3, eta=0.0)
+    for e in range(3):
+        r = dense.solve_energy(*args(p, e))
+        assert r["T_LR"] == pytest.approx(r["T_RL"], rel=1e-11)
+
+
+def test_eta_identity_at_complex_energy():
+    """T_LR - T_RL = 2 eta [Tr(Gamma_L G^H S G) - Tr(Gamma_L G S G^H)] restricted to block (1,1)
+    (reading c10; needs the full G, tiny inputs only)."""
+    p = tiny(4, 4, n_e=2, eta=5e-2)
+    bs, nb = 4, 4
+    for e in range(2):
+        r = dense.solve_energy(*args(p, e))
+        T = dense.assemble_T(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e])
+        G = np.linalg.inv(T)
+        S = dense.assemble_A(1.0, np.zeros_like(p.H_diag), np.zeros_like(p.H_upper), p.S_diag, p.S_upper)
+        GL = np.zeros_like(G)
+        GL[:bs, :bs] = dense.gamma(p.Sigma_L[e])
+        eta = p.E[e].imag
+        rhs = 2 * eta * (np.trace(GL @ G.conj().T @ S @ G) - np.trace(GL @ G @ S @ G.conj().T)).real
+        assert abs(r["T_LR"] - r["T_RL"]) > 1e-6           # they really differ at eta != 0
+        assert r["T_LR"] - r["T_RL"] == pytest.approx(rhs, rel=1e-8, abs=1e-12)
+
+
+def test_transmission_bounds_and_zero_cases():
+    p = tiny(5, 4, n_e=3)
+    for e in range(3):
+        r = dense.solve_energy(*args(p, e))
+        assert -1e-12 <= r["T_LR"] <= 5 + 1e-12             # 0 <= T <= bs (Gamma >= 0, reading c7)
+    z = np.zeros((5, 5), dtype=np.complex128)
+    a = list(args(p, 0))
+    a[5] = z                                                 # Sigma_L = 0 => Gamma_L = 0 => T = 0
+    assert dense.solve_energy(*a)["T_LR"] == pytest.approx(0.0, abs=1e-14)
+    p2 = tiny(5, 4, n_e=1)
+    p2.H_upper[1] = 0.0
+    p2.S_upper[1] = 0.0                                      # decoupled halves => G_1N = 0 => T = 0
+    assert dense.solve_energy(*args(p2, 0))["T_LR"] == pytest.approx(0.0, abs=1e-14)
+
+
+def test_gamma_is_positive_semidefinite_for_generator():
+    p = tiny(8, 2)
+    w = np.linalg.eigvalsh(dense.gamma(p.Sigma_L[0]))
+    assert w.min() >= -1e-12
+
+
+# --------------------------------------------------------------------------------------------
+# inverse block columns
+# --------------------------------------------------------------------------------------------
+def test_inverse_columns_vs_dense_inverse_and_structure():
+    p = tiny(4, 5, eta=0.0)
+    E = p.E[1].real
+    Q, P = dense.inverse_columns(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    Ainv = np.linalg.inv(dense.assemble_A(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper))
+    bs, nb = 4, 5
+    for i in range(nb):
+        assert np.allclose(Q[i], Ainv[i * bs:(i + 1) * bs, :bs], rtol=1e-9, atol=1e-11)
+        assert np.allclose(P[i], Ainv[i * bs:(i + 1) * bs, -bs:], rtol=1e-9, atol=1e-11)
+    # A Hermitian at real E  =>  (A^-1)_{1,nb} = ((A^-1)_{nb,1})^H
+    assert np.allclose(P[0], Q[nb - 1].conj().T, rtol=1e-9, atol=1e-11)
+    assert residual.inverse_column_residual(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper, Q, P) < 1e-14
+
+
+# --------------------------------------------------------------------------------------------
+# the paper's algebra (Algorithm 1, Eq. 11-13) against the plain definition, incl. our readings c1-c4
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb", [(2, 2), (3, 4), (8, 6)])
+def test_algorithm1_and_four_steps_reach_the_plain_definition(bs, nb):
+    p = tiny(bs, nb, inj_last=True)
+    for e in range(p.n_energy):
+        Q, _ = stepwise.algorithm1_first_column(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+        P, _ = stepwise.algorithm1_last_column(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+        Qo, Po = dense.inverse_columns(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+        assert np.allclose(Q, Qo, rtol=1e-8, atol=1e-10)
+        assert np.allclose(P, Po, rtol=1e-8, atol=1e-10)
+        x, R, x1 = stepwise.four_steps(Q, P, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], p.Inj_last[e])
+        r = dense.solve_energy(*args(p, e))
+        assert np.allclose(x, r["X"], rtol=1e-8, atol=1e-10)
+        assert np.allclose(x1, r["X"], rtol=1e-8, atol=1e-10)
+        # first / last block columns of T^-1 are [Q P] R^-1  =>  G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22
+        Rinv = np.linalg.inv(R)
+        G1N = Q[0] @ Rinv[:bs, bs:] + P[0] @ Rinv[bs:, bs:]
+        assert np.allclose(G1N, r["G_1N"], rtol=1e-8, atol=1e-10)
+
+
+# --------------------------------------------------------------------------------------------
+# Tier B (banded) pinned to Tier A (dense); Tier C residual pinned to the dense residual
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb", [(1, 2), (3, 2), (16, 8), (40, 5)])
+def test_banded_matches_dense(bs, nb):
+    p = tiny(bs, nb, inj_last=True)
+    for e in range(p.n_energy):
+        rd = dense.solve_energy(*args(p, e))
+        rb = banded.solve_energy(*args(p, e))
+        assert residual.rel_frobenius(rb["X"], rd["X"]) < 1e-11
+        assert residual.rel_T(rb["T_LR"], rd["T_LR"]) < 1e-10
+        assert residual.rel_T(rb["T_RL"], rd["T_RL"]) < 1e-10
+        assert np.allclose(rb["G_1N"], rd["G_1N"], rtol=1e-9, atol=1e-12)
+
+
+def test_banded_matches_dense_medium():
+    p = inputs.random_problem(128, 6, 1, 16, seed=0)
+    rd = dense.solve_energy(*args(p, 0))
+    rb = banded.solve_energy(*args(p, 0))
+    assert residual.rel_frobenius(rb["X"], rd["X"]) < 1e-11
+    assert residual.rel_T(rb["T_LR"], rd["T_LR"]) < 1e-10
+
+
+def test_residual_matches_dense_residual():
+    p = tiny(5, 4, inj_last=True)
+    r = dense.solve_energy(*args(p, 0))
+    X = r["X"] + 1e-6 * inputs.complex_gaussian(1, 99, 0, r["X"].shape, 1.0)   # perturbed on purpose
+    T = dense.assemble_T(p.E[0], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[0], p.Sigma_R[0])
+    b = dense.pad_injection(p.Inj_first[0], p.Inj_last[0], 4)
+    want = np.linalg.norm(T @ X - b) / (np.linalg.norm(T) * np.linalg.norm(X) + np.linalg.norm(b))
+    got = residual.backward_error(p.E[0], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[0], p.Sigma_R[0],
+                                  p.Inj_first[0], p.Inj_last[0], X)
+    assert got == pytest.approx(want, rel=1e-10)
+    assert residual.backward_error(*args(p, 0), r["X"]) < 1e-14
+
+
+def test_config0_oracle_is_within_its_own_tolerances():
+    """BASELINE.json config 0: backward error of the oracle itself is far below the 1e-12 gate."""
+    p = inputs.make_problem(inputs.CONFIGS["C0"])
+    X, T = dense.solve_all(p)
+    assert X.shape == (4, 128, 4) and T.shape == (4,)
+    for e in range(4):
+        assert residual.backward_error(*args(p, e), X[e]) < 1e-14
+        assert 0.0 <= T[e] <= 16.0
+
+
+# --------------------------------------------------------------------------------------------
+# stored fixtures (tests/golden/, written by tests/golden/make_golden.py from oracle/ or a closed form)
+# --------------------------------------------------------------------------------------------
+def _golden(name):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)
+    return np.loadtxt(path, comments="#")
+
+
+def test_golden_impurity_chain_table():
+    tab = _golden("impurity_chain.txt")
+    p = inputs.perfect_chain_problem(1, 9, 7, t=-1.0)
+    p.H_diag[4, 0, 0] = 0.7
+    for e in range(7):
+        assert p.E[e].real == pytest.approx(tab[e, 0], abs=1e-15)
+        assert dense.solve_energy(*args(p, e))["T_LR"] == pytest.approx(tab[e, 1], rel=1e-12)
+
+
+def test_golden_config0_is_reproducible():
+    tab = _golden("c0_transmission.txt")
+    p = inputs.make_problem(inputs.CONFIGS["C0"])
+    X, T = dense.solve_all(p)
+    assert np.allclose(p.E.real, tab[:, 0], atol=1e-15) and np.allclose(p.E.imag, tab[:, 1], atol=1e-18)
+    assert np.allclose(T, tab[:, 2], rtol=1e-10)
+    assert np.allclose(np.linalg.norm(X, axis=(1, 2)), tab[:, 3], rtol=1e-10)
