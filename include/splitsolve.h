@@ -1,0 +1,168 @@
+/*
+ * libsplitsolve -- the GPU half of the SplitSolve algorithm (arxiv/paper_1812_01396, §3B,
+ * L125-175) for one NVIDIA B200 (sm_100a).  C ABI: plain pointers and sizes, no C++/torch types.
+ *
+ * For each energy point E the library solves the open-boundary Schroedinger equation (Eq. 5)
+ *
+ *        (E*S - H - Sigma_L - Sigma_R) * X = Inj ,
+ *
+ * H, S block tridiagonal with nb diagonal blocks of size bs x bs (L127), complex FP64 throughout:
+ *   pre-processing  (Alg. 1, and its mirror, L167): forward/backward block-Schur sweeps over
+ *                   A = E*S - H give Q_i = (A^-1)_{i,1} and P_i = (A^-1)_{i,nb}, i = 1..nb;
+ *   post-processing (L141-146, L148, L155, L175): R = 1 - C*[Q P] (2bs x 2bs corner system),
+ *                   w = R^-1 b',  X_i = Q_i w_top + P_i w_bot;
+ *   transmission    T(E) = Re Tr(Gamma_L G_1N Gamma_R G_1N^H), Gamma = i(Sigma - Sigma^H),
+ *                   G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22      (BASELINE.json north_star; L23, L85).
+ *
+ * Conventions
+ *   - ss_cplx is {double re, im}: identical to C99 `double _Complex`, numpy/torch complex128.
+ *   - All matrices are ROW-MAJOR (C-contiguous), dense, leading dimension = number of columns unless a
+ *     leading dimension argument says otherwise.  Blocks are 0-indexed in memory: H_diag[i] is the paper's
+ *     H_{i+1,i+1}; H_upper[i] is H_{i+1,i+2}.  The lower blocks are implied: H_{i+1,i} = H_{i,i+1}^H (L154),
+ *     and A_{i+1,i} = E*S_{i,i+1}^H - H_{i,i+1}^H with E NOT conjugated.
+ *   - Pointers named *_dev are CUDA device pointers (16-byte aligned), *_host are host pointers.
+ *     The caller owns every buffer it passes in.  Device inputs of ss_set_hamiltonian are BORROWED: they
+ *     must stay valid and unchanged while the handle uses them.  The handle owns its workspace.
+ *   - Every function returns an ss_status_t (except the pure queries); nothing throws or aborts.
+ *   - A handle is not thread-safe.  Device work is enqueued on the stream given to ss_solve (NULL = the
+ *     legacy default stream); ss_solve returns after enqueueing, results are complete after
+ *     ss_synchronize / ss_transmission or a synchronisation of that stream by the caller.
+ *   - Limits of this version: 2 <= nb, 1 <= bs <= 4096, 1 <= n_energy, 0 <= nrhs.
+ */
+#ifndef SPLITSOLVE_H
+#define SPLITSOLVE_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { double re, im; } ss_cplx;
+typedef struct ss_handle_s* ss_handle_t;
+
+typedef enum {
+    SS_OK = 0,
+    SS_ERR_INVALID_ARG = 1,   /* NULL pointer, size out of range */
+    SS_ERR_NOT_READY = 2,     /* ss_solve before ss_set_hamiltonian, ss_transmission before ss_solve */
+    SS_ERR_ALLOC = 3,         /* device or host allocation failed */
+    SS_ERR_SINGULAR = 4,      /* an exactly zero pivot was met; see ss_last_info */
+    SS_ERR_CUDA = 5           /* a CUDA runtime call or kernel launch failed */
+} ss_status_t;
+
+/* ---- life cycle -------------------------------------------------------------------------------------- */
+
+/* Creates a solver for nb diagonal blocks of size bs and up to n_energy energy points per ss_solve.
+ * Allocates nothing on the device yet (workspace is allocated lazily by the first ss_solve, when nrhs is
+ * known; see ss_workspace_bytes). */
+ss_status_t ss_create(int nb, int bs, int n_energy, ss_handle_t* out);
+
+/* Frees the handle and all device memory it owns.  NULL is allowed. */
+ss_status_t ss_destroy(ss_handle_t h);
+
+/* ---- inputs ------------------------------------------------------------------------------------------ */
+
+/* Registers H and S (resident in HBM, borrowed -- L184 "stored in their memory").
+ *   H_diag_dev, S_diag_dev   : [nb  ][bs][bs]
+ *   H_upper_dev, S_upper_dev : [nb-1][bs][bs]  = blocks (i, i+1) */
+ss_status_t ss_set_hamiltonian(ss_handle_t h, const ss_cplx* H_diag_dev, const ss_cplx* H_upper_dev,
+                               const ss_cplx* S_diag_dev, const ss_cplx* S_upper_dev);
+
+/* Same, from HOST buffers: the handle allocates device copies it owns and uploads (synchronous). */
+ss_status_t ss_set_hamiltonian_host(ss_handle_t h, const ss_cplx* H_diag_host, const ss_cplx* H_upper_host,
+                                    const ss_cplx* S_diag_host, const ss_cplx* S_upper_host);
+
+/* ---- the hot path ------------------------------------------------------------------------------------ */
+
+/* Solves all n_energy energy points.
+ *   E_host        : [n_energy] complex energies (host; copied before return)
+ *   Sigma_L_dev   : [n_energy][bs][bs]  boundary self-energy of the left contact  (top-left block of C, L148)
+ *   Sigma_R_dev   : [n_energy][bs][bs]  right contact (bottom-right block)
+ *   Inj_first_dev : [n_energy][bs][nrhs] non-zero rows of Inj in the first block row (L127); may be NULL iff nrhs==0
+ *   Inj_last_dev  : same for the last block row, or NULL = zeros
+ *   X_dev         : out [n_energy][nb*bs][nrhs]; may be NULL iff nrhs == 0
+ *   cuda_stream   : cudaStream_t (as void*), NULL = default stream.  All work is ordered after what is
+ *                   already enqueued on it and is complete when it drains.
+ * The sweep (a0-a4) reads neither Sigma nor Inj (pre-/post-processing split of L150-152).
+ * Errors: argument checks synchronously; a zero pivot is reported by ss_synchronize / ss_transmission. */
+ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L_dev, const ss_cplx* Sigma_R_dev,
+                     const ss_cplx* Inj_first_dev, const ss_cplx* Inj_last_dev, int nrhs, ss_cplx* X_dev,
+                     void* cuda_stream);
+
+/* Same with HOST buffers for everything (pageable or pinned): uploads Sigma/Inj into device buffers the
+ * handle owns, runs ss_solve on an internal stream, downloads X (may be NULL) and T (may be NULL), synchronises.
+ * Returns SS_ERR_SINGULAR if a pivot was exactly zero. */
+ss_status_t ss_solve_host(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L_host,
+                          const ss_cplx* Sigma_R_host, const ss_cplx* Inj_first_host, const ss_cplx* Inj_last_host,
+                          int nrhs, ss_cplx* X_host, double* T_host);
+
+/* Waits for the last ss_solve; returns SS_ERR_SINGULAR if any pivot was exactly zero. */
+ss_status_t ss_synchronize(ss_handle_t h);
+
+/* T_host: out [n_energy], T_LR(E) of the last ss_solve.  Synchronises. */
+ss_status_t ss_transmission(ss_handle_t h, double* T_host);
+
+/* ---- queries ----------------------------------------------------------------------------------------- */
+
+/* Borrowed device pointers to the inverse block columns of energy `energy` of the last ss_solve, each
+ * [nb][bs][bs]: Q_first[i] = (A^-1)_{i+1,1}, Q_last[i] = (A^-1)_{i+1,nb}.  Valid until the next ss_solve. */
+ss_status_t ss_inverse_columns(ss_handle_t h, int energy, const ss_cplx** Q_first_dev, const ss_cplx** Q_last_dev);
+
+/* Copies the same two block columns into caller-owned device buffers [nb][bs][bs] (either may be NULL),
+ * ordered on the stream of the last ss_solve. */
+ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cplx* Q_first_out_dev, ss_cplx* Q_last_out_dev);
+
+/* Location of the first exactly-zero pivot of the last ss_solve (-1s if none): energy index, 1-based block
+ * index i of Alg. 1 (0 = the corner system R), column 0 = first-column sweep / 1 = mirror sweep. Synchronises. */
+ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int* column);
+
+/* Closed-form flop count of steps a1-a7 per energy point (LAPACK convention: complex multiply-add = 8 flops;
+ * ZGEMM 8MNK, ZGETRF (8/3)n^3, ZTRSM 4n^2 nrhs).  ss_flops_sweep counts a1-a4 only: (160/3 nb - 32) bs^3. */
+double ss_flops(ss_handle_t h, int nrhs);
+double ss_flops_sweep(ss_handle_t h);
+
+/* Device bytes the handle allocates for (nb, bs, n_energy, nrhs), excluding caller-owned inputs/outputs. */
+size_t ss_workspace_bytes(int nb, int bs, int n_energy, int nrhs);
+
+/* Device time in milliseconds of the phases of the last ss_solve (CUDA events on its stream):
+ * phase 0 = sweep a0-a4, 1 = post-processing a5-a7, 2 = whole call.  Synchronises. */
+ss_status_t ss_phase_ms(ss_handle_t h, int phase, float* ms);
+
+/* Number of kernel launches the last ss_solve enqueued. */
+long long ss_launch_count(ss_handle_t h);
+
+/* Options: name in {"nb_lu" (outer LU block, 32..128, multiple of 16), "transmission" (0/1, default 1)}. */
+ss_status_t ss_set_option(ss_handle_t h, const char* name, int value);
+
+const char* ss_strerror(ss_status_t s);
+
+/* ---- building blocks (device pointers; the kernels the hot path is made of) ----------------------------- */
+
+/* Batched complex-FP64 GEMM on the FP64 tensor pipe (mma.sync f64):
+ *   C[z] = alpha * A[z] * B[z] + beta * C[z],  z = 0..batch-1,  A: M x K (lda), B: K x N (ldb), C: M x N (ldc),
+ * row-major, matrices of batch z at base + z*stride (elements).  alpha, beta real.  M, N, K >= 0. */
+ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const ss_cplx* A_dev, int lda, long long strideA,
+                             const ss_cplx* B_dev, int ldb, long long strideB, double beta, ss_cplx* C_dev, int ldc,
+                             long long strideC, int batch, void* cuda_stream);
+
+/* Batched blocked right-looking LU with partial pivoting (ZGETRF) of the leading n x n part of the
+ * n x ncols (ncols >= n, ld) row-major matrices AB[z]; the row interchanges and the L-solve are applied to
+ * the trailing ncols - n columns too (so that AB[:, n:] becomes L^-1 P B).  ipiv_dev: [batch][n] 0-based
+ * row indices (LAPACK semantics: row j was swapped with row ipiv[j]); info_dev: [batch], 0 or 1 + index of
+ * the first zero pivot.  n <= 8192. */
+ss_status_t ss_zgetrf_batched(int n, int ncols, ss_cplx* AB_dev, int ld, long long stride, int* ipiv_dev,
+                              int* info_dev, int batch, void* cuda_stream);
+
+/* Batched solve A X = B (ZGESV): LU as above on AB = [A | B] (n x (n + nrhs), ld), then blocked ZTRSM back
+ * substitution with the upper factor; X[z] (n x nrhs, ldx) at X_dev + z*strideX.  AB is overwritten. */
+ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB_dev, int ld, long long stride, ss_cplx* X_dev, int ldx,
+                             long long strideX, int* ipiv_dev, int* info_dev, int batch, void* cuda_stream);
+
+/* FP64 pipe microbenchmark (register-resident mma.sync.m8n8k4.f64 chains on all SMs): returns sustained
+ * TFLOP/s over about `ms` milliseconds; the measured roofline denominator bench.py prints beside the nominal one. */
+ss_status_t ss_fp64_peak_tflops(double ms, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPLITSOLVE_H */

@@ -1,0 +1,241 @@
+"""Thin ctypes binding of libsplitsolve (include/splitsolve.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  torch is used for device buffers and streams
+(`tensor.data_ptr()`, `torch.cuda.current_stream().cuda_stream`).  There is no CPU fallback: loading fails
+loudly when the shared library is missing.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_double, c_float, c_int, c_longlong, c_size_t, c_void_p
+
+PKG_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(PKG_DIR, "libsplitsolve.so")
+
+SS_OK, SS_ERR_INVALID_ARG, SS_ERR_NOT_READY, SS_ERR_ALLOC, SS_ERR_SINGULAR, SS_ERR_CUDA = range(6)
+
+# every symbol include/splitsolve.h declares: name -> (restype, argtypes)
+SIGNATURES = {
+    "ss_create": (c_int, [c_int, c_int, c_int, POINTER(c_void_p)]),
+    "ss_destroy": (c_int, [c_void_p]),
+    "ss_set_hamiltonian": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "ss_set_hamiltonian_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "ss_solve": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]),
+    "ss_solve_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]),
+    "ss_synchronize": (c_int, [c_void_p]),
+    "ss_transmission": (c_int, [c_void_p, c_void_p]),
+    "ss_inverse_columns": (c_int, [c_void_p, c_int, POINTER(c_void_p), POINTER(c_void_p)]),
+    "ss_copy_inverse_columns": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
+    "ss_last_info": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int), POINTER(c_int)]),
+    "ss_flops": (c_double, [c_void_p, c_int]),
+    "ss_flops_sweep": (c_double, [c_void_p]),
+    "ss_workspace_bytes": (c_size_t, [c_int, c_int, c_int, c_int]),
+    "ss_phase_ms": (c_int, [c_void_p, c_int, POINTER(c_float)]),
+    "ss_launch_count": (c_longlong, [c_void_p]),
+    "ss_set_option": (c_int, [c_void_p, c_char_p, c_int]),
+    "ss_strerror": (c_char_p, [c_int]),
+    "ss_zgemm_batched": (c_int, [c_int, c_int, c_int, c_double, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong,
+                                 c_double, c_void_p, c_int, c_longlong, c_int, c_void_p]),
+    "ss_zgetrf_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_void_p, c_int, c_void_p]),
+    "ss_zgesv_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong, c_void_p,
+                                 c_void_p, c_int, c_void_p]),
+    "ss_fp64_peak_tflops": (c_int, [c_double, POINTER(c_double)]),
+}
+
+_lib = None
+
+
+class SplitSolveError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = load().ss_strerror(status).decode() if _lib is not None else str(status)
+        super().__init__(f"{where}: {msg} (status {status})")
+
+
+def load() -> ctypes.CDLL:
+    """Loads libsplitsolve.so (built in-tree by build.py).  No fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1812_01396_b200.build` "
+                               "(the CUDA extension is required; there is no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(status: int, where: str):
+    if status != SS_OK:
+        raise SplitSolveError(status, where)
+
+
+def _dev(t, name):
+    import torch
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CUDA complex128 tensor")
+    return t.data_ptr()
+
+
+def _stream():
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+class SplitSolve:
+    """ss_create / ss_set_hamiltonian / ss_solve / ss_transmission with torch tensors as buffers."""
+
+    def __init__(self, nb: int, bs: int, n_energy: int):
+        self._h = c_void_p()
+        self.nb, self.bs, self.n_energy = nb, bs, n_energy
+        _check(load().ss_create(nb, bs, n_energy, byref(self._h)), "ss_create")
+        self._keep = []
+
+    def close(self):
+        if self._h:
+            load().ss_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, name: str, value: int):
+        _check(load().ss_set_option(self._h, name.encode(), int(value)), "ss_set_option")
+
+    def set_hamiltonian(self, H_diag, H_upper, S_diag, S_upper):
+        self._keep = [H_diag, H_upper, S_diag, S_upper]      # borrowed by the library: keep alive
+        _check(load().ss_set_hamiltonian(self._h, _dev(H_diag, "H_diag"), _dev(H_upper, "H_upper"),
+                                         _dev(S_diag, "S_diag"), _dev(S_upper, "S_upper")), "ss_set_hamiltonian")
+
+    def set_hamiltonian_host(self, H_diag, H_upper, S_diag, S_upper):
+        """Host buffers: numpy complex128 arrays or CPU torch tensors (C-contiguous)."""
+        _check(load().ss_set_hamiltonian_host(self._h, _host(H_diag), _host(H_upper), _host(S_diag), _host(S_upper)),
+               "ss_set_hamiltonian_host")
+
+    def solve(self, E, Sigma_L, Sigma_R, Inj_first, Inj_last=None, X=None):
+        """E: host complex128 (numpy / list); other arguments CUDA complex128 tensors. Returns X (enqueued)."""
+        import numpy as np
+        import torch
+        E = np.ascontiguousarray(np.asarray(E, dtype=np.complex128))
+        assert E.shape == (self.n_energy,)
+        nrhs = 0 if Inj_first is None else int(Inj_first.shape[-1])
+        if X is None and nrhs > 0:
+            X = torch.empty((self.n_energy, self.nb * self.bs, nrhs), dtype=torch.complex128, device=Sigma_L.device)
+        self._keep_solve = [Sigma_L, Sigma_R, Inj_first, Inj_last, X]
+        _check(load().ss_solve(self._h, E.ctypes.data, _dev(Sigma_L, "Sigma_L"), _dev(Sigma_R, "Sigma_R"),
+                               _dev(Inj_first, "Inj_first"), _dev(Inj_last, "Inj_last"), nrhs, _dev(X, "X"),
+                               _stream()), "ss_solve")
+        return X
+
+    def solve_host(self, E, Sigma_L, Sigma_R, Inj_first, Inj_last, X_out, T_out):
+        """All host buffers (numpy or pinned CPU torch tensors); blocking; H2D/D2H copies inside the call."""
+        import numpy as np
+        E = np.ascontiguousarray(np.asarray(E, dtype=np.complex128))
+        nrhs = 0 if Inj_first is None else int(Inj_first.shape[-1])
+        _check(load().ss_solve_host(self._h, E.ctypes.data, _host(Sigma_L), _host(Sigma_R), _host(Inj_first),
+                                    _host(Inj_last), nrhs, _host(X_out), _host(T_out)), "ss_solve_host")
+
+    def synchronize(self):
+        _check(load().ss_synchronize(self._h), "ss_synchronize")
+
+    def transmission(self):
+        import numpy as np
+        T = np.empty(self.n_energy, dtype=np.float64)
+        _check(load().ss_transmission(self._h, T.ctypes.data), "ss_transmission")
+        return T
+
+    def inverse_columns(self, energy: int):
+        """Copies of Q = (A^-1)[:, first block] and P = (A^-1)[:, last block], each [nb, bs, bs] (CUDA tensors)."""
+        import torch
+        Q = torch.empty((self.nb, self.bs, self.bs), dtype=torch.complex128, device="cuda")
+        P = torch.empty_like(Q)
+        _check(load().ss_copy_inverse_columns(self._h, energy, Q.data_ptr(), P.data_ptr()), "ss_copy_inverse_columns")
+        self.synchronize()
+        return Q, P
+
+    def last_info(self):
+        e, b, c = c_int(), c_int(), c_int()
+        _check(load().ss_last_info(self._h, byref(e), byref(b), byref(c)), "ss_last_info")
+        return e.value, b.value, c.value
+
+    def flops(self, nrhs: int) -> float:
+        return float(load().ss_flops(self._h, nrhs))
+
+    def flops_sweep(self) -> float:
+        return float(load().ss_flops_sweep(self._h))
+
+    def phase_ms(self, phase: int) -> float:
+        ms = c_float()
+        _check(load().ss_phase_ms(self._h, phase, byref(ms)), "ss_phase_ms")
+        return float(ms.value)
+
+    def launch_count(self) -> int:
+        return int(load().ss_launch_count(self._h))
+
+
+def _host(a):
+    if a is None:
+        return None
+    import numpy as np
+    try:
+        import torch
+        if isinstance(a, torch.Tensor):
+            assert not a.is_cuda and a.is_contiguous()
+            return a.data_ptr()
+    except ImportError:
+        pass
+    assert isinstance(a, np.ndarray) and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data
+
+
+def workspace_bytes(nb, bs, n_energy, nrhs) -> int:
+    return int(load().ss_workspace_bytes(nb, bs, n_energy, nrhs))
+
+
+def zgemm_batched(A, B, C, alpha=1.0, beta=0.0):
+    """C[z] = alpha A[z] B[z] + beta C[z]; A [batch,M,K], B [batch,K,N], C [batch,M,N] CUDA complex128."""
+    batch, M, K = A.shape
+    N = B.shape[2]
+    _check(load().ss_zgemm_batched(M, N, K, alpha, _dev(A, "A"), K, M * K, _dev(B, "B"), N, K * N, beta,
+                                   _dev(C, "C"), N, M * N, batch, _stream()), "ss_zgemm_batched")
+    return C
+
+
+def zgetrf_batched(AB, n):
+    """In-place LU of the leading n x n part of AB [batch, n, ncols]; returns (ipiv, info) int32 CUDA tensors."""
+    import torch
+    batch, rows, ncols = AB.shape
+    assert rows == n
+    ipiv = torch.zeros((batch, n), dtype=torch.int32, device=AB.device)
+    info = torch.zeros((batch,), dtype=torch.int32, device=AB.device)
+    _check(load().ss_zgetrf_batched(n, ncols, _dev(AB, "AB"), ncols, n * ncols, ipiv.data_ptr(), info.data_ptr(), batch,
+                                    _stream()), "ss_zgetrf_batched")
+    return ipiv, info
+
+
+def zgesv_batched(AB, n):
+    """Solves A X = B for AB = [A | B] [batch, n, n + nrhs] (overwritten); returns X [batch, n, nrhs], ipiv, info."""
+    import torch
+    batch, rows, ncols = AB.shape
+    nrhs = ncols - n
+    X = torch.empty((batch, n, nrhs), dtype=torch.complex128, device=AB.device)
+    ipiv = torch.zeros((batch, n), dtype=torch.int32, device=AB.device)
+    info = torch.zeros((batch,), dtype=torch.int32, device=AB.device)
+    _check(load().ss_zgesv_batched(n, nrhs, _dev(AB, "AB"), ncols, n * ncols, _dev(X, "X"), nrhs, n * nrhs,
+                                   ipiv.data_ptr(), info.data_ptr(), batch, _stream()), "ss_zgesv_batched")
+    return X, ipiv, info
+
+
+def fp64_peak_tflops(ms: float = 200.0) -> float:
+    out = c_double()
+    _check(load().ss_fp64_peak_tflops(ms, byref(out)), "ss_fp64_peak_tflops")
+    return float(out.value)

@@ -1,0 +1,571 @@
+// libsplitsolve: handle, workspace, the SplitSolve driver (Alg. 1 + mirror, post-processing, T(E)) and the C ABI
+// declared in include/splitsolve.h.  Only the CUDA runtime is linked: no cuBLAS / cuSOLVER / torch, no CPU fallback.
+#include "../../include/splitsolve.h"
+
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "sweep.cuh"
+#include "zgetrf.cuh"
+
+using namespace ss;
+
+struct ss_handle_s {
+    int nb = 0, bs = 0, n_energy = 0;
+    const cplx *Hd = nullptr, *Hu = nullptr, *Sd = nullptr, *Su = nullptr;
+    cplx* own_hs[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool have_h = false, solved = false;
+    // options
+    int nb_lu = 128;
+    int want_T = 1;
+    // workspace (allocated for ws_nrhs)
+    int ws_nrhs = -1;
+    cplx *slots = nullptr, *aug = nullptr, *aop = nullptr, *tinv = nullptr, *raug = nullptr, *wz = nullptr;
+    cplx *gam_l = nullptr, *gam_r = nullptr, *g1n = nullptr, *w1 = nullptr, *w2 = nullptr, *E_dev = nullptr;
+    double *tpart = nullptr, *T_dev = nullptr;
+    int *ipiv = nullptr, *info = nullptr;
+    int tinv_blocks_total = 0;
+    cplx* E_pinned = nullptr;
+    // host-path buffers
+    cplx *hp_sigl = nullptr, *hp_sigr = nullptr, *hp_inj1 = nullptr, *hp_inj2 = nullptr, *hp_x = nullptr;
+    int hp_nrhs = -1;
+    cudaStream_t own_stream = nullptr;
+    // last solve
+    cudaStream_t last_stream = nullptr;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    long long launches = 0;
+    int last_nrhs = 0;
+};
+
+static const int TRACE_PARTS = 592;   // 4 x 148 CTAs per energy for the trace reduction
+
+static inline long long cdiv(long long a, long long b) { return (a + b - 1) / b; }
+
+static void free_dev(void* p) { if (p) cudaFree(p); }
+
+static void free_workspace(ss_handle_t h) {
+    free_dev(h->slots); free_dev(h->aug); free_dev(h->aop); free_dev(h->tinv); free_dev(h->raug); free_dev(h->wz);
+    free_dev(h->gam_l); free_dev(h->gam_r); free_dev(h->g1n); free_dev(h->w1); free_dev(h->w2); free_dev(h->E_dev);
+    free_dev(h->tpart); free_dev(h->T_dev); free_dev(h->ipiv); free_dev(h->info);
+    h->slots = h->aug = h->aop = h->tinv = h->raug = h->wz = nullptr;
+    h->gam_l = h->gam_r = h->g1n = h->w1 = h->w2 = h->E_dev = nullptr;
+    h->tpart = h->T_dev = nullptr; h->ipiv = h->info = nullptr;
+    h->ws_nrhs = -1;
+}
+
+struct WsSizes {
+    size_t slots, aug, aop, tinv, raug, wz, sq, E, tpart, T, ipiv, info;
+    int tinv_blocks;
+    size_t total() const { return slots + aug + aop + tinv + raug + wz + 5 * sq + E + tpart + T + ipiv + info; }
+};
+
+static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
+    WsSizes w;
+    const size_t B2 = (size_t)bs * bs, C = sizeof(cplx);
+    w.slots = (size_t)nE * 2 * (nb + 1) * B2 * C;
+    w.aug = (size_t)nE * 2 * bs * 2 * bs * C;
+    w.aop = (size_t)nE * 2 * B2 * C;
+    int blk_sweep = 2 * nE * (int)cdiv(bs, 128), blk_corner = nE * (int)cdiv(2 * bs, 128);
+    w.tinv_blocks = blk_sweep > blk_corner ? blk_sweep : blk_corner;
+    w.tinv = (size_t)w.tinv_blocks * 128 * 128 * C;
+    const size_t W = (size_t)3 * bs + nrhs;
+    w.raug = (size_t)nE * 2 * bs * W * C;
+    w.wz = (size_t)nE * 2 * bs * ((size_t)nrhs + bs) * C;
+    w.sq = (size_t)nE * B2 * C;
+    w.E = (size_t)nE * C;
+    w.tpart = (size_t)nE * TRACE_PARTS * sizeof(double);
+    w.T = (size_t)nE * sizeof(double);
+    w.ipiv = (size_t)3 * nE * 2 * bs * sizeof(int);
+    w.info = (size_t)3 * nE * sizeof(int);
+    return w;
+}
+
+static ss_status_t ensure_workspace(ss_handle_t h, int nrhs) {
+    if (h->ws_nrhs >= nrhs) return SS_OK;
+    free_workspace(h);
+    WsSizes w = ws_sizes(h->nb, h->bs, h->n_energy, nrhs);
+    bool ok = true;
+    auto A = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 16) != cudaSuccess) ok = false; };
+    A((void**)&h->slots, w.slots); A((void**)&h->aug, w.aug); A((void**)&h->aop, w.aop); A((void**)&h->tinv, w.tinv);
+    A((void**)&h->raug, w.raug); A((void**)&h->wz, w.wz);
+    A((void**)&h->gam_l, w.sq); A((void**)&h->gam_r, w.sq); A((void**)&h->g1n, w.sq); A((void**)&h->w1, w.sq);
+    A((void**)&h->w2, w.sq); A((void**)&h->E_dev, w.E); A((void**)&h->tpart, w.tpart); A((void**)&h->T_dev, w.T);
+    A((void**)&h->ipiv, w.ipiv); A((void**)&h->info, w.info);
+    if (!ok) { cudaGetLastError(); free_workspace(h); return SS_ERR_ALLOC; }
+    h->tinv_blocks_total = w.tinv_blocks;
+    h->ws_nrhs = nrhs;
+    return SS_OK;
+}
+
+extern "C" size_t ss_workspace_bytes(int nb, int bs, int n_energy, int nrhs) {
+    if (nb < 2 || bs < 1 || n_energy < 1 || nrhs < 0) return 0;
+    return ws_sizes(nb, bs, n_energy, nrhs).total();
+}
+
+extern "C" const char* ss_strerror(ss_status_t s) {
+    switch (s) {
+        case SS_OK: return "ok";
+        case SS_ERR_INVALID_ARG: return "invalid argument";
+        case SS_ERR_NOT_READY: return "not ready (call order)";
+        case SS_ERR_ALLOC: return "allocation failed";
+        case SS_ERR_SINGULAR: return "exactly zero pivot";
+        case SS_ERR_CUDA: return "CUDA error";
+    }
+    return "unknown status";
+}
+
+extern "C" ss_status_t ss_create(int nb, int bs, int n_energy, ss_handle_t* out) {
+    if (!out) return SS_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (nb < 2 || bs < 1 || bs > 4096 || n_energy < 1) return SS_ERR_INVALID_ARG;
+    ss_handle_t h = new (std::nothrow) ss_handle_s();
+    if (!h) return SS_ERR_ALLOC;
+    h->nb = nb; h->bs = bs; h->n_energy = n_energy;
+    for (int i = 0; i < 3; i++)
+        if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { cudaGetLastError(); delete h; return SS_ERR_CUDA; }
+    if (cudaMallocHost((void**)&h->E_pinned, sizeof(cplx) * (size_t)n_energy) != cudaSuccess) {
+        cudaGetLastError(); delete h; return SS_ERR_ALLOC;
+    }
+    *out = h;
+    return SS_OK;
+}
+
+static void free_host_path(ss_handle_t h) {
+    free_dev(h->hp_sigl); free_dev(h->hp_sigr); free_dev(h->hp_inj1); free_dev(h->hp_inj2); free_dev(h->hp_x);
+    h->hp_sigl = h->hp_sigr = h->hp_inj1 = h->hp_inj2 = h->hp_x = nullptr;
+    h->hp_nrhs = -1;
+}
+
+extern "C" ss_status_t ss_destroy(ss_handle_t h) {
+    if (!h) return SS_OK;
+    cudaDeviceSynchronize();
+    free_workspace(h);
+    free_host_path(h);
+    for (int i = 0; i < 4; i++) free_dev(h->own_hs[i]);
+    for (int i = 0; i < 3; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    if (h->E_pinned) cudaFreeHost(h->E_pinned);
+    if (h->own_stream) cudaStreamDestroy(h->own_stream);
+    delete h;
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_set_hamiltonian(ss_handle_t h, const ss_cplx* Hd, const ss_cplx* Hu, const ss_cplx* Sd,
+                                          const ss_cplx* Su) {
+    if (!h || !Hd || !Hu || !Sd || !Su) return SS_ERR_INVALID_ARG;
+    h->Hd = (const cplx*)Hd; h->Hu = (const cplx*)Hu; h->Sd = (const cplx*)Sd; h->Su = (const cplx*)Su;
+    h->have_h = true; h->solved = false;
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_set_hamiltonian_host(ss_handle_t h, const ss_cplx* Hd, const ss_cplx* Hu, const ss_cplx* Sd,
+                                               const ss_cplx* Su) {
+    if (!h || !Hd || !Hu || !Sd || !Su) return SS_ERR_INVALID_ARG;
+    const size_t B2 = (size_t)h->bs * h->bs * sizeof(cplx);
+    const size_t bytes[4] = {B2 * h->nb, B2 * (h->nb - 1), B2 * h->nb, B2 * (h->nb - 1)};
+    const ss_cplx* src[4] = {Hd, Hu, Sd, Su};
+    for (int i = 0; i < 4; i++) {
+        if (!h->own_hs[i] && cudaMalloc((void**)&h->own_hs[i], bytes[i]) != cudaSuccess) {
+            cudaGetLastError(); return SS_ERR_ALLOC;
+        }
+        if (cudaMemcpy(h->own_hs[i], src[i], bytes[i], cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError(); return SS_ERR_CUDA;
+        }
+    }
+    return ss_set_hamiltonian(h, (ss_cplx*)h->own_hs[0], (ss_cplx*)h->own_hs[1], (ss_cplx*)h->own_hs[2],
+                              (ss_cplx*)h->own_hs[3]);
+}
+
+extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value) {
+    if (!h || !name) return SS_ERR_INVALID_ARG;
+    if (!strcmp(name, "nb_lu")) {
+        if (value < 16 || value > 128 || value % 16) return SS_ERR_INVALID_ARG;
+        h->nb_lu = value; return SS_OK;
+    }
+    if (!strcmp(name, "transmission")) { h->want_T = value ? 1 : 0; return SS_OK; }
+    return SS_ERR_INVALID_ARG;
+}
+
+extern "C" double ss_flops_sweep(ss_handle_t h) {
+    if (!h) return 0.0;
+    double bs3 = (double)h->bs * h->bs * h->bs;
+    return (160.0 / 3.0 * h->nb - 32.0) * bs3;
+}
+
+extern "C" double ss_flops(ss_handle_t h, int nrhs) {
+    if (!h || nrhs < 0) return 0.0;
+    const double bs = h->bs, nb = h->nb, m = nrhs;
+    const double bs3 = bs * bs * bs;
+    double sweep = (160.0 / 3.0 * nb - 32.0) * bs3;
+    // a5: 4 GEMM (32 bs^3) + ZGETRF(2bs) (64/3 bs^3) + 2 ZTRSM with m rhs (2 * 4 (2bs)^2 m = 32 bs^2 m)
+    double a5 = 32.0 * bs3 + 64.0 / 3.0 * bs3 + 32.0 * bs * bs * m;
+    double a6 = 16.0 * nb * bs * bs * m;
+    // a7: R^-1[:, bs:] (2 ZTRSM with bs rhs: 32 bs^3) + G (16 bs^3) + two Gamma products (16 bs^3) + trace (8 bs^2)
+    double a7 = h->want_T ? (64.0 * bs3 + 8.0 * bs * bs) : 0.0;
+    return sweep + a5 + a6 + a7;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// the hot path
+// ---------------------------------------------------------------------------------------------------------
+static void launch_form(Ctx& ctx, FormSide s0, FormSide s1, const cplx* E, BPtr dst, int ld, int bs, int batch) {
+    dim3 grid((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)batch);
+    form_kernel<<<grid, 256, 0, ctx.st>>>(s0, s1, E, dst, ld, bs);
+    ctx.note(cudaGetLastError());
+}
+
+// a0-a4: Algorithm 1 and its mirror (L167), all energies and both columns in lockstep.
+// Chain z = 2*e + col.  Slot layout per chain (nb+1 slots of bs x bs): column 0 keeps X_i in slot i (X_1 in slot 0)
+// and ends with Q_i in slot i-1; column 1 keeps Y_i in slot i-1 (Y_nb in slot nb) and ends with P_i in slot i.
+static void run_sweep(ss_handle_t h, Ctx& ctx) {
+    const int nb = h->nb, bs = h->bs, nE = h->n_energy, batch = 2 * nE;
+    const long long B2 = (long long)bs * bs;
+    const long long s_slot_e = 2LL * (nb + 1) * B2;
+    auto slot = [&](int col, int idx) { return h->slots + ((long long)col * (nb + 1) + idx) * B2; };
+    const int ldg = 2 * bs;
+    const BPtr aug = bp_chain(h->aug, h->aug + (long long)bs * ldg, 2LL * bs * ldg);
+    const BPtr aop = bp_chain(h->aop, h->aop + B2, 2 * B2);
+    LuWork w;
+    w.tinv = h->tinv; w.tinv_blocks = h->tinv_blocks_total; w.ipiv = h->ipiv; w.ipiv_stride = 2 * bs; w.info = h->info;
+    const int info_stride = 2 * bs + 2;
+
+    for (int s = 0; s < nb; s++) {
+        const int i_f = nb - s, i_m = s + 1;                       // 1-based block index of each chain
+        // right-hand sides: A_{i,i-1} (column 0) / A_{i,i+1} (column 1); identity at the ends (L164, reading c1)
+        FormSide r0 = (i_f > 1) ? FormSide{h->Su + (long long)(i_f - 2) * B2, h->Hu + (long long)(i_f - 2) * B2, FORM_CONJT}
+                                : FormSide{nullptr, nullptr, FORM_IDENT};
+        FormSide r1 = (i_m < nb) ? FormSide{h->Su + (long long)(i_m - 1) * B2, h->Hu + (long long)(i_m - 1) * B2, FORM_PLAIN}
+                                 : FormSide{nullptr, nullptr, FORM_IDENT};
+        launch_form(ctx, r0, r1, h->E_dev, bp_offset(aug, bs), ldg, bs, batch);
+        GemmArgs g{};
+        g.M = bs; g.N = bs; g.K = 0;
+        g.A = aop; g.lda = bs; g.B = aop; g.ldb = bs;
+        if (s > 0) {
+            // left operands: A_{i,i+1} (column 0) / A_{i,i-1} (column 1)
+            FormSide a0{h->Su + (long long)(i_f - 1) * B2, h->Hu + (long long)(i_f - 1) * B2, FORM_PLAIN};
+            FormSide a1{h->Su + (long long)(i_m - 2) * B2, h->Hu + (long long)(i_m - 2) * B2, FORM_CONJT};
+            launch_form(ctx, a0, a1, h->E_dev, aop, bs, bs, batch);
+            g.K = bs;
+            g.B = bp_chain(slot(0, i_f + 1), slot(1, i_m - 2), s_slot_e);   // X_{i+1} / Y_{i-1}
+        }
+        // a1 (+ a0 for the diagonal block, fused in the epilogue): D = E S_ii - H_ii - A_op * X_prev
+        g.C = aug; g.ldc = ldg; g.Cin = aug; g.ldcin = ldg; g.alpha = 1.0; g.beta = 0.0;
+        g.S = bp_chain(h->Sd + (long long)(i_f - 1) * B2, h->Sd + (long long)(i_m - 1) * B2, 0);
+        g.H = bp_chain(h->Hd + (long long)(i_f - 1) * B2, h->Hd + (long long)(i_m - 1) * B2, 0);
+        g.lds = bs; g.E = h->E_dev;
+        ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_SCHUR, ctx.st));
+        // a2 + the L half of a3
+        lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, h->nb_lu, w, s * info_stride);
+        // U half of a3: X_i / Y_i into its slot
+        BPtr out = bp_chain(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
+        back_substitute(ctx, aug, ldg, bs, bs, out, bs, batch, w);
+    }
+    // a4: Q_i = -X_i Q_{i-1} (i = 2..nb), P_i = -Y_i P_{i+1} (i = nb-1..1)
+    for (int r = 1; r < nb; r++) {
+        const int i0 = r + 1, i1 = nb - r;
+        GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_chain(slot(0, i0), slot(1, i1 - 1), s_slot_e), bs,
+                              bp_chain(slot(0, i0 - 2), slot(1, i1 + 1), s_slot_e), bs, 0.0,
+                              bp_chain(slot(0, i0 - 1), slot(1, i1), s_slot_e), bs);
+        ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_STD, ctx.st));
+    }
+}
+
+// a5-a7: corner system, solution, transmission (north_star for T).
+static void run_post(ss_handle_t h, Ctx& ctx, const cplx* SigL, const cplx* SigR, const cplx* inj1, const cplx* inj2,
+                     int m, cplx* X) {
+    const int nb = h->nb, bs = h->bs, nE = h->n_energy;
+    const long long B2 = (long long)bs * bs;
+    const long long s_slot_e = 2LL * (nb + 1) * B2;
+    auto slot = [&](int col, int idx) { return h->slots + ((long long)col * (nb + 1) + idx) * B2; };
+    const int zc = h->want_T ? bs : 0;                // columns of e_2 (for (R^-1)_{12}, (R^-1)_{22})
+    const int W = 2 * bs + m + zc;
+    const int nr = m + zc;
+    const long long s_r = 2LL * bs * W, s_w = 2LL * bs * nr;
+    {
+        dim3 grid((unsigned)min((long long)8, cdiv(W, 256)), (unsigned)(2 * bs), (unsigned)nE);
+        corner_init_kernel<<<grid, 256, 0, ctx.st>>>(h->raug, s_r, W, bs, m, inj1, inj2);
+        ctx.note(cudaGetLastError());
+    }
+    // R = 1 - C [Q P]:  R11 -= Sigma_L Q_1, R12 -= Sigma_L P_1, R21 -= Sigma_R Q_nb, R22 -= Sigma_R P_nb
+    const cplx* sig[2] = {SigL, SigR};
+    for (int br = 0; br < 2; br++)
+        for (int bc = 0; bc < 2; bc++) {
+            const cplx* Bsrc = (bc == 0) ? slot(0, br == 0 ? 0 : nb - 1) : slot(1, br == 0 ? 1 : nb);
+            GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(Bsrc, s_slot_e), bs, 1.0,
+                                  bp_strided(h->raug + (long long)br * bs * W + (long long)bc * bs, s_r), W);
+            ctx.note(gemm_launch(g, nE, GEMM_BIG, EPI_STD, ctx.st));
+        }
+    LuWork w;
+    w.tinv = h->tinv; w.tinv_blocks = h->tinv_blocks_total;
+    w.ipiv = h->ipiv + (long long)2 * nE * 2 * bs; w.ipiv_stride = 2 * bs; w.info = h->info + 2 * nE;
+    lu_factor(ctx, bp_strided(h->raug, s_r), W, 2 * bs, W, nE, h->nb_lu, w, 0);
+    back_substitute(ctx, bp_strided(h->raug, s_r), W, 2 * bs, nr, bp_strided(h->wz, s_w), nr, nE, w);
+    // a6: X_i = Q_i w_top + P_i w_bot, batch z = e*nb + (i-1)
+    if (m > 0) {
+        GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(0, 0), nb, B2, s_slot_e), bs,
+                              bp_two_level(h->wz, nb, 0, s_w), nr, 0.0,
+                              bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
+        ctx.note(gemm_launch(g, nE * nb, GEMM_BIG, EPI_STD, ctx.st));
+        GemmArgs g2 = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(1, 1), nb, B2, s_slot_e), bs,
+                               bp_two_level(h->wz + (long long)bs * nr, nb, 0, s_w), nr, 1.0,
+                               bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
+        ctx.note(gemm_launch(g2, nE * nb, GEMM_BIG, EPI_STD, ctx.st));
+    }
+    // a7: G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22;  T = Re Tr(Gamma_L G Gamma_R G^H)
+    if (h->want_T) {
+        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(0, 0), s_slot_e), bs, bp_strided(h->wz + m, s_w), nr, 0.0,
+                              bp_strided(h->g1n, B2), bs);
+        ctx.note(gemm_launch(g, nE, GEMM_BIG, EPI_STD, ctx.st));
+        GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(1, 1), s_slot_e), bs,
+                               bp_strided(h->wz + (long long)bs * nr + m, s_w), nr, 1.0, bp_strided(h->g1n, B2), bs);
+        ctx.note(gemm_launch(g2, nE, GEMM_BIG, EPI_STD, ctx.st));
+        dim3 gg((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)nE);
+        gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigL, h->gam_l, bs); ctx.note(cudaGetLastError());
+        gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigR, h->gam_r, bs); ctx.note(cudaGetLastError());
+        GemmArgs g3 = gemm_std(bs, bs, bs, 1.0, bp_strided(h->gam_l, B2), bs, bp_strided(h->g1n, B2), bs, 0.0,
+                               bp_strided(h->w1, B2), bs);
+        ctx.note(gemm_launch(g3, nE, GEMM_BIG, EPI_STD, ctx.st));
+        GemmArgs g4 = gemm_std(bs, bs, bs, 1.0, bp_strided(h->w1, B2), bs, bp_strided(h->gam_r, B2), bs, 0.0,
+                               bp_strided(h->w2, B2), bs);
+        ctx.note(gemm_launch(g4, nE, GEMM_BIG, EPI_STD, ctx.st));
+        int parts = (int)min((long long)TRACE_PARTS, cdiv(B2, 256));
+        trace_partial_kernel<<<dim3((unsigned)parts, (unsigned)nE), 256, 0, ctx.st>>>(h->w2, h->g1n, B2, B2, h->tpart);
+        ctx.note(cudaGetLastError());
+        trace_final_kernel<<<nE, 32, 0, ctx.st>>>(h->tpart, parts, h->T_dev);
+        ctx.note(cudaGetLastError());
+    }
+}
+
+extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L, const ss_cplx* Sigma_R,
+                                const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs, ss_cplx* X,
+                                void* cuda_stream) {
+    if (!h || !E_host || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
+    if (nrhs > 0 && (!Inj_first || !X)) return SS_ERR_INVALID_ARG;
+    if (!h->have_h) return SS_ERR_NOT_READY;
+    ss_status_t st = ensure_workspace(h, nrhs);
+    if (st != SS_OK) return st;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (h->solved) cudaEventSynchronize(h->ev[2]);        // E_pinned of the previous call is free again
+    memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
+    Ctx ctx; ctx.st = stream;
+    if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
+        cudaMemsetAsync(h->info, 0, sizeof(int) * 3 * (size_t)h->n_energy, stream) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    cudaEventRecord(h->ev[0], stream);
+    run_sweep(h, ctx);
+    cudaEventRecord(h->ev[1], stream);
+    run_post(h, ctx, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first, (const cplx*)Inj_last, nrhs, (cplx*)X);
+    cudaEventRecord(h->ev[2], stream);
+    h->launches = ctx.launches;
+    h->last_stream = stream;
+    h->last_nrhs = nrhs;
+    h->solved = true;
+    if (ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
+static ss_status_t check_info(ss_handle_t h) {
+    const int n = 3 * h->n_energy;
+    int* host = (int*)malloc(sizeof(int) * (size_t)n);
+    if (!host) return SS_ERR_ALLOC;
+    cudaError_t e = cudaMemcpy(host, h->info, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost);
+    ss_status_t st = SS_OK;
+    if (e != cudaSuccess) { cudaGetLastError(); st = SS_ERR_CUDA; }
+    else for (int i = 0; i < n; i++) if (host[i] != 0) { st = SS_ERR_SINGULAR; break; }
+    free(host);
+    return st;
+}
+
+extern "C" ss_status_t ss_synchronize(ss_handle_t h) {
+    if (!h) return SS_ERR_INVALID_ARG;
+    if (!h->solved) return SS_ERR_NOT_READY;
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return check_info(h);
+}
+
+extern "C" ss_status_t ss_transmission(ss_handle_t h, double* T_host) {
+    if (!h || !T_host) return SS_ERR_INVALID_ARG;
+    if (!h->solved || !h->want_T) return SS_ERR_NOT_READY;
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (cudaMemcpy(T_host, h->T_dev, sizeof(double) * (size_t)h->n_energy, cudaMemcpyDeviceToHost) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    return check_info(h);
+}
+
+extern "C" ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int* column) {
+    if (!h || !energy || !block || !column) return SS_ERR_INVALID_ARG;
+    if (!h->solved) return SS_ERR_NOT_READY;
+    *energy = *block = *column = -1;
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    const int nE = h->n_energy, n = 3 * nE;
+    int* host = (int*)malloc(sizeof(int) * (size_t)n);
+    if (!host) return SS_ERR_ALLOC;
+    if (cudaMemcpy(host, h->info, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost) != cudaSuccess) {
+        cudaGetLastError(); free(host); return SS_ERR_CUDA;
+    }
+    const int info_stride = 2 * h->bs + 2;
+    for (int i = 0; i < n; i++) {
+        if (!host[i]) continue;
+        if (i < 2 * nE) {
+            int s = (host[i] - 1) / info_stride;
+            *energy = i >> 1; *column = i & 1;
+            *block = (i & 1) ? s + 1 : h->nb - s;
+        } else {
+            *energy = i - 2 * nE; *column = -1; *block = 0;
+        }
+        break;
+    }
+    free(host);
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_inverse_columns(ss_handle_t h, int energy, const ss_cplx** Q_first, const ss_cplx** Q_last) {
+    if (!h || !Q_first || !Q_last || energy < 0 || energy >= h->n_energy) return SS_ERR_INVALID_ARG;
+    if (!h->solved) return SS_ERR_NOT_READY;
+    const long long B2 = (long long)h->bs * h->bs;
+    const cplx* base = h->slots + (long long)energy * 2 * (h->nb + 1) * B2;
+    *Q_first = (const ss_cplx*)base;                                   // column 0, slots 0..nb-1
+    *Q_last = (const ss_cplx*)(base + (long long)(h->nb + 1) * B2 + B2);   // column 1, slots 1..nb
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cplx* Q_out, ss_cplx* P_out) {
+    const ss_cplx *q = nullptr, *p = nullptr;
+    ss_status_t s = ss_inverse_columns(h, energy, &q, &p);
+    if (s != SS_OK) return s;
+    const size_t bytes = sizeof(cplx) * (size_t)h->nb * h->bs * h->bs;
+    if (Q_out && cudaMemcpyAsync(Q_out, q, bytes, cudaMemcpyDeviceToDevice, h->last_stream) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    if (P_out && cudaMemcpyAsync(P_out, p, bytes, cudaMemcpyDeviceToDevice, h->last_stream) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_phase_ms(ss_handle_t h, int phase, float* ms) {
+    if (!h || !ms || phase < 0 || phase > 2) return SS_ERR_INVALID_ARG;
+    if (!h->solved) return SS_ERR_NOT_READY;
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    cudaError_t e = (phase == 0) ? cudaEventElapsedTime(ms, h->ev[0], h->ev[1])
+                  : (phase == 1) ? cudaEventElapsedTime(ms, h->ev[1], h->ev[2])
+                                 : cudaEventElapsedTime(ms, h->ev[0], h->ev[2]);
+    if (e != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
+extern "C" long long ss_launch_count(ss_handle_t h) { return h ? h->launches : 0; }
+
+extern "C" ss_status_t ss_solve_host(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* SigL, const ss_cplx* SigR,
+                                     const ss_cplx* Inj1, const ss_cplx* Inj2, int nrhs, ss_cplx* X_host, double* T_host) {
+    if (!h || !E_host || !SigL || !SigR || nrhs < 0 || (nrhs > 0 && !Inj1)) return SS_ERR_INVALID_ARG;
+    if (!h->have_h) return SS_ERR_NOT_READY;
+    const size_t C = sizeof(cplx), B2 = (size_t)h->bs * h->bs, nE = h->n_energy;
+    const size_t inj_bytes = nE * h->bs * (size_t)nrhs * C, x_bytes = nE * (size_t)h->nb * h->bs * nrhs * C;
+    if (!h->own_stream && cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    if (h->hp_nrhs < nrhs) {
+        free_host_path(h);
+        bool ok = cudaMalloc((void**)&h->hp_sigl, nE * B2 * C) == cudaSuccess && cudaMalloc((void**)&h->hp_sigr, nE * B2 * C) == cudaSuccess &&
+                  cudaMalloc((void**)&h->hp_inj1, inj_bytes ? inj_bytes : 16) == cudaSuccess &&
+                  cudaMalloc((void**)&h->hp_inj2, inj_bytes ? inj_bytes : 16) == cudaSuccess &&
+                  cudaMalloc((void**)&h->hp_x, x_bytes ? x_bytes : 16) == cudaSuccess;
+        if (!ok) { cudaGetLastError(); free_host_path(h); return SS_ERR_ALLOC; }
+        h->hp_nrhs = nrhs;
+    }
+    cudaStream_t st = h->own_stream;
+    bool ok = cudaMemcpyAsync(h->hp_sigl, SigL, nE * B2 * C, cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemcpyAsync(h->hp_sigr, SigR, nE * B2 * C, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    if (ok && nrhs > 0) ok = cudaMemcpyAsync(h->hp_inj1, Inj1, inj_bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    if (ok && nrhs > 0 && Inj2) ok = cudaMemcpyAsync(h->hp_inj2, Inj2, inj_bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); return SS_ERR_CUDA; }
+    ss_status_t s = ss_solve(h, E_host, (ss_cplx*)h->hp_sigl, (ss_cplx*)h->hp_sigr, nrhs ? (ss_cplx*)h->hp_inj1 : nullptr,
+                             (nrhs && Inj2) ? (ss_cplx*)h->hp_inj2 : nullptr, nrhs, nrhs ? (ss_cplx*)h->hp_x : nullptr, st);
+    if (s != SS_OK) return s;
+    if (X_host && nrhs > 0 && cudaMemcpyAsync(X_host, h->hp_x, x_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    if (T_host && h->want_T && cudaMemcpyAsync(T_host, h->T_dev, sizeof(double) * nE, cudaMemcpyDeviceToHost, st) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return check_info(h);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// building blocks
+// ---------------------------------------------------------------------------------------------------------
+extern "C" ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const ss_cplx* A, int lda, long long sA,
+                                        const ss_cplx* B, int ldb, long long sB, double beta, ss_cplx* C, int ldc,
+                                        long long sC, int batch, void* stream) {
+    if (M < 0 || N < 0 || K < 0 || batch < 0 || !C || (K > 0 && (!A || !B))) return SS_ERR_INVALID_ARG;
+    if (lda < K || ldb < N || ldc < N) return SS_ERR_INVALID_ARG;
+    GemmArgs g = gemm_std(M, N, K, alpha, bp_strided((const cplx*)(A ? A : C), sA), lda, bp_strided((const cplx*)(B ? B : C), sB), ldb,
+                          beta, bp_strided((cplx*)C, sC), ldc);
+    cudaError_t e = gemm_launch(g, batch, GEMM_BIG, EPI_STD, (cudaStream_t)stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
+static ss_status_t lu_common(int n, int nrhs_solve, int ncols, ss_cplx* AB, int ld, long long stride, ss_cplx* X, int ldx,
+                             long long sX, int* ipiv, int* info, int batch, void* stream) {
+    if (n < 1 || n > LEAF_TPB * LEAF_MAXC || ncols < n || ld < ncols || batch < 1 || !AB || !ipiv || !info)
+        return SS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    LuWork w;
+    const int nblk = (int)cdiv(n, 128);
+    if (cudaMalloc((void**)&w.tinv, sizeof(cplx) * 128 * 128 * (size_t)nblk * batch) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_ALLOC;
+    }
+    w.tinv_blocks = nblk * batch; w.ipiv = ipiv; w.ipiv_stride = n; w.info = info;
+    Ctx ctx; ctx.st = st;
+    cudaMemsetAsync(info, 0, sizeof(int) * (size_t)batch, st);
+    BPtr Ab = bp_strided((cplx*)AB, stride);
+    lu_factor(ctx, Ab, ld, n, ncols, batch, 128, w, 0);
+    if (nrhs_solve > 0) back_substitute(ctx, Ab, ld, n, nrhs_solve, bp_strided((cplx*)X, sX), ldx, batch, w);
+    cudaError_t e = cudaStreamSynchronize(st);
+    cudaFree(w.tinv);
+    if (e != cudaSuccess || ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_zgetrf_batched(int n, int ncols, ss_cplx* AB, int ld, long long stride, int* ipiv, int* info,
+                                         int batch, void* stream) {
+    return lu_common(n, 0, ncols, AB, ld, stride, nullptr, 0, 0, ipiv, info, batch, stream);
+}
+
+extern "C" ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB, int ld, long long stride, ss_cplx* X, int ldx,
+                                        long long sX, int* ipiv, int* info, int batch, void* stream) {
+    if (nrhs < 0 || (nrhs > 0 && (!X || ldx < nrhs))) return SS_ERR_INVALID_ARG;
+    return lu_common(n, nrhs, n + nrhs, AB, ld, stride, X, ldx, sX, ipiv, info, batch, stream);
+}
+
+extern "C" ss_status_t ss_fp64_peak_tflops(double ms, double* tflops) {
+    if (!tflops || ms <= 0) return SS_ERR_INVALID_ARG;
+    int dev = 0, nsm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    double* out = nullptr;
+    if (cudaMalloc((void**)&out, 64) != cudaSuccess) { cudaGetLastError(); return SS_ERR_ALLOC; }
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = nsm * 4, iters = 20000;           // 16 warps per SM, 8 independent DMMA chains each
+    const double fl_per_launch = 2.0 * 8 * 8 * 4 * 8 * (double)iters * blocks * 4;
+    fp64_peak_kernel<<<blocks, 128>>>(out, iters);
+    cudaDeviceSynchronize();
+    double best = 0.0, spent = 0.0;
+    while (spent < ms) {
+        cudaEventRecord(e0); fp64_peak_kernel<<<blocks, 128>>>(out, iters); cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float t = 0.f; cudaEventElapsedTime(&t, e0, e1);
+        spent += t;
+        double tf = fl_per_launch / (t * 1e-3) * 1e-12;
+        if (tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+    if (cudaGetLastError() != cudaSuccess) return SS_ERR_CUDA;
+    *tflops = best;
+    return SS_OK;
+}

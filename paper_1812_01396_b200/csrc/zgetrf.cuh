@@ -1,0 +1,428 @@
+// Batched blocked right-looking ZGETRF with partial pivoting + blocked ZTRSM back substitution (sm_100a).
+//
+// "Solve (A_ii - A_{i,i+1} X_{i+1}) X_i = A_{i,i-1}" of Algorithm 1;
+// the paper used MAGMA zgesv_nopiv_gpu (L186) and names "the LU factorization and backward substitution"
+// as the bottleneck (L266).  Here: partial pivoting (north_star), everything on the GPU, batched over all
+// independent chains (energies x {first, last} column, L167/L204), and organised so that all O(n^3) work is
+// DMMA GEMM (zgemm.cuh):
+//
+//   LU of the augmented matrix [D | B] (n x ncols, row-major): the row interchanges and the L-solve are applied
+//   to B by the same trailing updates, so only the U-solve remains afterwards.
+//     outer block NB (<=128):  panel (inner blocks of JB=16 columns)  ->  L11^-1 (trtri)  ->  U12 = L11^-1 A12 (GEMM,
+//     in place, one CTA owns all rows of its columns)  ->  A22 -= L21 U12 (GEMM).
+//     inner block JB=16:  leaf panel kernel  ->  row swaps on all other columns  ->  16 x w triangular solve  ->
+//     rank-16 GEMM update of the rest of the panel.
+//   Leaf panel kernel: one thread owns one matrix ROW of the 16-column panel in registers; one thread-block
+//   cluster (<=16 CTAs x 512 threads, up to 8192 rows) per matrix.  Per column: warp-shuffle arg-max, CTA
+//   candidate through shared memory, candidates + candidate rows exchanged through DISTRIBUTED shared memory,
+//   one cluster barrier, rank-1 update in registers.  Pivoting is implicit (no data moves until the final
+//   store), bookkeeping reproduces LAPACK's sequential-swap ipiv.
+//   Back substitution (left-looking, block rows of NB): T_j = Y_j - U_{j,>j} X_{>j} (GEMM), X_j = U_jj^-1 T_j (GEMM).
+#pragma once
+#include <cooperative_groups.h>
+#include "zgemm.cuh"
+
+namespace ss {
+namespace cg = cooperative_groups;
+
+constexpr int LEAF_JB = 16;       // columns per leaf panel
+constexpr int LEAF_TPB = 512;     // threads (= rows) per CTA
+constexpr int LEAF_MAXC = 16;     // max cluster size
+
+struct LeafCand {                 // one CTA's pivot candidate for one column
+    double val;                   // |re| + |im| (LAPACK izamax metric), -1 if the CTA has no active row
+    int pos;                      // current row position inside the panel
+    int pad;
+    cplx row[LEAF_JB];
+};
+
+// Factor the m x jb panel at (row0, col0) of each batch matrix.  grid = (csize, batch), cluster (csize,1,1).
+__global__ void __launch_bounds__(LEAF_TPB, 1)
+lu_leaf_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restrict__ ipiv, int ipiv_stride,
+               int* __restrict__ info, int info_base) {
+    cg::cluster_group cluster = cg::this_cluster();
+    const int csize = (int)cluster.num_blocks();
+    const int crank = (int)cluster.block_rank();
+    const int z = blockIdx.y;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = LEAF_TPB / 32;
+
+    __shared__ LeafCand slots[2][LEAF_MAXC];
+    __shared__ double w_val[NW];
+    __shared__ int w_pos[NW];
+    __shared__ int w_tid[NW];
+    __shared__ int cta_owner;
+
+    cplx* __restrict__ A = bptr(Ab, z) + (long long)row0 * ld + col0;
+    const int r = crank * LEAF_TPB + tid;       // my row inside the panel
+    const bool valid = r < m;
+
+    cplx a[LEAF_JB];
+#pragma unroll
+    for (int k = 0; k < LEAF_JB; k++) a[k] = make_c(0.0, 0.0);
+    if (valid) {
+        const cplx* src = A + (long long)r * ld;
+#pragma unroll
+        for (int k = 0; k < LEAF_JB; k++)
+            if (k < jb) a[k] = src[k];
+    }
+    int cur_pos = r;
+    bool done = !valid;
+    int final_pos = r;
+
+#pragma unroll
+    for (int j = 0; j < LEAF_JB; j++) {
+        if (j < jb) {
+            const int buf = j & 1;
+            // ---- local arg-max (ties -> lowest position)
+            double v = done ? -1.0 : (fabs(a[j].re) + fabs(a[j].im));
+            int pp = cur_pos, tt = tid;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                double ov = __shfl_xor_sync(0xffffffffu, v, o);
+                int op = __shfl_xor_sync(0xffffffffu, pp, o);
+                int ot = __shfl_xor_sync(0xffffffffu, tt, o);
+                if (ov > v || (ov == v && op < pp)) { v = ov; pp = op; tt = ot; }
+            }
+            if (lane == 0) { w_val[warp] = v; w_pos[warp] = pp; w_tid[warp] = tt; }
+            __syncthreads();
+            if (warp == 0) {
+                double v2 = lane < NW ? w_val[lane] : -2.0;
+                int p2 = lane < NW ? w_pos[lane] : 0x7fffffff;
+                int t2 = lane < NW ? w_tid[lane] : 0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    double ov = __shfl_xor_sync(0xffffffffu, v2, o);
+                    int op = __shfl_xor_sync(0xffffffffu, p2, o);
+                    int ot = __shfl_xor_sync(0xffffffffu, t2, o);
+                    if (ov > v2 || (ov == v2 && op < p2)) { v2 = ov; p2 = op; t2 = ot; }
+                }
+                if (lane == 0) cta_owner = (v2 >= 0.0) ? t2 : -1;
+            }
+            __syncthreads();
+            // ---- publish this CTA's candidate to every CTA of the cluster (DSMEM)
+            const int owner = cta_owner;
+            if (owner < 0) {
+                if (tid == 0)
+                    for (int c = 0; c < csize; c++) {
+                        LeafCand* dst = cluster.map_shared_rank(&slots[buf][crank], c);
+                        dst->val = -1.0; dst->pos = 0x7fffffff;
+                    }
+            } else if (tid == owner) {
+                double myv = fabs(a[j].re) + fabs(a[j].im);
+                for (int c = 0; c < csize; c++) {
+                    LeafCand* dst = cluster.map_shared_rank(&slots[buf][crank], c);
+                    dst->val = myv; dst->pos = cur_pos;
+#pragma unroll
+                    for (int k = 0; k < LEAF_JB; k++) dst->row[k] = a[k];
+                }
+            }
+            cluster.sync();
+            // ---- winner among the csize candidates
+            int win = 0; double wv = slots[buf][0].val; int wp = slots[buf][0].pos;
+            for (int c = 1; c < csize; c++) {
+                double cv = slots[buf][c].val; int cp = slots[buf][c].pos;
+                if (cv > wv || (cv == wv && cp < wp)) { wv = cv; wp = cp; win = c; }
+            }
+            if (wv < 0.0) { wp = j; }                     // no rows left (m < jb): nothing to do
+            const bool singular = !(wv > 0.0);
+            if (crank == 0 && tid == 0) {
+                ipiv[(long long)z * ipiv_stride + row0 + j] = row0 + wp;
+                if (singular && wv >= 0.0) atomicCAS(&info[z], 0, info_base + row0 + j + 1);
+            }
+            if (!done) {
+                if (cur_pos == wp && wv >= 0.0) {
+                    done = true; final_pos = j;           // I am the pivot row: becomes row j of U
+                } else {
+                    if (cur_pos == j) cur_pos = wp;       // LAPACK swap bookkeeping
+                    if (!singular) {
+                        const cplx* prow = slots[buf][win].row;
+                        cplx rinv = crecip(prow[j]);
+                        cplx l = cmul(a[j], rinv);
+                        a[j] = l;
+#pragma unroll
+                        for (int k = j + 1; k < LEAF_JB; k++) a[k] = cfnma(a[k], l, prow[k]);
+                    }
+                }
+            }
+        }
+    }
+    if (valid) {
+        if (!done) final_pos = cur_pos;
+        cplx* dst = A + (long long)final_pos * ld;
+#pragma unroll
+        for (int k = 0; k < LEAF_JB; k++)
+            if (k < jb) dst[k] = a[k];
+    }
+}
+
+// Apply the row interchanges ipiv[row0 .. row0+jb) to columns [0, skip_lo) U [skip_hi, ncols) of each matrix.
+// One thread per column: consecutive threads touch consecutive elements of a row (coalesced in row-major).
+__global__ void __launch_bounds__(256)
+laswp_kernel(BPtr Ab, int ld, int ncols, int row0, int jb, int skip_lo, int skip_hi,
+             const int* __restrict__ ipiv, int ipiv_stride) {
+    const int z = blockIdx.y;
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nleft = skip_lo;
+    const int total = nleft + (ncols - skip_hi);
+    if (c >= total) return;
+    if (c >= nleft) c = skip_hi + (c - nleft);
+    cplx* __restrict__ A = bptr(Ab, z);
+    const int* piv = ipiv + (long long)z * ipiv_stride + row0;
+    for (int j = 0; j < jb; j++) {
+        int p = piv[j];
+        if (p != row0 + j) {
+            cplx* x = A + (long long)(row0 + j) * ld + c;
+            cplx* y = A + (long long)p * ld + c;
+            cplx tx = *x, ty = *y;
+            *x = ty; *y = tx;
+        }
+    }
+}
+
+// A12 <- L11^-1 A12 for the jb x w block right of a leaf (L11 = unit lower jb x jb at (row0, row0), jb <= 16).
+// One thread per column of A12.
+__global__ void __launch_bounds__(128)
+trsm_leaf_kernel(BPtr Ab, int ld, int row0, int jb, int c0, int w) {
+    __shared__ cplx L[LEAF_JB][LEAF_JB];
+    const int z = blockIdx.y;
+    cplx* __restrict__ A = bptr(Ab, z);
+    for (int i = threadIdx.x; i < jb * jb; i += blockDim.x) {
+        int rr = i / jb, cc = i % jb;
+        L[rr][cc] = A[(long long)(row0 + rr) * ld + row0 + cc];
+    }
+    __syncthreads();
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= w) return;
+    cplx x[LEAF_JB];
+#pragma unroll
+    for (int rr = 0; rr < LEAF_JB; rr++)
+        if (rr < jb) x[rr] = A[(long long)(row0 + rr) * ld + c0 + c];
+#pragma unroll
+    for (int rr = 1; rr < LEAF_JB; rr++) {
+        if (rr < jb) {
+            cplx s = x[rr];
+#pragma unroll
+            for (int k = 0; k < LEAF_JB; k++)
+                if (k < rr) s = cfnma(s, L[rr][k], x[k]);
+            x[rr] = s;
+        }
+    }
+#pragma unroll
+    for (int rr = 1; rr < LEAF_JB; rr++)
+        if (rr < jb) A[(long long)(row0 + rr) * ld + c0 + c] = x[rr];
+}
+
+// Inverse of an nt x nt (nt <= 128) triangular block T (row-major, ld) into Tinv (row-major, ldo = 128-padded):
+// lower (unit or not) or upper.  16x16 blocked forward substitution, one CTA (256 threads) per (block column, matrix).
+// Upper is handled as the index-reversed lower problem.  Everything outside the triangle of Tinv (up to the
+// padded size pad) is written as zero, the padded diagonal as one.
+struct TrtriArgs {
+    BPtr T; int ld;            // source matrices
+    long long t_step;          // element offset between consecutive diagonal blocks of one matrix (blockIdx.y)
+    int n_total;               // order of the whole triangular matrix (diag block y has min(128, n_total - 128 y) rows)
+    cplx* out;                 // [batch][nblocks][128*128]
+    int nblocks;
+    int upper, unit;
+};
+
+__global__ void __launch_bounds__(256)
+trtri_kernel(TrtriArgs p) {
+    constexpr int B = 16, NBK = 8, P = 128;
+    __shared__ cplx X[NBK][B][B + 1];    // inverse blocks of my block column
+    __shared__ cplx D[B][B + 1];
+    __shared__ cplx S[B][B + 1];
+    const int jbk = blockIdx.x, yb = blockIdx.y, z = blockIdx.z;
+    const int nt = min(P, p.n_total - P * yb);
+    const cplx* __restrict__ T = bptr(p.T, z) + (long long)yb * p.t_step;
+    cplx* __restrict__ O = p.out + ((long long)z * p.nblocks + yb) * (P * P);
+    const int tid = threadIdx.x, tr = tid / B, tc = tid % B;
+    const int upper = p.upper, unit = p.unit;
+    // element (i, j) of the (index-reversed if upper) lower-triangular matrix, identity-padded to 128
+    auto elem = [&](int i, int j) -> cplx {
+        if (i >= nt || j >= nt) return make_c(i == j ? 1.0 : 0.0, 0.0);
+        if (j > i) return make_c(0.0, 0.0);
+        if (unit && i == j) return make_c(1.0, 0.0);
+        int ii = upper ? nt - 1 - i : i, jj = upper ? nt - 1 - j : j;
+        return T[(long long)ii * p.ld + jj];
+    };
+    auto diag_inverse = [&](int bk) {      // D <- inverse of diagonal block bk (lower, 16x16)
+        S[tr][tc] = elem(bk * B + tr, bk * B + tc);
+        __syncthreads();
+        if (tid < B) {
+            int c = tid;
+            cplx x[B];
+#pragma unroll
+            for (int i = 0; i < B; i++) x[i] = make_c(0.0, 0.0);
+#pragma unroll
+            for (int i = 0; i < B; i++) {
+                if (i >= c) {
+                    cplx s = make_c(i == c ? 1.0 : 0.0, 0.0);
+#pragma unroll
+                    for (int k = 0; k < B; k++)
+                        if (k >= c && k < i) s = cfnma(s, S[i][k], x[k]);
+                    x[i] = cmul(s, crecip(S[i][i]));
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < B; i++) D[i][c] = x[i];
+        }
+        __syncthreads();
+    };
+    diag_inverse(jbk);
+    X[jbk][tr][tc] = D[tr][tc];
+    __syncthreads();
+    for (int ib = jbk + 1; ib < NBK; ib++) {
+        cplx s = make_c(0.0, 0.0);
+        for (int kb = jbk; kb < ib; kb++) {
+#pragma unroll
+            for (int k = 0; k < B; k++) s = cfma(s, elem(ib * B + tr, kb * B + k), X[kb][k][tc]);
+        }
+        diag_inverse(ib);                  // syncs inside; S is overwritten there, so stash s afterwards
+        S[tr][tc] = s;
+        __syncthreads();
+        cplx o = make_c(0.0, 0.0);
+#pragma unroll
+        for (int k = 0; k < B; k++) o = cfnma(o, D[tr][k], S[k][tc]);
+        X[ib][tr][tc] = o;
+        __syncthreads();
+    }
+    // write block column jbk of the inverse (zeros above the diagonal blocks), undoing the index reversal.
+    // Reversal applies to the nt x nt part only; the identity padding stays in place.
+    for (int ib = 0; ib < NBK; ib++) {
+        int i = ib * B + tr, j = jbk * B + tc;
+        cplx v = (ib >= jbk) ? X[ib][tr][tc] : make_c(0.0, 0.0);
+        int oi = i, oj = j;
+        if (upper && i < nt && j < nt) { oi = nt - 1 - i; oj = nt - 1 - j; }
+        if (upper && ((i < nt) != (j < nt))) v = make_c(0.0, 0.0);
+        O[(long long)oi * P + oj] = v;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host drivers
+// ---------------------------------------------------------------------------------------------------------
+struct Ctx {
+    cudaStream_t st = nullptr;
+    long long launches = 0;
+    cudaError_t err = cudaSuccess;
+    void note(cudaError_t e) { if (err == cudaSuccess && e != cudaSuccess) err = e; launches++; }
+};
+
+struct LuWork {
+    cplx* tinv = nullptr;       // [batch][tinv_blocks][128*128] triangular-inverse scratch
+    int tinv_blocks = 0;
+    int* ipiv = nullptr;        // [batch][ipiv_stride]
+    int ipiv_stride = 0;
+    int* info = nullptr;        // [batch]
+};
+
+static inline GemmArgs gemm_std(int M, int N, int K, double alpha, BPtr A, int lda, BPtr B, int ldb, double beta,
+                                BPtr C, int ldc) {
+    GemmArgs g{};
+    g.M = M; g.N = N; g.K = K; g.A = A; g.lda = lda; g.B = B; g.ldb = ldb; g.C = C; g.ldc = ldc;
+    g.Cin = C; g.ldcin = ldc; g.alpha = alpha; g.beta = beta; g.E = nullptr;
+    return g;
+}
+
+static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, int jb, const LuWork& w, int info_base,
+                        int batch) {
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(lu_leaf_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        configured = true;
+    }
+    int need = (m + LEAF_TPB - 1) / LEAF_TPB;
+    int csize = 1;
+    while (csize < need) csize <<= 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)csize, (unsigned)batch, 1);
+    cfg.blockDim = dim3(LEAF_TPB, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = ctx.st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)csize;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
+}
+
+// LU with partial pivoting of the leading n x n part of the n x ncols matrices; interchanges and L-solve applied
+// to all ncols columns.  nb_lu: outer block (multiple of 16, <= 128).  n <= LEAF_TPB * LEAF_MAXC.
+static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, int nb_lu, const LuWork& w,
+                      int info_base) {
+    for (int j0 = 0; j0 < n; j0 += nb_lu) {
+        const int nbw = min(nb_lu, n - j0);
+        for (int c = j0; c < j0 + nbw; c += LEAF_JB) {
+            const int jb = min(LEAF_JB, j0 + nbw - c);
+            const int m = n - c;
+            launch_leaf(ctx, Ab, ld, c, c, m, jb, w, info_base, batch);
+            {
+                int total = c + (ncols - (c + jb));
+                if (total > 0) {
+                    dim3 grid((unsigned)((total + 255) / 256), (unsigned)batch);
+                    laswp_kernel<<<grid, 256, 0, ctx.st>>>(Ab, ld, ncols, c, jb, c, c + jb, w.ipiv, w.ipiv_stride);
+                    ctx.note(cudaGetLastError());
+                }
+            }
+            const int wcols = j0 + nbw - (c + jb);
+            if (wcols > 0) {
+                dim3 grid((unsigned)((wcols + 127) / 128), (unsigned)batch);
+                trsm_leaf_kernel<<<grid, 128, 0, ctx.st>>>(Ab, ld, c, jb, c + jb, wcols);
+                ctx.note(cudaGetLastError());
+                if (m - jb > 0) {
+                    GemmArgs g = gemm_std(m - jb, wcols, jb, -1.0, bp_offset(Ab, (long long)(c + jb) * ld + c), ld,
+                                          bp_offset(Ab, (long long)c * ld + c + jb), ld, 1.0,
+                                          bp_offset(Ab, (long long)(c + jb) * ld + c + jb), ld);
+                    ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_STD, ctx.st));
+                }
+            }
+        }
+        const int rest = ncols - (j0 + nbw);
+        if (rest > 0) {
+            TrtriArgs t{};
+            t.T = bp_offset(Ab, (long long)j0 * ld + j0); t.ld = ld; t.t_step = 0; t.n_total = nbw;
+            t.out = w.tinv; t.nblocks = 1; t.upper = 0; t.unit = 1;
+            trtri_kernel<<<dim3(8, 1, (unsigned)batch), 256, 0, ctx.st>>>(t);
+            ctx.note(cudaGetLastError());
+            BPtr A12 = bp_offset(Ab, (long long)j0 * ld + j0 + nbw);
+            GemmArgs g = gemm_std(nbw, rest, nbw, 1.0, bp_strided(w.tinv, 128 * 128), 128, A12, ld, 0.0, A12, ld);
+            ctx.note(gemm_launch(g, batch, GEMM_TALL, EPI_STD, ctx.st));
+            const int mrest = n - (j0 + nbw);
+            if (mrest > 0) {
+                GemmArgs u = gemm_std(mrest, rest, nbw, -1.0, bp_offset(Ab, (long long)(j0 + nbw) * ld + j0), ld, A12, ld,
+                                      1.0, bp_offset(Ab, (long long)(j0 + nbw) * ld + j0 + nbw), ld);
+                ctx.note(gemm_launch(u, batch, GEMM_BIG, EPI_STD, ctx.st));
+            }
+        }
+    }
+}
+
+// X = U^-1 Y with U = upper factor in AB[:, 0:n], Y = AB[:, n:n+nrhs] (overwritten).  Left-looking over block rows.
+static void back_substitute(Ctx& ctx, BPtr Ab, int ld, int n, int nrhs, BPtr X, int ldx, int batch, const LuWork& w) {
+    if (nrhs <= 0 || n <= 0) return;
+    const int P = 128;
+    const int nblk = (n + P - 1) / P;
+    TrtriArgs t{};
+    t.T = Ab; t.ld = ld; t.t_step = (long long)P * ld + P; t.n_total = n; t.out = w.tinv; t.nblocks = nblk;
+    t.upper = 1; t.unit = 0;
+    trtri_kernel<<<dim3(8, (unsigned)nblk, (unsigned)batch), 256, 0, ctx.st>>>(t);
+    ctx.note(cudaGetLastError());
+    for (int jb = nblk - 1; jb >= 0; jb--) {
+        const int j = jb * P, nbj = min(P, n - j), kk = n - j - nbj;
+        BPtr Yj = bp_offset(Ab, (long long)j * ld + n);
+        if (kk > 0) {
+            GemmArgs g = gemm_std(nbj, nrhs, kk, -1.0, bp_offset(Ab, (long long)j * ld + j + nbj), ld,
+                                  bp_offset(X, (long long)(j + nbj) * ldx), ldx, 1.0, Yj, ld);
+            ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_STD, ctx.st));
+        }
+        GemmArgs g2 = gemm_std(nbj, nrhs, nbj, 1.0, bp_strided(w.tinv + (long long)jb * P * P, (long long)nblk * P * P), P,
+                               Yj, ld, 0.0, bp_offset(X, (long long)j * ldx), ldx);
+        ctx.note(gemm_launch(g2, batch, GEMM_BIG, EPI_STD, ctx.st));
+    }
+}
+
+}  // namespace ss

@@ -1,0 +1,276 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+    normwise backward error <= 1e-12, relative Frobenius error of X <= 1e-8, relative T(E) error <= 1e-9.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import banded, dense, residual  # noqa: E402
+from paper_1812_01396_b200 import inputs  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+TOL_BWD, TOL_X, TOL_T = 1e-12, 1e-8, 1e-9
+
+
+def dev(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(lib, p, want_inverse=False, options=None):
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    for k, v in (options or {}).items():
+        ss.set_option(k, v)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    X = ss.solve(p.E, dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first), dev(p.Inj_last))
+    T = ss.transmission()
+    out = dict(X=None if X is None else X.cpu().numpy(), T=T, ss=ss)
+    if want_inverse:
+        out["QP"] = [tuple(t.cpu().numpy() for t in ss.inverse_columns(e)) for e in range(p.n_energy)]
+    return out
+
+
+def oracle_args(p, e):
+    il = None if p.Inj_last is None else p.Inj_last[e]
+    return (p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], il)
+
+
+def check_against_oracle(p, out, energies=None, solver=dense):
+    worst = dict(bwd=0.0, x=0.0, t=0.0)
+    for e in (range(p.n_energy) if energies is None else energies):
+        r = solver.solve_energy(*oracle_args(p, e))
+        bwd = residual.backward_error(*oracle_args(p, e), out["X"][e])
+        ex = residual.rel_frobenius(out["X"][e], r["X"])
+        et = residual.rel_T(out["T"][e], r["T_LR"])
+        assert bwd <= TOL_BWD, (e, bwd)
+        assert ex <= TOL_X, (e, ex)
+        assert et <= TOL_T, (e, et, out["T"][e], r["T_LR"])
+        worst = dict(bwd=max(worst["bwd"], bwd), x=max(worst["x"], ex), t=max(worst["t"], et))
+    return worst
+
+
+# ------------------------------------------------------------------------------------------------------
+# building blocks
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("M,N,K,batch", [(64, 64, 64, 1), (1, 1, 1, 2), (37, 53, 29, 3), (130, 70, 200, 2),
+                                         (200, 16, 3, 2), (5, 300, 17, 1), (64, 64, 0, 1)])
+def test_zgemm_batched_vs_numpy(lib, M, N, K, batch):
+    A = inputs.complex_gaussian(1, 50, M, (batch, M, K), 1.0)
+    B = inputs.complex_gaussian(1, 51, N, (batch, K, N), 1.0)
+    C0 = inputs.complex_gaussian(1, 52, K, (batch, M, N), 1.0)
+    for alpha, beta in ((1.0, 0.0), (-1.0, 1.0), (0.5, -2.0)):
+        C = dev(C0.copy())
+        lib.zgemm_batched(dev(A), dev(B), C, alpha, beta)
+        want = alpha * np.matmul(A, B) + beta * C0
+        scale = (np.abs(A).max() * np.abs(B).max() * K if K else 0.0) + np.abs(C0).max() * abs(beta) + 1e-300
+        assert np.abs(C.cpu().numpy() - want).max() <= 1e-14 * scale * 4
+
+
+@pytest.mark.parametrize("n,nrhs,batch", [(1, 1, 1), (7, 3, 2), (16, 16, 1), (33, 5, 3), (128, 40, 2), (200, 37, 2),
+                                          (513, 10, 1), (700, 129, 1)])
+def test_zgesv_batched_vs_numpy(lib, n, nrhs, batch):
+    A = inputs.complex_gaussian(2, 60, n, (batch, n, n), 1.0)
+    B = inputs.complex_gaussian(2, 61, n, (batch, n, nrhs), 1.0)
+    AB = dev(np.concatenate([A, B], axis=2))
+    X, ipiv, info = lib.zgesv_batched(AB, n)
+    assert int(info.abs().max()) == 0
+    X = X.cpu().numpy()
+    for z in range(batch):
+        want = np.linalg.solve(A[z], B[z])
+        res = np.linalg.norm(A[z] @ X[z] - B[z]) / (np.linalg.norm(A[z]) * np.linalg.norm(X[z]) + np.linalg.norm(B[z]))
+        assert res <= 1e-13, (z, res)
+        assert np.linalg.norm(X[z] - want) <= 1e-9 * np.linalg.norm(want)
+
+
+@pytest.mark.parametrize("n", [5, 16, 100, 300])
+def test_zgetrf_factors_and_pivots(lib, n):
+    """P A = L U reconstructed from the in-place factors and LAPACK-style sequential swaps; partial pivoting
+    means every |L_ij| <= 1 in the pivot metric up to the |re|+|im| vs modulus slack (sqrt 2)."""
+    batch = 2
+    A = inputs.complex_gaussian(3, 70, n, (batch, n, n), 1.0)
+    AB = dev(A.copy())
+    ipiv, info = lib.zgetrf_batched(AB, n)
+    LU = AB.cpu().numpy()
+    ipiv = ipiv.cpu().numpy()
+    assert int(info.abs().max()) == 0
+    for z in range(batch):
+        L = np.tril(LU[z], -1) + np.eye(n)
+        U = np.triu(LU[z])
+        PA = A[z].copy()
+        for j in range(n):
+            p = ipiv[z, j]
+            assert j <= p < n
+            if p != j:
+                PA[[j, p]] = PA[[p, j]]
+        assert np.linalg.norm(PA - L @ U) <= 1e-13 * np.linalg.norm(A[z]) * n
+        assert np.abs(np.tril(LU[z], -1)).max() <= np.sqrt(2.0) + 1e-12
+
+
+def test_zgesv_needs_pivoting(lib):
+    """A matrix whose leading entries are zero: no-pivot LU (the paper's zgesv_nopiv, L186) would divide by zero."""
+    n = 48
+    A = inputs.complex_gaussian(4, 80, 0, (1, n, n), 1.0)
+    A[0, np.arange(n), np.arange(n)] = 0.0
+    B = inputs.complex_gaussian(4, 81, 0, (1, n, 4), 1.0)
+    X, ipiv, info = lib.zgesv_batched(dev(np.concatenate([A, B], axis=2)), n)
+    assert int(info[0]) == 0
+    assert np.linalg.norm(A[0] @ X.cpu().numpy()[0] - B[0]) <= 1e-12 * np.linalg.norm(A[0]) * np.linalg.norm(B[0])
+
+
+def test_zgetrf_reports_exact_singularity(lib):
+    n = 20
+    A = inputs.complex_gaussian(5, 90, 0, (1, n, n), 1.0)
+    A[0, :, 7] = 0.0
+    _, info = lib.zgetrf_batched(dev(A), n)
+    assert int(info[0]) == 8          # 1 + index of the first zero pivot
+
+
+# ------------------------------------------------------------------------------------------------------
+# the hot path
+# ------------------------------------------------------------------------------------------------------
+def test_config0_all_energies(lib):
+    p = inputs.make_problem(inputs.CONFIGS["C0"])
+    out = run_gpu(lib, p, want_inverse=True)
+    check_against_oracle(p, out)
+    for e in range(p.n_energy):
+        Q, P = dense.inverse_columns(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+        assert residual.rel_frobenius(out["QP"][e][0], Q) <= TOL_X
+        assert residual.rel_frobenius(out["QP"][e][1], P) <= TOL_X
+    assert out["ss"].launch_count() > 0
+
+
+@pytest.mark.parametrize("bs,nb,n_e,nrhs,inj_last", [(1, 2, 1, 1, False), (2, 3, 2, 1, True), (5, 2, 3, 7, True),
+                                                     (16, 2, 1, 16, False), (17, 5, 2, 3, True), (33, 4, 2, 40, True),
+                                                     (100, 6, 3, 37, False), (130, 3, 2, 150, True),
+                                                     (200, 5, 2, 37, True)])
+def test_ragged_sizes_vs_dense_oracle(lib, bs, nb, n_e, nrhs, inj_last):
+    """Sizes that are not multiples of any tile (64-wide GEMM tiles, 16-column panels, 128 LU blocks)."""
+    p = inputs.random_problem(bs, nb, n_e, nrhs, seed=11, inj_last=inj_last)
+    out = run_gpu(lib, p)
+    check_against_oracle(p, out)
+
+
+def test_real_energy_symmetry_and_reciprocity(lib):
+    """At Im E = 0: P_1 = Q_nb^H (A Hermitian, L154)."""
+    p = inputs.random_problem(24, 5, 2, 4, seed=3, eta=0.0)
+    out = run_gpu(lib, p, want_inverse=True)
+    check_against_oracle(p, out)
+    for e in range(2):
+        Q, P = out["QP"][e]
+        assert np.linalg.norm(P[0] - Q[-1].conj().T) <= 1e-9 * np.linalg.norm(P[0])
+
+
+def test_perfect_chain_small_closed_form(lib):
+    p = inputs.perfect_chain_problem(8, 12, 6)      # even count: the midpoint grid never hits E = 0 (D_nb = 0 there)
+    out = run_gpu(lib, p)
+    k = inputs.chain_wavevector(p.E, -1.0)
+    for e in range(6):
+        expect = np.concatenate([np.exp(1j * k[e] * j) * np.eye(8) for j in range(1, 13)])
+        assert np.abs(out["X"][e] - expect).max() <= 1e-10
+        assert abs(out["T"][e] - 8.0) <= 8.0 * TOL_T
+
+
+def test_config1_perfect_chain_full_size(lib):
+    """BASELINE.json config 1: T(E) = 64 exactly, X_j = e^{ikj} 1; all 64 energies (closed form), 3 vs Tier B."""
+    cfg = inputs.CONFIGS["C1"]
+    p = inputs.make_problem(cfg)
+    out = run_gpu(lib, p)
+    k = inputs.chain_wavevector(p.E, -1.0)
+    j = np.arange(1, cfg.nb + 1)
+    for e in range(cfg.n_energy):
+        assert abs(out["T"][e] - 64.0) <= 64.0 * TOL_T, (e, out["T"][e])
+        Xb = out["X"][e].reshape(cfg.nb, cfg.bs, cfg.bs)
+        expect = np.exp(1j * k[e] * j)[:, None, None] * np.eye(cfg.bs)[None]
+        assert np.linalg.norm(Xb - expect) <= TOL_X * np.linalg.norm(expect)
+        assert residual.backward_error(*oracle_args(p, e), out["X"][e]) <= TOL_BWD
+    check_against_oracle(p, out, energies=(0, 31, 63), solver=banded)
+
+
+def test_zero_self_energy_and_decoupled_device(lib):
+    """Sigma = 0 => R = 1, X = Q b', T = 0; H_upper = S_upper = 0 somewhere => T = 0 (reading c19)."""
+    p = inputs.random_problem(12, 4, 2, 3, seed=5)
+    p.Sigma_L[:] = 0.0
+    out = run_gpu(lib, p)
+    check_against_oracle(p, out, energies=[])
+    for e in range(2):
+        assert abs(out["T"][e]) <= 1e-13
+        r = dense.solve_energy(*oracle_args(p, e))
+        assert residual.rel_frobenius(out["X"][e], r["X"]) <= TOL_X
+    p2 = inputs.random_problem(12, 4, 1, 3, seed=6)
+    p2.H_upper[1] = 0.0
+    p2.S_upper[1] = 0.0
+    out2 = run_gpu(lib, p2)
+    assert abs(out2["T"][0]) <= 1e-13
+    assert residual.backward_error(*oracle_args(p2, 0), out2["X"][0]) <= TOL_BWD
+
+
+def test_nrhs_zero_transmission_only(lib):
+    p = inputs.random_problem(20, 3, 2, 1, seed=8)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    assert ss.solve(p.E, dev(p.Sigma_L), dev(p.Sigma_R), None) is None
+    T = ss.transmission()
+    for e in range(2):
+        r = dense.solve_energy(*oracle_args(p, e))
+        assert residual.rel_T(T[e], r["T_LR"]) <= TOL_T
+
+
+def test_call_order_and_singular_reporting(lib):
+    p = inputs.random_problem(8, 3, 1, 2, seed=9)
+    ss = lib.SplitSolve(p.nb, p.bs, 1)
+    with pytest.raises(lib.SplitSolveError) as ei:
+        ss.solve(p.E, dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first))
+    assert ei.value.status == lib.SS_ERR_NOT_READY
+    with pytest.raises(lib.SplitSolveError) as ei:
+        ss.transmission()
+    assert ei.value.status == lib.SS_ERR_NOT_READY
+    # exactly singular A: H = 0, S = 0 in the last diagonal block and its couplings -> zero pivot in block nb
+    p.H_diag[2] = 0; p.S_diag[2] = 0; p.H_upper[1] = 0; p.S_upper[1] = 0
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    ss.solve(p.E, dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first))
+    with pytest.raises(lib.SplitSolveError) as ei:
+        ss.synchronize()
+    assert ei.value.status == lib.SS_ERR_SINGULAR
+    e, b, c = ss.last_info()
+    assert e == 0 and b == 3
+
+
+def test_host_buffer_entry_points(lib):
+    p = inputs.random_problem(40, 4, 2, 9, seed=10, inj_last=True)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_hamiltonian_host(p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    X = np.empty((2, p.nb * p.bs, 9), dtype=np.complex128)
+    T = np.empty(2)
+    ss.solve_host(p.E, p.Sigma_L, p.Sigma_R, p.Inj_first, p.Inj_last, X, T)
+    check_against_oracle(p, dict(X=X, T=T))
+
+
+def test_lu_block_option_and_repeat_solve_is_deterministic(lib):
+    p = inputs.random_problem(150, 3, 2, 5, seed=12)
+    a = run_gpu(lib, p, options={"nb_lu": 32})
+    check_against_oracle(p, a)
+    b = run_gpu(lib, p)
+    c = run_gpu(lib, p)
+    assert np.array_equal(b["X"], c["X"]) and np.array_equal(b["T"], c["T"])
+
+
+def test_config2_medium_subset_vs_banded_oracle(lib):
+    """BASELINE.json config 2 (bs=512, nb=64) with fewer energies resident: 2 energies checked against Tier B,
+    every energy against the residual (Tier C)."""
+    cfg = inputs.CONFIGS["C2"]
+    p = inputs.random_problem(cfg.bs, cfg.nb, 4, cfg.nrhs, seed=0, threads=8)
+    # the energy grid of the full config has 32 points; take points 0, 10, 21, 31 of it
+    full = inputs.energy_grid(cfg.n_energy, cfg.e_lo, cfg.e_hi, cfg.eta)
+    sel = [0, 10, 21, 31]
+    p.E = full[sel].copy()
+    for i, e in enumerate(sel):
+        p.Sigma_L[i] = inputs.sigma_block(0, e, cfg.bs, "L")
+        p.Sigma_R[i] = inputs.sigma_block(0, e, cfg.bs, "R")
+        p.Inj_first[i] = inputs.inj_block(0, e, cfg.bs, cfg.nrhs)
+    out = run_gpu(lib, p)
+    for e in range(4):
+        assert residual.backward_error(*oracle_args(p, e), out["X"][e]) <= TOL_BWD
+        assert -1e-9 <= out["T"][e] <= cfg.bs
+    check_against_oracle(p, out, energies=(0, 3), solver=banded)
