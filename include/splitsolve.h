@@ -131,7 +131,13 @@ ss_status_t ss_phase_ms(ss_handle_t h, int phase, float* ms);
 /* Number of kernel launches the last ss_solve enqueued. */
 long long ss_launch_count(ss_handle_t h);
 
-/* Options: name in {"nb_lu" (outer LU block, 32..128, multiple of 16), "transmission" (0/1, default 1)}. */
+/* With option "profile_gemm" = 1, every launch of the GEMM kernel in ss_solve is bracketed by CUDA events on the
+ * solve's stream; this returns, for the last ss_solve, the summed device time of those launches (ms), their
+ * algorithmic flops (8 M N K per complex GEMM) and their number.  Synchronises. */
+ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long* launches);
+
+/* Options: "nb_lu" (outer LU block, 16..128, multiple of 16; default 128), "transmission" (0/1, default 1:
+ * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0). */
 ss_status_t ss_set_option(ss_handle_t h, const char* name, int value);
 
 const char* ss_strerror(ss_status_t s);

@@ -32,6 +32,7 @@ SIGNATURES = {
     "ss_flops_sweep": (c_double, [c_void_p]),
     "ss_workspace_bytes": (c_size_t, [c_int, c_int, c_int, c_int]),
     "ss_phase_ms": (c_int, [c_void_p, c_int, POINTER(c_float)]),
+    "ss_gemm_profile": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_longlong)]),
     "ss_launch_count": (c_longlong, [c_void_p]),
     "ss_set_option": (c_int, [c_void_p, c_char_p, c_int]),
     "ss_strerror": (c_char_p, [c_int]),
@@ -177,6 +178,12 @@ class SplitSolve:
         ms = c_float()
         _check(load().ss_phase_ms(self._h, phase, byref(ms)), "ss_phase_ms")
         return float(ms.value)
+
+    def gemm_profile(self):
+        """(device ms, algorithmic flops, launches) of the GEMM kernel in the last solve (option profile_gemm=1)."""
+        ms, fl, n = c_double(), c_double(), c_longlong()
+        _check(load().ss_gemm_profile(self._h, byref(ms), byref(fl), byref(n)), "ss_gemm_profile")
+        return float(ms.value), float(fl.value), int(n.value)
 
     def launch_count(self) -> int:
         return int(load().ss_launch_count(self._h))

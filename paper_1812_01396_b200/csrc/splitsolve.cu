@@ -19,6 +19,8 @@ struct ss_handle_s {
     // options
     int nb_lu = 128;
     int want_T = 1;
+    int profile_gemm = 0;
+    GemmProfile prof;
     // workspace (allocated for ws_nrhs)
     int ws_nrhs = -1;
     cplx *slots = nullptr, *aug = nullptr, *aop = nullptr, *tinv = nullptr, *raug = nullptr, *wz = nullptr;
@@ -144,6 +146,7 @@ extern "C" ss_status_t ss_destroy(ss_handle_t h) {
     free_host_path(h);
     for (int i = 0; i < 4; i++) free_dev(h->own_hs[i]);
     for (int i = 0; i < 3; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    for (cudaEvent_t e : h->prof.ev) cudaEventDestroy(e);
     if (h->E_pinned) cudaFreeHost(h->E_pinned);
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
     delete h;
@@ -183,6 +186,7 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         h->nb_lu = value; return SS_OK;
     }
     if (!strcmp(name, "transmission")) { h->want_T = value ? 1 : 0; return SS_OK; }
+    if (!strcmp(name, "profile_gemm")) { h->profile_gemm = value ? 1 : 0; return SS_OK; }
     return SS_ERR_INVALID_ARG;
 }
 
@@ -253,7 +257,7 @@ static void run_sweep(ss_handle_t h, Ctx& ctx) {
         g.S = bp_chain(h->Sd + (long long)(i_f - 1) * B2, h->Sd + (long long)(i_m - 1) * B2, 0);
         g.H = bp_chain(h->Hd + (long long)(i_f - 1) * B2, h->Hd + (long long)(i_m - 1) * B2, 0);
         g.lds = bs; g.E = h->E_dev;
-        ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_SCHUR, ctx.st));
+        gemm_run(ctx, g, batch, GEMM_BIG, EPI_SCHUR);
         // a2 + the L half of a3
         lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, h->nb_lu, w, s * info_stride);
         // U half of a3: X_i / Y_i into its slot
@@ -266,7 +270,7 @@ static void run_sweep(ss_handle_t h, Ctx& ctx) {
         GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_chain(slot(0, i0), slot(1, i1 - 1), s_slot_e), bs,
                               bp_chain(slot(0, i0 - 2), slot(1, i1 + 1), s_slot_e), bs, 0.0,
                               bp_chain(slot(0, i0 - 1), slot(1, i1), s_slot_e), bs);
-        ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g, batch, GEMM_BIG, EPI_STD);
     }
 }
 
@@ -293,7 +297,7 @@ static void run_post(ss_handle_t h, Ctx& ctx, const cplx* SigL, const cplx* SigR
             const cplx* Bsrc = (bc == 0) ? slot(0, br == 0 ? 0 : nb - 1) : slot(1, br == 0 ? 1 : nb);
             GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(Bsrc, s_slot_e), bs, 1.0,
                                   bp_strided(h->raug + (long long)br * bs * W + (long long)bc * bs, s_r), W);
-            ctx.note(gemm_launch(g, nE, GEMM_BIG, EPI_STD, ctx.st));
+            gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         }
     LuWork w;
     w.tinv = h->tinv; w.tinv_blocks = h->tinv_blocks_total;
@@ -305,29 +309,29 @@ static void run_post(ss_handle_t h, Ctx& ctx, const cplx* SigL, const cplx* SigR
         GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(0, 0), nb, B2, s_slot_e), bs,
                               bp_two_level(h->wz, nb, 0, s_w), nr, 0.0,
                               bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
-        ctx.note(gemm_launch(g, nE * nb, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g, nE * nb, GEMM_BIG, EPI_STD);
         GemmArgs g2 = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(1, 1), nb, B2, s_slot_e), bs,
                                bp_two_level(h->wz + (long long)bs * nr, nb, 0, s_w), nr, 1.0,
                                bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
-        ctx.note(gemm_launch(g2, nE * nb, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g2, nE * nb, GEMM_BIG, EPI_STD);
     }
     // a7: G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22;  T = Re Tr(Gamma_L G Gamma_R G^H)
     if (h->want_T) {
         GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(0, 0), s_slot_e), bs, bp_strided(h->wz + m, s_w), nr, 0.0,
                               bp_strided(h->g1n, B2), bs);
-        ctx.note(gemm_launch(g, nE, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(1, 1), s_slot_e), bs,
                                bp_strided(h->wz + (long long)bs * nr + m, s_w), nr, 1.0, bp_strided(h->g1n, B2), bs);
-        ctx.note(gemm_launch(g2, nE, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g2, nE, GEMM_BIG, EPI_STD);
         dim3 gg((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)nE);
         gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigL, h->gam_l, bs); ctx.note(cudaGetLastError());
         gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigR, h->gam_r, bs); ctx.note(cudaGetLastError());
         GemmArgs g3 = gemm_std(bs, bs, bs, 1.0, bp_strided(h->gam_l, B2), bs, bp_strided(h->g1n, B2), bs, 0.0,
                                bp_strided(h->w1, B2), bs);
-        ctx.note(gemm_launch(g3, nE, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g3, nE, GEMM_BIG, EPI_STD);
         GemmArgs g4 = gemm_std(bs, bs, bs, 1.0, bp_strided(h->w1, B2), bs, bp_strided(h->gam_r, B2), bs, 0.0,
                                bp_strided(h->w2, B2), bs);
-        ctx.note(gemm_launch(g4, nE, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g4, nE, GEMM_BIG, EPI_STD);
         int parts = (int)min((long long)TRACE_PARTS, cdiv(B2, 256));
         trace_partial_kernel<<<dim3((unsigned)parts, (unsigned)nE), 256, 0, ctx.st>>>(h->w2, h->g1n, B2, B2, h->tpart);
         ctx.note(cudaGetLastError());
@@ -348,6 +352,8 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
     if (h->solved) cudaEventSynchronize(h->ev[2]);        // E_pinned of the previous call is free again
     memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
     Ctx ctx; ctx.st = stream;
+    h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
+    ctx.prof = h->profile_gemm ? &h->prof : nullptr;
     if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
         cudaMemsetAsync(h->info, 0, sizeof(int) * 3 * (size_t)h->n_energy, stream) != cudaSuccess) {
         cudaGetLastError(); return SS_ERR_CUDA;
@@ -453,6 +459,20 @@ extern "C" ss_status_t ss_phase_ms(ss_handle_t h, int phase, float* ms) {
                   : (phase == 1) ? cudaEventElapsedTime(ms, h->ev[1], h->ev[2])
                                  : cudaEventElapsedTime(ms, h->ev[0], h->ev[2]);
     if (e != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long* launches) {
+    if (!h || !ms || !flops || !launches) return SS_ERR_INVALID_ARG;
+    if (!h->solved || !h->profile_gemm) return SS_ERR_NOT_READY;
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    double total = 0.0;
+    for (size_t i = 0; i + 1 < h->prof.used; i += 2) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, h->prof.ev[i], h->prof.ev[i + 1]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+        total += t;
+    }
+    *ms = total; *flops = h->prof.flops; *launches = h->prof.launches;
     return SS_OK;
 }
 

@@ -20,6 +20,7 @@
 //   Back substitution (left-looking, block rows of NB): T_j = Y_j - U_{j,>j} X_{>j} (GEMM), X_j = U_jj^-1 T_j (GEMM).
 #pragma once
 #include <cooperative_groups.h>
+#include <vector>
 #include "zgemm.cuh"
 
 namespace ss {
@@ -302,12 +303,39 @@ trtri_kernel(TrtriArgs p) {
 // ---------------------------------------------------------------------------------------------------------
 // host drivers
 // ---------------------------------------------------------------------------------------------------------
+struct GemmProfile {                 // optional per-launch CUDA-event timing of the GEMM kernel (bench.py's roofline)
+    std::vector<cudaEvent_t> ev;     // pairs: start, stop
+    size_t used = 0;                 // events used by the last solve
+    double flops = 0.0;              // 8 M N K batch summed over the timed launches
+    long long launches = 0;
+};
+
 struct Ctx {
     cudaStream_t st = nullptr;
     long long launches = 0;
     cudaError_t err = cudaSuccess;
+    GemmProfile* prof = nullptr;
     void note(cudaError_t e) { if (err == cudaSuccess && e != cudaSuccess) err = e; launches++; }
 };
+
+static void gemm_run(Ctx& ctx, const GemmArgs& g, int batch, int cfg, int epi) {
+    GemmProfile* pr = ctx.prof;
+    if (pr && g.M > 0 && g.N > 0 && batch > 0) {
+        if (pr->used + 2 > pr->ev.size()) {
+            cudaEvent_t a, b;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { ctx.note(cudaErrorMemoryAllocation); return; }
+            pr->ev.push_back(a); pr->ev.push_back(b);
+        }
+        cudaEventRecord(pr->ev[pr->used], ctx.st);
+        ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st));
+        cudaEventRecord(pr->ev[pr->used + 1], ctx.st);
+        pr->used += 2;
+        pr->flops += 8.0 * g.M * g.N * g.K * batch;
+        pr->launches++;
+    } else {
+        ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st));
+    }
+}
 
 struct LuWork {
     cplx* tinv = nullptr;       // [batch][tinv_blocks][128*128] triangular-inverse scratch
@@ -377,7 +405,7 @@ static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, in
                     GemmArgs g = gemm_std(m - jb, wcols, jb, -1.0, bp_offset(Ab, (long long)(c + jb) * ld + c), ld,
                                           bp_offset(Ab, (long long)c * ld + c + jb), ld, 1.0,
                                           bp_offset(Ab, (long long)(c + jb) * ld + c + jb), ld);
-                    ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_STD, ctx.st));
+                    gemm_run(ctx, g, batch, GEMM_BIG, EPI_STD);
                 }
             }
         }
@@ -390,12 +418,12 @@ static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, in
             ctx.note(cudaGetLastError());
             BPtr A12 = bp_offset(Ab, (long long)j0 * ld + j0 + nbw);
             GemmArgs g = gemm_std(nbw, rest, nbw, 1.0, bp_strided(w.tinv, 128 * 128), 128, A12, ld, 0.0, A12, ld);
-            ctx.note(gemm_launch(g, batch, GEMM_TALL, EPI_STD, ctx.st));
+            gemm_run(ctx, g, batch, GEMM_TALL, EPI_STD);
             const int mrest = n - (j0 + nbw);
             if (mrest > 0) {
                 GemmArgs u = gemm_std(mrest, rest, nbw, -1.0, bp_offset(Ab, (long long)(j0 + nbw) * ld + j0), ld, A12, ld,
                                       1.0, bp_offset(Ab, (long long)(j0 + nbw) * ld + j0 + nbw), ld);
-                ctx.note(gemm_launch(u, batch, GEMM_BIG, EPI_STD, ctx.st));
+                gemm_run(ctx, u, batch, GEMM_BIG, EPI_STD);
             }
         }
     }
@@ -417,11 +445,11 @@ static void back_substitute(Ctx& ctx, BPtr Ab, int ld, int n, int nrhs, BPtr X, 
         if (kk > 0) {
             GemmArgs g = gemm_std(nbj, nrhs, kk, -1.0, bp_offset(Ab, (long long)j * ld + j + nbj), ld,
                                   bp_offset(X, (long long)(j + nbj) * ldx), ldx, 1.0, Yj, ld);
-            ctx.note(gemm_launch(g, batch, GEMM_BIG, EPI_STD, ctx.st));
+            gemm_run(ctx, g, batch, GEMM_BIG, EPI_STD);
         }
         GemmArgs g2 = gemm_std(nbj, nrhs, nbj, 1.0, bp_strided(w.tinv + (long long)jb * P * P, (long long)nblk * P * P), P,
                                Yj, ld, 0.0, bp_offset(X, (long long)j * ldx), ldx);
-        ctx.note(gemm_launch(g2, batch, GEMM_BIG, EPI_STD, ctx.st));
+        gemm_run(ctx, g2, batch, GEMM_BIG, EPI_STD);
     }
 }
 

@@ -1,0 +1,36 @@
+"""Times the library's batched complex-FP64 GEMM kernel alone (ss_zgemm_batched) and prints TFLOP/s.
+  python -m paper_1812_01396_b200.gemm_bench [M N K batch [reps]]
+Used for the ncu `--set full` capture of the dominant kernel (profiles/) and for tuning."""
+import sys
+
+import torch
+
+from . import binding
+
+
+def main():
+    a = [int(x) for x in sys.argv[1:]]
+    M, N, K, batch = (a + [2048, 2048, 2048, 16])[:4] if len(a) < 4 else a[:4]
+    reps = a[4] if len(a) > 4 else 5
+    g = torch.Generator(device="cuda").manual_seed(0)
+    A = torch.randn((batch, M, K), dtype=torch.complex128, device="cuda", generator=g)
+    B = torch.randn((batch, K, N), dtype=torch.complex128, device="cuda", generator=g)
+    C = torch.zeros((batch, M, N), dtype=torch.complex128, device="cuda")
+    for _ in range(2):
+        binding.zgemm_batched(A, B, C)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = 1e30
+    for _ in range(reps):
+        e0.record()
+        binding.zgemm_batched(A, B, C)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    err = (C[0] - A[0] @ B[0]).abs().max().item() / (K ** 0.5)
+    print(f"zgemm M={M} N={N} K={K} batch={batch}: {best:.3f} ms  {8.0 * M * N * K * batch / best / 1e9:.2f} TFLOP/s  "
+          f"max err/sqrt(K) {err:.2e}")
+
+
+if __name__ == "__main__":
+    main()
