@@ -153,7 +153,7 @@ def run_reference(args, cfg):
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
-    from paper_1812_01396_b200 import binding, build
+    from paper_1812_01396_b200 import binding, build, sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -171,12 +171,12 @@ def run_ours(args, cfg):
     threads = max(1, (os.cpu_count() or 1) // max(1, world))
     if cfg.kind == "chain":
         p = inputs.perfect_chain_problem(bs, nb, nE * world)
-        idx = np.arange(rank, nE * world, world)
+        idx = sharding.energy_indices(nE * world, rank, world)
         p.E, p.Sigma_L, p.Sigma_R, p.Inj_first = p.E[idx], p.Sigma_L[idx], p.Sigma_R[idx], p.Inj_first[idx]
     else:
         p = inputs.random_problem(bs, nb, 1, 1, seed=cfg.seed, threads=threads)      # H, S only
         grid = inputs.energy_grid(nE * world, cfg.e_lo, cfg.e_hi, cfg.eta)
-        idx = np.arange(rank, nE * world, world)
+        idx = sharding.energy_indices(nE * world, rank, world)
         p.E = grid[idx].copy()
         p.Sigma_L = np.stack([inputs.sigma_block(cfg.seed, int(e), bs, "L") for e in idx])
         p.Sigma_R = np.stack([inputs.sigma_block(cfg.seed, int(e), bs, "R") for e in idx])
@@ -223,12 +223,8 @@ def run_ours(args, cfg):
     ms_total = ev0.elapsed_time(ev1)
     launches = ss.launch_count()
     ss.set_option("profile_gemm", 0)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-        Tall = [torch.empty(nE, dtype=torch.float64, device="cuda") for _ in range(world)]
-        dist.all_gather(Tall, torch.from_numpy(T_last).cuda())
+    ms_total = sharding.max_over_ranks(ms_total, world, device="cuda")
+    T_all = sharding.gather_transmission(T_last, nE * world, rank, world, device="cuda")   # 8 B per energy
     ms_step = ms_total / args.steps
     value = nE * world / (ms_step * 1e-3)
 
@@ -254,10 +250,7 @@ def run_ours(args, cfg):
             e2e_step()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = sharding.max_over_ranks(dt, world, device="cuda")
         h2d = sum(host[k].numel() * 16 for k in host) + nE * 16
         d2h = Xh.numel() * 16 + nE * 8
         e2e = {"value": nE * world * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -283,7 +276,7 @@ def run_ours(args, cfg):
                          "gemm_flops_share": gemm_fl / (flops_step * args.steps)},
             "gpu_launches": int(launches * args.steps),
             "clocks": clocks.summary(),
-            "T_first_energy": float(T_last[0]),
+            "T_first_energy": float(T_all[0]),
         }
         if e2e:
             line["e2e"] = e2e
