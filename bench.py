@@ -32,6 +32,12 @@ UNIT = "solves/s"
 # FP64 roofline denominator: 148 SMs x 64 FP64 FMA/clk/SM x 2 flop x 1.965 GHz; the DMMA
 # microbenchmark in the library (ss_fp64_peak_tflops) measures 37.07 on this pool's B200s and is printed beside it.
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# real flops executed per algorithmic (LAPACK-convention) flop: 4M executes 8 per complex multiply-add, 3M 6
+EXECUTED_RATIO = {False: 1.0, True: 0.75}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant GEMM shape (a1/a4 of C3: M=N=K=2048,
+# batch 16; algorithmic bytes 3 x 16 x 67.1 MB = 3.22e9) from the committed `ncu --set full` captures
+NCU_TRAFFIC = {False: {"bytes": 7.14e9, "note": "profiles/r01_zgemm_ncu_full.md (4M, 2048^3 x16 launch; algorithmic 3.22e9 B)"},
+               True: {"bytes": 6.37e9, "note": "profiles/r01_zgemm3m_ncu_full.md (3M 64x32, 2048^3 x16 launch; algorithmic 3.22e9 B)"}}
 
 
 def parse():
@@ -41,6 +47,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C3", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--gemm-variant", type=int, default=None, help="complex-GEMM kernel variant (binding.GEMM_VARIANTS); "
+                    "default: the library default (3M)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -190,6 +198,10 @@ def run_ours(args, cfg):
     devt = {k: v.cuda(non_blocking=True) for k, v in host.items()}
     torch.cuda.synchronize()
 
+    if args.gemm_variant is not None:
+        binding.set_default_gemm_variant(args.gemm_variant)
+    variant = binding.get_default_gemm_variant()
+    is3m = variant != 0
     ss = binding.SplitSolve(nb, bs, nE)
     ss.set_hamiltonian(devt["H_diag"], devt["H_upper"], devt["S_diag"], devt["S_upper"])
     X = torch.empty((nE, nb * bs, m), dtype=torch.complex128, device="cuda")
@@ -268,9 +280,16 @@ def run_ours(args, cfg):
             "tflops": {"whole_solve": flops_step / (ms_step * 1e-3) / 1e12, "sweep_a1_a4": sweep_tf,
                        "sweep_frac_of_fp64_peak": sweep_tf / FP64_PEAK_NOMINAL_TFLOPS, "flops_per_step": flops_step,
                        "convention": "LAPACK (complex multiply-add = 8 flops), closed form ss_flops"},
-            "roofline": {"bound": "tensor", "kernel": "zgemm_kernel (DMMA.8x8x4, mma.sync f64)", "achieved": gemm_tf,
+            "roofline": {"bound": "tensor",
+                         "kernel": ("zgemm3m_kernel" if is3m else "zgemm_kernel") + f" [{binding.GEMM_VARIANTS[variant]}] "
+                         "(DMMA.8x8x4, mma.sync f64)", "achieved": gemm_tf,
                          "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": gemm_tf / FP64_PEAK_NOMINAL_TFLOPS,
-                         "traffic": None, "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz; no FP64 peak in "
+                         "flops_convention": "algorithmic = 8 M N K per complex GEMM (LAPACK); the 3M kernel executes 6 real "
+                         "flops per complex multiply-add, so frac may exceed the executed-flop pipe utilisation frac_executed",
+                         "executed_over_algorithmic": EXECUTED_RATIO[is3m],
+                         "frac_executed": gemm_tf * EXECUTED_RATIO[is3m] / FP64_PEAK_NOMINAL_TFLOPS,
+                         "traffic": NCU_TRAFFIC[is3m]["bytes"], "traffic_note": NCU_TRAFFIC[is3m]["note"],
+                         "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz; no FP64 peak in "
                          "MEASURED_PEAKS.json", "peak_measured_dmma_microbench": peak_measured,
                          "gemm_launches": gemm_n, "gemm_share_of_step": gemm_ms / ms_total,
                          "gemm_flops_share": gemm_fl / (flops_step * args.steps)},

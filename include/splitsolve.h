@@ -137,7 +137,8 @@ long long ss_launch_count(ss_handle_t h);
 ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long* launches);
 
 /* Options: "nb_lu" (outer LU block, 16..128, multiple of 16; default 128), "transmission" (0/1, default 1:
- * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0). */
+ * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0), "gemm_variant" (see ss_set_default_gemm_variant;
+ * default = the process-wide default at ss_create). */
 ss_status_t ss_set_option(ss_handle_t h, const char* name, int value);
 
 const char* ss_strerror(ss_status_t s);
@@ -163,6 +164,14 @@ ss_status_t ss_zgetrf_batched(int n, int ncols, ss_cplx* AB_dev, int ld, long lo
  * substitution with the upper factor; X[z] (n x nrhs, ldx) at X_dev + z*strideX.  AB is overwritten. */
 ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB_dev, int ld, long long stride, ss_cplx* X_dev, int ldx,
                              long long strideX, int* ipiv_dev, int* info_dev, int batch, void* cuda_stream);
+
+/* Arithmetic / tile shape of the complex GEMM kernel (north_star: "4M or 3M ... whichever reaches the higher fraction
+ * of the chip's FP64 peak"):  0 = 4M (four real products per complex product, 64x64 tile);  1..5 = 3M (three real
+ * products, P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi); 6 instead of 8 real flops per complex multiply-add; rounding
+ * differs, normwise error stays O(u)) with CTA tiles 64x32 (4-stage, default), 64x32 (3-stage), 64x64, 64x96, 128x48.  The process-wide default
+ * (initially 1) applies to handles created afterwards and to the handle-less building blocks above. */
+ss_status_t ss_set_default_gemm_variant(int variant);
+int ss_get_default_gemm_variant(void);
 
 /* FP64 pipe microbenchmark (register-resident mma.sync.m8n8k4.f64 chains on all SMs): returns sustained
  * TFLOP/s over about `ms` milliseconds; the measured roofline denominator bench.py prints beside the nominal one. */

@@ -42,6 +42,8 @@ SIGNATURES = {
     "ss_zgesv_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong, c_void_p,
                                  c_void_p, c_int, c_void_p]),
     "ss_fp64_peak_tflops": (c_int, [c_double, POINTER(c_double)]),
+    "ss_set_default_gemm_variant": (c_int, [c_int]),
+    "ss_get_default_gemm_variant": (c_int, []),
 }
 
 _lib = None
@@ -240,6 +242,17 @@ def zgesv_batched(AB, n):
     _check(load().ss_zgesv_batched(n, nrhs, _dev(AB, "AB"), ncols, n * ncols, _dev(X, "X"), nrhs, n * nrhs,
                                    ipiv.data_ptr(), info.data_ptr(), batch, _stream()), "ss_zgesv_batched")
     return X, ipiv, info
+
+
+GEMM_VARIANTS = {0: "4M 64x64", 1: "3M 64x32 s4", 2: "3M 64x32 s3", 3: "3M 64x64", 4: "3M 64x96", 5: "3M 128x48"}
+
+
+def set_default_gemm_variant(variant: int):
+    _check(load().ss_set_default_gemm_variant(int(variant)), "ss_set_default_gemm_variant")
+
+
+def get_default_gemm_variant() -> int:
+    return int(load().ss_get_default_gemm_variant())
 
 
 def fp64_peak_tflops(ms: float = 200.0) -> float:

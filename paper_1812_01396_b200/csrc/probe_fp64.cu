@@ -44,6 +44,36 @@ __device__ __forceinline__ void mma16816(double (&c)[4], const double (&a)[8], c
                    "d"(b[0]), "d"(b[1]), "d"(b[2]), "d"(b[3]));
 }
 
+// Mixed: even warps issue DMMA chains, odd warps DFMA chains (are the two FP64 paths one physical pipe or two?).
+// flops counted for both; if the sum exceeds the single-path peak the pipes are separate.
+__global__ void k_mixed(double* out, int iters, double fa, double fb, int dfma_every) {
+    const int warp = threadIdx.x >> 5;
+    double s = 0;
+    if (dfma_every > 0 && (warp % dfma_every) == dfma_every - 1) {
+        double acc[8];
+#pragma unroll
+        for (int i = 0; i < 8; i++) acc[i] = threadIdx.x * 1e-3 + i;
+        for (int it = 0; it < iters; it++) {
+#pragma unroll
+            for (int i = 0; i < 8; i++) acc[i] = fma(acc[i], fa, fb);
+        }
+#pragma unroll
+        for (int i = 0; i < 8; i++) s += acc[i];
+    } else {
+        double c[8][2];
+#pragma unroll
+        for (int i = 0; i < 8; i++) { c[i][0] = 0; c[i][1] = 0; }
+        double a = threadIdx.x * 1e-9, b = 1e-9 * (threadIdx.x % 7);
+        for (int it = 0; it < iters; it++) {
+#pragma unroll
+            for (int i = 0; i < 8; i++) mma884(c[i], a, b);
+        }
+#pragma unroll
+        for (int i = 0; i < 8; i++) s += c[i][0] + c[i][1];
+    }
+    if (s == 12345.678) out[0] = s;
+}
+
 template <int NACC>
 __global__ void k_mma884(double* out, int iters) {
     double c[NACC][2];
@@ -202,6 +232,16 @@ int main(int argc, char** argv) {
         printf("DMMA m16n8k16 x2acc warps/SM=%d : %.3f ms %.2f TFLOP/s\n", wps, t * 1e3, 2.0 * 16 * 8 * 16 * 2 * iters * nw / t * 1e-12);
         t = timeit([&] { k_mma16816<1><<<blocks, th>>>(out, iters); });
         printf("DMMA m16n8k16 x1acc warps/SM=%d : %.3f ms %.2f TFLOP/s\n", wps, t * 1e3, 2.0 * 16 * 8 * 16 * 1 * iters * nw / t * 1e-12);
+    }
+    // mixed DMMA + DFMA warps: one pipe or two?
+    for (int every = 2; every <= 4; every *= 2) {
+        int th = 512, blocks = nsm * 2, iters = 4000;     // 32 warps per SM
+        double nw = (double)blocks * th / 32;
+        double nw_dfma = nw / every, nw_dmma = nw - nw_dfma;
+        double t = timeit([&] { k_mixed<<<blocks, th>>>(out, iters, 1.0000001, 1e-9, every); });
+        double fl_dmma = 2.0 * 8 * 8 * 4 * 8 * iters * nw_dmma, fl_dfma = 2.0 * 8 * iters * 32 * nw_dfma;
+        printf("MIXED 1 DFMA warp in %d (same iters): %.3f ms  DMMA %.2f + DFMA %.2f = %.2f TFLOP/s\n", every, t * 1e3,
+               fl_dmma / t * 1e-12, fl_dfma / t * 1e-12, (fl_dmma + fl_dfma) / t * 1e-12);
     }
     // sustained: run ~4 s of DFMA and ~4 s of DMMA m16n8k16, report TF in 0.5 s slices
     if (argc > 1) {

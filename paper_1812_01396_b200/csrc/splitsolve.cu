@@ -11,6 +11,8 @@
 
 using namespace ss;
 
+static int g_default_variant = GV_3M_64x32s4;   // process-wide default GEMM variant (new handles, handle-less building blocks)
+
 struct ss_handle_s {
     int nb = 0, bs = 0, n_energy = 0;
     const cplx *Hd = nullptr, *Hu = nullptr, *Sd = nullptr, *Su = nullptr;
@@ -20,6 +22,7 @@ struct ss_handle_s {
     int nb_lu = 128;
     int want_T = 1;
     int profile_gemm = 0;
+    int gemm_variant = g_default_variant;
     GemmProfile prof;
     // workspace (allocated for ws_nrhs)
     int ws_nrhs = -1;
@@ -187,6 +190,10 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
     }
     if (!strcmp(name, "transmission")) { h->want_T = value ? 1 : 0; return SS_OK; }
     if (!strcmp(name, "profile_gemm")) { h->profile_gemm = value ? 1 : 0; return SS_OK; }
+    if (!strcmp(name, "gemm_variant")) {
+        if (value < 0 || value >= GV_COUNT) return SS_ERR_INVALID_ARG;
+        h->gemm_variant = value; return SS_OK;
+    }
     return SS_ERR_INVALID_ARG;
 }
 
@@ -351,7 +358,7 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     if (h->solved) cudaEventSynchronize(h->ev[2]);        // E_pinned of the previous call is free again
     memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
-    Ctx ctx; ctx.st = stream;
+    Ctx ctx; ctx.st = stream; ctx.variant = h->gemm_variant;
     h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
     ctx.prof = h->profile_gemm ? &h->prof : nullptr;
     if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
@@ -525,7 +532,7 @@ extern "C" ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const
     if (lda < K || ldb < N || ldc < N) return SS_ERR_INVALID_ARG;
     GemmArgs g = gemm_std(M, N, K, alpha, bp_strided((const cplx*)(A ? A : C), sA), lda, bp_strided((const cplx*)(B ? B : C), sB), ldb,
                           beta, bp_strided((cplx*)C, sC), ldc);
-    cudaError_t e = gemm_launch(g, batch, GEMM_BIG, EPI_STD, (cudaStream_t)stream);
+    cudaError_t e = gemm_launch(g, batch, GEMM_BIG, EPI_STD, (cudaStream_t)stream, g_default_variant);
     if (e != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }
@@ -541,7 +548,7 @@ static ss_status_t lu_common(int n, int nrhs_solve, int ncols, ss_cplx* AB, int 
         cudaGetLastError(); return SS_ERR_ALLOC;
     }
     w.tinv_blocks = nblk * batch; w.ipiv = ipiv; w.ipiv_stride = n; w.info = info;
-    Ctx ctx; ctx.st = st;
+    Ctx ctx; ctx.st = st; ctx.variant = g_default_variant;
     cudaMemsetAsync(info, 0, sizeof(int) * (size_t)batch, st);
     BPtr Ab = bp_strided((cplx*)AB, stride);
     lu_factor(ctx, Ab, ld, n, ncols, batch, 128, w, 0);
@@ -562,6 +569,14 @@ extern "C" ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB, int ld, lo
     if (nrhs < 0 || (nrhs > 0 && (!X || ldx < nrhs))) return SS_ERR_INVALID_ARG;
     return lu_common(n, nrhs, n + nrhs, AB, ld, stride, X, ldx, sX, ipiv, info, batch, stream);
 }
+
+extern "C" ss_status_t ss_set_default_gemm_variant(int variant) {
+    if (variant < 0 || variant >= GV_COUNT) return SS_ERR_INVALID_ARG;
+    g_default_variant = variant;
+    return SS_OK;
+}
+
+extern "C" int ss_get_default_gemm_variant(void) { return g_default_variant; }
 
 extern "C" ss_status_t ss_fp64_peak_tflops(double ms, double* tflops) {
     if (!tflops || ms <= 0) return SS_ERR_INVALID_ARG;

@@ -247,7 +247,7 @@ static cudaError_t gemm_launch_t(GemmArgs a, int batch, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st) {
+static cudaError_t gemm4m_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st) {
     if (cfg == GEMM_TALL) return gemm_launch_t<CfgTall, 128, 32, 4, 1, 8, 4, EPI_STD, 2>(a, batch, st);
     if (epi == EPI_SCHUR) return gemm_launch_t<CfgBig, 64, 64, 2, 2, 8, 4, EPI_SCHUR, 2>(a, batch, st);
     return gemm_launch_t<CfgBig, 64, 64, 2, 2, 8, 4, EPI_STD, 2>(a, batch, st);

@@ -1,0 +1,268 @@
+// Batched complex-FP64 GEMM, "3M" arithmetic on the FP64 tensor pipe (DMMA.8x8x4 via mma.sync.m8n8k4.f64), sm_100a.
+//
+// Same contract and epilogues as zgemm.cuh (the updates inside a2/a3, a5-a7's products;
+// PAPER.md L186 "two matrix-matrix multiplications" per Q_i).  north_star: "a complex-FP64 GEMM (4M or 3M over real
+// FP64 MMA or FMA, whichever ... reach[es] the higher fraction of the chip's FP64 peak)".
+//
+// 3M: with A = Ar + i Ai, B = Br + i Bi, three REAL products
+//       P1 = Ar Br,   P2 = Ai Bi,   P3 = (Ar + Ai)(Br + Bi)
+//     give  Re C = P1 - P2,  Im C = P3 - P1 - P2 :  6 instead of 8 real flops per complex multiply-add.
+// The operands stay interleaved (re, im) exactly as stored: one LDS.128 of the staged tile IS the (Ar, Ai) -- resp.
+// (Br, Bi) -- fragment pair of m8n8k4 (A: lane holds row lane>>2, k lane&3; B: k lane&3, column lane>>2), the sum
+// fragment costs one DADD, and every DMMA covers 8 x 8 COMPLEX outputs x 4 complex k.  Each thread owns, per m8n8
+// tile, the complex outputs (row lane>>2, columns 2(lane&3), 2(lane&3)+1) -- a 32-byte contiguous store.
+//
+// Staging: cp.async 16 B = one complex element per request, zero-filled out of range (M, N, K, leading dimensions
+// and sub-matrix offsets arbitrary), STAGES-deep ring, one __syncthreads per K chunk.  Shared-memory row strides are
+// chosen so that both fragment LDS.128 patterns are bank-conflict-free: A stride == 8 (mod 16) doubles, B stride
+// == 4 (mod 16) doubles.
+#pragma once
+#include "zgemm.cuh"
+
+namespace ss {
+
+template <int BM_, int BN_, int WARPS_M_, int WARPS_N_, int KC_, int STAGES_, int MINB_>
+struct Gemm3Cfg {
+    static constexpr int BM = BM_, BN = BN_, WARPS_M = WARPS_M_, WARPS_N = WARPS_N_, KC = KC_, STAGES = STAGES_, MINB = MINB_;
+    static constexpr int NT = WARPS_M * WARPS_N * 32;
+    static constexpr int WM = BM / WARPS_M, WN = BN / WARPS_N;   // warp tile, complex elements
+    static constexpr int MI = WM / 8, NJ = WN / 8;               // m8 / n8 tiles per warp
+    static constexpr int LDA_S = 2 * KC + 8;                     // doubles
+    static constexpr int LDB_S = 2 * BN + 4;                     // doubles
+    static constexpr int STAGE_D = BM * LDA_S + KC * LDB_S;      // doubles per stage
+    static constexpr int SMEM_BYTES = STAGES * STAGE_D * 8;
+    static constexpr int CH_A = BM * KC, CH_B = KC * BN;         // 16-byte chunks per stage
+    static constexpr int ITER_A = (CH_A + NT - 1) / NT, ITER_B = (CH_B + NT - 1) / NT;
+    static_assert(WM % 8 == 0 && WN % 8 == 0 && KC % 4 == 0, "warp tile");
+    static_assert((2 * KC) % 16 == 0 && (2 * BN) % 16 == 0, "bank layout");
+    static_assert(LDA_S % 16 == 8 && LDB_S % 16 == 4, "bank layout");
+};
+
+template <class Cfg, int EPI>
+__global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmArgs p) {
+    extern __shared__ __align__(16) double smem[];
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = Cfg::KC, STAGES = Cfg::STAGES;
+    constexpr int NT = Cfg::NT, MI = Cfg::MI, NJ = Cfg::NJ, LDA_S = Cfg::LDA_S, LDB_S = Cfg::LDB_S;
+    constexpr int STAGE_D = Cfg::STAGE_D;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int z = blockIdx.y;
+
+    // grouped rasterisation: 8 tile rows share the B columns in L2
+    int tile_m, tile_n;
+    {
+        constexpr int GM = 8;
+        int pid = blockIdx.x;
+        int per_group = GM * p.tiles_n;
+        int group = pid / per_group;
+        int first_m = group * GM;
+        int gsize = min(p.tiles_m - first_m, GM);
+        int r = pid - group * per_group;
+        tile_m = first_m + r % gsize;
+        tile_n = r / gsize;
+    }
+    const int m0 = tile_m * BM, n0 = tile_n * BN;
+    const int M = p.M, N = p.N, K = p.K;
+
+    const cplx* __restrict__ Ag = bptr(p.A, z);
+    const cplx* __restrict__ Bg = bptr(p.B, z);
+
+    // ---- per-thread staging descriptors (chunk c of the A tile: row c / KC, k c % KC; of the B tile: k c / BN, col c % BN)
+    const cplx* a_src[Cfg::ITER_A]; int a_dst[Cfg::ITER_A]; int a_kc[Cfg::ITER_A]; bool a_ok[Cfg::ITER_A];
+#pragma unroll
+    for (int q = 0; q < Cfg::ITER_A; q++) {
+        int c = tid + q * NT;
+        int row = c / KC, kc = c % KC;
+        a_kc[q] = (c < Cfg::CH_A) ? kc : (1 << 28);          // beyond the tile: never in range
+        a_ok[q] = (c < Cfg::CH_A) && (m0 + row) < M;
+        a_src[q] = Ag + (long long)(a_ok[q] ? (m0 + row) : 0) * p.lda + kc;
+        a_dst[q] = (c < Cfg::CH_A) ? row * LDA_S + 2 * kc : -1;
+    }
+    const cplx* b_src[Cfg::ITER_B]; int b_dst[Cfg::ITER_B]; int b_kr[Cfg::ITER_B]; bool b_ok[Cfg::ITER_B];
+#pragma unroll
+    for (int q = 0; q < Cfg::ITER_B; q++) {
+        int c = tid + q * NT;
+        int kr = c / BN, col = c % BN;
+        b_kr[q] = (c < Cfg::CH_B) ? kr : (1 << 28);
+        b_ok[q] = (c < Cfg::CH_B) && (n0 + col) < N;
+        b_src[q] = Bg + (long long)kr * p.ldb + (b_ok[q] ? (n0 + col) : 0);
+        b_dst[q] = (c < Cfg::CH_B) ? BM * LDA_S + kr * LDB_S + 2 * col : -1;
+    }
+
+    auto load_stage = [&](int kt, int stage) {
+        double* sbase = smem + stage * STAGE_D;
+        const int k0 = kt * KC;
+#pragma unroll
+        for (int q = 0; q < Cfg::ITER_A; q++) {
+            if (a_dst[q] < 0) continue;
+            bool ok = a_ok[q] && (k0 + a_kc[q] < K);
+            cp_async16(sbase + a_dst[q], ok ? (const void*)(a_src[q] + k0) : (const void*)Ag, ok ? 16 : 0);
+        }
+#pragma unroll
+        for (int q = 0; q < Cfg::ITER_B; q++) {
+            if (b_dst[q] < 0) continue;
+            bool ok = b_ok[q] && (k0 + b_kr[q] < K);
+            cp_async16(sbase + b_dst[q], ok ? (const void*)(b_src[q] + (long long)k0 * p.ldb) : (const void*)Bg, ok ? 16 : 0);
+        }
+    };
+
+    // ---- fragment offsets (doubles, within a stage)
+    const int wm0 = (warp / Cfg::WARPS_N) * Cfg::WM, wn0 = (warp % Cfg::WARPS_N) * Cfg::WN;
+    const int a_off = (wm0 + g) * LDA_S + 2 * t;                        // + 8 i LDA_S + 8 ks
+    const int b_off = BM * LDA_S + t * LDB_S + 2 * (wn0 + g);           // + 16 j + 4 ks LDB_S
+
+    double P1[MI][NJ][2], P2[MI][NJ][2], P3[MI][NJ][2];
+#pragma unroll
+    for (int i = 0; i < MI; i++)
+#pragma unroll
+        for (int j = 0; j < NJ; j++) {
+            P1[i][j][0] = P1[i][j][1] = 0.0;
+            P2[i][j][0] = P2[i][j][1] = 0.0;
+            P3[i][j][0] = P3[i][j][1] = 0.0;
+        }
+
+    const int KT = (K + KC - 1) / KC;
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; s++) {
+        if (s < KT) load_stage(s, s);
+        cp_async_commit();
+    }
+
+    for (int kt = 0; kt < KT; kt++) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            int nk = kt + STAGES - 1;
+            if (nk < KT) load_stage(nk, nk % STAGES);
+            cp_async_commit();
+        }
+        const double* sS = smem + (kt % STAGES) * STAGE_D;
+#pragma unroll
+        for (int ks = 0; ks < KC / 4; ks++) {
+            double ar[MI], ai[MI], as[MI], br[NJ], bi[NJ], bs[NJ];
+#pragma unroll
+            for (int i = 0; i < MI; i++) {
+                double2 v = *reinterpret_cast<const double2*>(sS + a_off + 8 * i * LDA_S + 8 * ks);
+                ar[i] = v.x; ai[i] = v.y; as[i] = v.x + v.y;
+            }
+#pragma unroll
+            for (int j = 0; j < NJ; j++) {
+                double2 v = *reinterpret_cast<const double2*>(sS + b_off + 16 * j + 4 * ks * LDB_S);
+                br[j] = v.x; bi[j] = v.y; bs[j] = v.x + v.y;
+            }
+#pragma unroll
+            for (int i = 0; i < MI; i++)
+#pragma unroll
+                for (int j = 0; j < NJ; j++) {
+                    dmma884(P1[i][j][0], P1[i][j][1], ar[i], br[j]);
+                    dmma884(P2[i][j][0], P2[i][j][1], ai[i], bi[j]);
+                    dmma884(P3[i][j][0], P3[i][j][1], as[i], bs[j]);
+                }
+        }
+    }
+    cp_async_wait<0>();
+
+    // ---- epilogue: thread owns complex C[m0+wm0+8i+g][n0+wn0+8j+2t+h], h = 0, 1
+    cplx* __restrict__ Cg = bptr(p.C, z);
+    if (EPI == EPI_STD) {
+        const cplx* Cin = (p.beta != 0.0) ? bptr(p.Cin, z) : nullptr;
+        const double alpha = p.alpha, beta = p.beta;
+#pragma unroll
+        for (int i = 0; i < MI; i++) {
+            int row = m0 + wm0 + 8 * i + g;
+            if (row >= M) continue;
+#pragma unroll
+            for (int j = 0; j < NJ; j++) {
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    int col = n0 + wn0 + 8 * j + 2 * t + h;
+                    if (col >= N) continue;
+                    double re = P1[i][j][h] - P2[i][j][h];
+                    double im = P3[i][j][h] - P1[i][j][h] - P2[i][j][h];
+                    cplx o = make_c(alpha * re, alpha * im);
+                    if (Cin) {
+                        cplx c = Cin[(long long)row * p.ldcin + col];
+                        o.re = fma(beta, c.re, o.re);
+                        o.im = fma(beta, c.im, o.im);
+                    }
+                    Cg[(long long)row * p.ldc + col] = o;
+                }
+            }
+        }
+    } else {
+        const cplx Ee = p.E[z >> 1];
+        const cplx* __restrict__ Sg = bptr(p.S, z);
+        const cplx* __restrict__ Hg = bptr(p.H, z);
+#pragma unroll
+        for (int i = 0; i < MI; i++) {
+            int row = m0 + wm0 + 8 * i + g;
+            if (row >= M) continue;
+#pragma unroll
+            for (int j = 0; j < NJ; j++) {
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    int col = n0 + wn0 + 8 * j + 2 * t + h;
+                    if (col >= N) continue;
+                    double re = P1[i][j][h] - P2[i][j][h];
+                    double im = P3[i][j][h] - P1[i][j][h] - P2[i][j][h];
+                    long long off = (long long)row * p.lds + col;
+                    cplx s = Sg[off], hh = Hg[off];
+                    cplx d = cmul(Ee, s);
+                    Cg[(long long)row * p.ldc + col] = make_c(d.re - hh.re - re, d.im - hh.im - im);
+                }
+            }
+        }
+    }
+}
+
+template <class Cfg, int EPI>
+static cudaError_t gemm3m_launch_t(GemmArgs a, int batch, cudaStream_t st) {
+    auto kern = zgemm3m_kernel<Cfg, EPI>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    a.tiles_m = (a.M + Cfg::BM - 1) / Cfg::BM;
+    a.tiles_n = (a.N + Cfg::BN - 1) / Cfg::BN;
+    if (a.tiles_m == 0 || a.tiles_n == 0 || batch == 0) return cudaSuccess;
+    dim3 grid((unsigned)(a.tiles_m * a.tiles_n), (unsigned)batch, 1);
+    kern<<<grid, Cfg::NT, Cfg::SMEM_BYTES, st>>>(a);
+    return cudaGetLastError();
+}
+
+// tile configurations.  Measured on B200 at M=N=K=2048 x 16 (profiles/r01_gemm_variants.md): the small tile with
+// three independent CTAs per SM wins (42.0 TFLOP/s LAPACK-convention vs 34.1 for 4M): with one CTA per SM every
+// __syncthreads idles the whole DMMA pipe, and the larger warp tiles do not fit 3 accumulator sets in registers.
+using C3_64x32s4 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3>;      // 4 warps of 32x16, 4-stage ring, 3 CTAs/SM   (default)
+using C3_64x32s3 = Gemm3Cfg<64, 32, 2, 2, 8, 3, 3>;      // same, 3-stage ring
+using C3_64x64 = Gemm3Cfg<64, 64, 2, 4, 16, 3, 1>;       // 8 warps of 32x16, 1 CTA/SM
+using C3_64x96 = Gemm3Cfg<64, 96, 2, 4, 16, 3, 1>;       // 8 warps of 32x24
+using C3_128x48 = Gemm3Cfg<128, 48, 4, 2, 16, 3, 1>;     // 8 warps of 32x24
+using C3_Tall = Gemm3Cfg<128, 32, 4, 2, 16, 3, 1>;       // one CTA owns all (<=128) rows of its columns: in-place L^-1 * A12
+
+// GEMM variants: 0 = 4M (zgemm.cuh), 1.. = 3M tile shapes.  GEMM_TALL always maps to the one-CTA-per-column
+// configuration of the same arithmetic.
+enum { GV_4M = 0, GV_3M_64x32s4 = 1, GV_3M_64x32s3 = 2, GV_3M_64x64 = 3, GV_3M_64x96 = 4, GV_3M_128x48 = 5, GV_COUNT = 6 };
+
+template <class Cfg>
+static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_t st) {
+    if (epi == EPI_SCHUR) return gemm3m_launch_t<Cfg, EPI_SCHUR>(a, batch, st);
+    return gemm3m_launch_t<Cfg, EPI_STD>(a, batch, st);
+}
+
+static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st, int variant) {
+    if (variant == GV_4M) return gemm4m_launch(a, batch, cfg, epi, st);
+    if (cfg == GEMM_TALL) return gemm3m_launch_t<C3_Tall, EPI_STD>(a, batch, st);
+    switch (variant) {
+        case GV_3M_64x32s3: return gemm3m_epi<C3_64x32s3>(a, batch, epi, st);
+        case GV_3M_64x64: return gemm3m_epi<C3_64x64>(a, batch, epi, st);
+        case GV_3M_64x96: return gemm3m_epi<C3_64x96>(a, batch, epi, st);
+        case GV_3M_128x48: return gemm3m_epi<C3_128x48>(a, batch, epi, st);
+        default: return gemm3m_epi<C3_64x32s4>(a, batch, epi, st);
+    }
+}
+
+}  // namespace ss

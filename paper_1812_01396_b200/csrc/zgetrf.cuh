@@ -21,7 +21,7 @@
 #pragma once
 #include <cooperative_groups.h>
 #include <vector>
-#include "zgemm.cuh"
+#include "zgemm3m.cuh"
 
 namespace ss {
 namespace cg = cooperative_groups;
@@ -315,6 +315,7 @@ struct Ctx {
     long long launches = 0;
     cudaError_t err = cudaSuccess;
     GemmProfile* prof = nullptr;
+    int variant = GV_4M;            // GEMM arithmetic / tile variant (zgemm3m.cuh)
     void note(cudaError_t e) { if (err == cudaSuccess && e != cudaSuccess) err = e; launches++; }
 };
 
@@ -327,13 +328,13 @@ static void gemm_run(Ctx& ctx, const GemmArgs& g, int batch, int cfg, int epi) {
             pr->ev.push_back(a); pr->ev.push_back(b);
         }
         cudaEventRecord(pr->ev[pr->used], ctx.st);
-        ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st));
+        ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st, ctx.variant));
         cudaEventRecord(pr->ev[pr->used + 1], ctx.st);
         pr->used += 2;
         pr->flops += 8.0 * g.M * g.N * g.K * batch;
         pr->launches++;
     } else {
-        ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st));
+        ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st, ctx.variant));
     }
 }
 

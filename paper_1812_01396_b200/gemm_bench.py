@@ -1,7 +1,8 @@
-"""Times the library's batched complex-FP64 GEMM kernel alone (ss_zgemm_batched) and prints TFLOP/s.
-  python -m paper_1812_01396_b200.gemm_bench [M N K batch [reps]]
+"""Times the library's batched complex-FP64 GEMM kernel alone (ss_zgemm_batched) and prints TFLOP/s
+(LAPACK convention: 8 flops per complex multiply-add, whatever the variant executes).
+  python -m paper_1812_01396_b200.gemm_bench [M N K batch [reps]] [--variant V[,V...]]
 Used for the ncu `--set full` capture of the dominant kernel (profiles/) and for tuning."""
-import sys
+import argparse
 
 import torch
 
@@ -9,27 +10,36 @@ from . import binding
 
 
 def main():
-    a = [int(x) for x in sys.argv[1:]]
-    M, N, K, batch = (a + [2048, 2048, 2048, 16])[:4] if len(a) < 4 else a[:4]
+    ap = argparse.ArgumentParser()
+    ap.add_argument("dims", nargs="*", type=int)
+    ap.add_argument("--variant", default=None, help="comma-separated GEMM variants (binding.GEMM_VARIANTS); default: library default")
+    args = ap.parse_args()
+    a = args.dims
+    M, N, K, batch = (a + [2048, 2048, 2048, 16][len(a):])[:4]
     reps = a[4] if len(a) > 4 else 5
+    variants = [binding.get_default_gemm_variant()] if args.variant is None else [int(v) for v in args.variant.split(",")]
     g = torch.Generator(device="cuda").manual_seed(0)
     A = torch.randn((batch, M, K), dtype=torch.complex128, device="cuda", generator=g)
     B = torch.randn((batch, K, N), dtype=torch.complex128, device="cuda", generator=g)
     C = torch.zeros((batch, M, N), dtype=torch.complex128, device="cuda")
-    for _ in range(2):
-        binding.zgemm_batched(A, B, C)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    best = 1e30
-    for _ in range(reps):
-        e0.record()
-        binding.zgemm_batched(A, B, C)
-        e1.record()
+    ref = A[0] @ B[0]
+    for v in variants:
+        binding.set_default_gemm_variant(v)
+        C.zero_()
+        for _ in range(2):
+            binding.zgemm_batched(A, B, C)
         torch.cuda.synchronize()
-        best = min(best, e0.elapsed_time(e1))
-    err = (C[0] - A[0] @ B[0]).abs().max().item() / (K ** 0.5)
-    print(f"zgemm M={M} N={N} K={K} batch={batch}: {best:.3f} ms  {8.0 * M * N * K * batch / best / 1e9:.2f} TFLOP/s  "
-          f"max err/sqrt(K) {err:.2e}")
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = 1e30
+        for _ in range(reps):
+            e0.record()
+            binding.zgemm_batched(A, B, C)
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        err = (C[0] - ref).abs().max().item() / (K ** 0.5)
+        print(f"zgemm[{binding.GEMM_VARIANTS[v]}] M={M} N={N} K={K} batch={batch}: {best:.3f} ms  "
+              f"{8.0 * M * N * K * batch / best / 1e9:.2f} TFLOP/s  max err/sqrt(K) {err:.2e}", flush=True)
 
 
 if __name__ == "__main__":

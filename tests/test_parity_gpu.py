@@ -56,16 +56,31 @@ def check_against_oracle(p, out, energies=None, solver=dense):
 # ------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("M,N,K,batch", [(64, 64, 64, 1), (1, 1, 1, 2), (37, 53, 29, 3), (130, 70, 200, 2),
                                          (200, 16, 3, 2), (5, 300, 17, 1), (64, 64, 0, 1)])
-def test_zgemm_batched_vs_numpy(lib, M, N, K, batch):
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+def test_zgemm_batched_vs_numpy(lib, M, N, K, batch, variant):
+    """Every GEMM variant (0 = 4M, 1..5 = 3M tile shapes) against numpy.matmul, normwise bound (3M's error bound is
+    normwise, not componentwise: Higham, Accuracy and Stability of Numerical Algorithms, §23.2.4)."""
     A = inputs.complex_gaussian(1, 50, M, (batch, M, K), 1.0)
     B = inputs.complex_gaussian(1, 51, N, (batch, K, N), 1.0)
     C0 = inputs.complex_gaussian(1, 52, K, (batch, M, N), 1.0)
-    for alpha, beta in ((1.0, 0.0), (-1.0, 1.0), (0.5, -2.0)):
-        C = dev(C0.copy())
-        lib.zgemm_batched(dev(A), dev(B), C, alpha, beta)
-        want = alpha * np.matmul(A, B) + beta * C0
-        scale = (np.abs(A).max() * np.abs(B).max() * K if K else 0.0) + np.abs(C0).max() * abs(beta) + 1e-300
-        assert np.abs(C.cpu().numpy() - want).max() <= 1e-14 * scale * 4
+    default = lib.get_default_gemm_variant()
+    try:
+        lib.set_default_gemm_variant(variant)
+        for alpha, beta in ((1.0, 0.0), (-1.0, 1.0), (0.5, -2.0)):
+            C = dev(C0.copy())
+            lib.zgemm_batched(dev(A), dev(B), C, alpha, beta)
+            want = alpha * np.matmul(A, B) + beta * C0
+            scale = (np.abs(A).max() * np.abs(B).max() * K if K else 0.0) + np.abs(C0).max() * abs(beta) + 1e-300
+            assert np.abs(C.cpu().numpy() - want).max() <= 1e-14 * scale * 4
+    finally:
+        lib.set_default_gemm_variant(default)
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+def test_hot_path_with_every_gemm_variant(lib, variant):
+    p = inputs.random_problem(150, 3, 2, 37, seed=13, inj_last=True)
+    out = run_gpu(lib, p, options={"gemm_variant": variant})
+    check_against_oracle(p, out)
 
 
 @pytest.mark.parametrize("n,nrhs,batch", [(1, 1, 1), (7, 3, 2), (16, 16, 1), (33, 5, 3), (128, 40, 2), (200, 37, 2),
