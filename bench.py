@@ -49,6 +49,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--gemm-variant", type=int, default=None, help="complex-GEMM kernel variant (binding.GEMM_VARIANTS); "
                     "default: the library default (3M)")
+    ap.add_argument("--stream-groups", type=int, default=None, help="stream groups the energies are split over "
+                    "(library default 4; 1 = single stream)")
+    ap.add_argument("--trace", default=None, help="write the phase timeline of the last timed step to this CSV")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -203,6 +206,10 @@ def run_ours(args, cfg):
     variant = binding.get_default_gemm_variant()
     is3m = variant != 0
     ss = binding.SplitSolve(nb, bs, nE)
+    groups = 4 if args.stream_groups is None else args.stream_groups
+    ss.set_option("stream_groups", groups)
+    if args.trace:
+        ss.set_option("trace", 1)
     ss.set_hamiltonian(devt["H_diag"], devt["H_upper"], devt["S_diag"], devt["S_upper"])
     X = torch.empty((nE, nb * bs, m), dtype=torch.complex128, device="cuda")
 
@@ -219,7 +226,11 @@ def run_ours(args, cfg):
         step()
     T_last = ss.transmission()
     sweep_ms, gemm_ms, gemm_fl, gemm_n = [], 0.0, 0.0, 0
-    ss.set_option("profile_gemm", 1)                 # CUDA events around every GEMM launch inside the timed region
+    serial = min(groups, nE) <= 1
+    # CUDA events around every GEMM launch.  On a single stream they are taken inside the timed region; with stream
+    # groups kernels of different groups overlap, so a launch's event-to-event time is not the kernel's own duration:
+    # then the per-launch GEMM timing comes from one extra step with stream_groups = 1, right after the timed region.
+    ss.set_option("profile_gemm", 1 if (serial or args.trace) else 0)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     with ClockSampler(local) as clocks:
@@ -228,12 +239,25 @@ def run_ours(args, cfg):
             step()
             T_last = ss.transmission()               # the step's result: synchronises, 8 B per energy
             sweep_ms.append(ss.phase_ms(0))
-            a, b, c = ss.gemm_profile()
-            gemm_ms += a; gemm_fl += b; gemm_n += c
+            if serial:
+                a, b, c = ss.gemm_profile()
+                gemm_ms += a; gemm_fl += b; gemm_n += c
         ev1.record()
         barrier()
     ms_total = ev0.elapsed_time(ev1)
     launches = ss.launch_count()
+    gemm_ref_ms = ms_total
+    if args.trace:
+        ss.trace_write(args.trace)
+        ss.set_option("trace", 0)
+    if not serial:
+        ss.set_option("stream_groups", 1)
+        ss.set_option("profile_gemm", 1)
+        step()
+        ss.transmission()
+        gemm_ms, gemm_fl, gemm_n = ss.gemm_profile()
+        gemm_ref_ms = ss.phase_ms(2)
+        ss.set_option("stream_groups", groups)
     ss.set_option("profile_gemm", 0)
     ms_total = sharding.max_over_ranks(ms_total, world, device="cuda")
     T_all = sharding.gather_transmission(T_last, nE * world, rank, world, device="cuda")   # 8 B per energy
@@ -275,7 +299,7 @@ def run_ours(args, cfg):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "c128 (f64 re/im)", "data": "synthetic",
             "config": {"workload": cfg.name, "bs": bs, "nb": nb, "n_energy_per_gpu": nE, "nrhs": m,
-                       "parallelism": f"energy-parallel x{world}", "l2": "inputs larger than L2 (H,S,slots >> 126 MB)"
+                       "parallelism": f"energy-parallel x{world}", "stream_groups": groups, "l2": "inputs larger than L2 (H,S,slots >> 126 MB)"
                        if bs >= 512 else "small workload: inputs fit L2 (launch-bound config)"},
             "tflops": {"whole_solve": flops_step / (ms_step * 1e-3) / 1e12, "sweep_a1_a4": sweep_tf,
                        "sweep_frac_of_fp64_peak": sweep_tf / FP64_PEAK_NOMINAL_TFLOPS, "flops_per_step": flops_step,
@@ -291,8 +315,11 @@ def run_ours(args, cfg):
                          "traffic": NCU_TRAFFIC[is3m]["bytes"], "traffic_note": NCU_TRAFFIC[is3m]["note"],
                          "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz; no FP64 peak in "
                          "MEASURED_PEAKS.json", "peak_measured_dmma_microbench": peak_measured,
-                         "gemm_launches": gemm_n, "gemm_share_of_step": gemm_ms / ms_total,
-                         "gemm_flops_share": gemm_fl / (flops_step * args.steps)},
+                         "gemm_launches": gemm_n, "gemm_share_of_step": gemm_ms / gemm_ref_ms,
+                         "gemm_flops_share": gemm_fl / (flops_step * (args.steps if serial else 1)),
+                         "measured_in": "timed region (single stream)" if serial else
+                         "one extra step with stream_groups=1 right after the timed region (kernels of different stream "
+                         f"groups overlap in the timed region); that serial step took {gemm_ref_ms:.1f} ms"},
             "gpu_launches": int(launches * args.steps),
             "clocks": clocks.summary(),
             "T_first_energy": float(T_all[0]),

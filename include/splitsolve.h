@@ -131,6 +131,10 @@ ss_status_t ss_phase_ms(ss_handle_t h, int phase, float* ms);
 /* Number of kernel launches the last ss_solve enqueued. */
 long long ss_launch_count(ss_handle_t h);
 
+/* Writes the phase timeline of the last ss_solve (option "trace" = 1, stream_groups > 1) as CSV
+ * "group,class,start_ms,end_ms" (times relative to the start of the solve) to `path`.  Synchronises. */
+ss_status_t ss_trace_write(ss_handle_t h, const char* path);
+
 /* With option "profile_gemm" = 1, every launch of the GEMM kernel in ss_solve is bracketed by CUDA events on the
  * solve's stream; this returns, for the last ss_solve, the summed device time of those launches (ms), their
  * algorithmic flops (8 M N K per complex GEMM) and their number.  Synchronises. */
@@ -138,7 +142,12 @@ ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long*
 
 /* Options: "nb_lu" (outer LU block, 16..128, multiple of 16; default 128), "transmission" (0/1, default 1:
  * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0), "gemm_variant" (see ss_set_default_gemm_variant;
- * default = the process-wide default at ss_create). */
+ * default = the process-wide default at ss_create), "trace" (0/1, default 0: record a CUDA-event
+ * timeline of every group's high-/low-priority phases, see ss_trace_write), "stream_groups" (1..16,
+ * default 4: the energy points are split
+ * over that many groups, each with a high-priority stream for the latency-bound panel kernels and a low-priority
+ * stream for the large GEMMs, forked from and joined back to the stream given to ss_solve; 1 = everything on that
+ * stream). */
 ss_status_t ss_set_option(ss_handle_t h, const char* name, int value);
 
 const char* ss_strerror(ss_status_t s);

@@ -34,6 +34,7 @@ SIGNATURES = {
     "ss_phase_ms": (c_int, [c_void_p, c_int, POINTER(c_float)]),
     "ss_gemm_profile": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_longlong)]),
     "ss_launch_count": (c_longlong, [c_void_p]),
+    "ss_trace_write": (c_int, [c_void_p, c_char_p]),
     "ss_set_option": (c_int, [c_void_p, c_char_p, c_int]),
     "ss_strerror": (c_char_p, [c_int]),
     "ss_zgemm_batched": (c_int, [c_int, c_int, c_int, c_double, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong,
@@ -186,6 +187,9 @@ class SplitSolve:
         ms, fl, n = c_double(), c_double(), c_longlong()
         _check(load().ss_gemm_profile(self._h, byref(ms), byref(fl), byref(n)), "ss_gemm_profile")
         return float(ms.value), float(fl.value), int(n.value)
+
+    def trace_write(self, path: str):
+        _check(load().ss_trace_write(self._h, str(path).encode()), "ss_trace_write")
 
     def launch_count(self) -> int:
         return int(load().ss_launch_count(self._h))

@@ -23,7 +23,14 @@ struct ss_handle_s {
     int want_T = 1;
     int profile_gemm = 0;
     int gemm_variant = g_default_variant;
+    int stream_groups = 4;
+    int want_trace = 0;
+    std::vector<TraceRec> trace;
     GemmProfile prof;
+    // stream groups (created on first use): per group a high- and a low-priority stream and two events
+    struct GroupRes { cudaStream_t hi = nullptr, lo = nullptr; cudaEvent_t ev_sw = nullptr, ev_mark = nullptr; };
+    std::vector<GroupRes> groups;
+    cudaEvent_t ev_fork = nullptr;
     // workspace (allocated for ws_nrhs)
     int ws_nrhs = -1;
     cplx *slots = nullptr, *aug = nullptr, *aop = nullptr, *tinv = nullptr, *raug = nullptr, *wz = nullptr;
@@ -150,8 +157,16 @@ extern "C" ss_status_t ss_destroy(ss_handle_t h) {
     for (int i = 0; i < 4; i++) free_dev(h->own_hs[i]);
     for (int i = 0; i < 3; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     for (cudaEvent_t e : h->prof.ev) cudaEventDestroy(e);
+    for (auto& r : h->trace) { cudaEventDestroy(r.t0); cudaEventDestroy(r.t1); }
     if (h->E_pinned) cudaFreeHost(h->E_pinned);
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
+    for (auto& g : h->groups) {
+        if (g.hi) cudaStreamDestroy(g.hi);
+        if (g.lo) cudaStreamDestroy(g.lo);
+        if (g.ev_sw) cudaEventDestroy(g.ev_sw);
+        if (g.ev_mark) cudaEventDestroy(g.ev_mark);
+    }
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     delete h;
     return SS_OK;
 }
@@ -190,6 +205,11 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
     }
     if (!strcmp(name, "transmission")) { h->want_T = value ? 1 : 0; return SS_OK; }
     if (!strcmp(name, "profile_gemm")) { h->profile_gemm = value ? 1 : 0; return SS_OK; }
+    if (!strcmp(name, "stream_groups")) {
+        if (value < 1 || value > 16) return SS_ERR_INVALID_ARG;
+        h->stream_groups = value; return SS_OK;
+    }
+    if (!strcmp(name, "trace")) { h->want_trace = value ? 1 : 0; return SS_OK; }
     if (!strcmp(name, "gemm_variant")) {
         if (value < 0 || value >= GV_COUNT) return SS_ERR_INVALID_ARG;
         h->gemm_variant = value; return SS_OK;
@@ -225,126 +245,173 @@ static void launch_form(Ctx& ctx, FormSide s0, FormSide s1, const cplx* E, BPtr 
     ctx.note(cudaGetLastError());
 }
 
-// a0-a4: Algorithm 1 and its mirror (L167), all energies and both columns in lockstep.
-// Chain z = 2*e + col.  Slot layout per chain (nb+1 slots of bs x bs): column 0 keeps X_i in slot i (X_1 in slot 0)
-// and ends with Q_i in slot i-1; column 1 keeps Y_i in slot i-1 (Y_nb in slot nb) and ends with P_i in slot i.
-static void run_sweep(ss_handle_t h, Ctx& ctx) {
-    const int nb = h->nb, bs = h->bs, nE = h->n_energy, batch = 2 * nE;
+// a0-a4: Algorithm 1 and its mirror (L167) for the energies [e0, e0 + nEg) of one stream group, both
+// columns in lockstep.  Chain z = 2*e + col.  Slot layout per chain (nb+1 slots of bs x bs): column 0 keeps X_i in slot i
+// (X_1 in slot 0) and ends with Q_i in slot i-1; column 1 keeps Y_i in slot i-1 (Y_nb in slot nb) and ends with P_i in
+// slot i.  sweep_step(s) is block step s of both sweeps (a0-a3), recursion_step(r) one product of a4.
+struct Group {
+    int e0 = 0, nE = 0;
+    Ctx ctx;
+};
+
+static void sweep_step(ss_handle_t h, Group& G, int s) {
+    Ctx& ctx = G.ctx;
+    const int nb = h->nb, bs = h->bs, e0 = G.e0, batch = 2 * G.nE;
     const long long B2 = (long long)bs * bs;
     const long long s_slot_e = 2LL * (nb + 1) * B2;
-    auto slot = [&](int col, int idx) { return h->slots + ((long long)col * (nb + 1) + idx) * B2; };
+    auto slot = [&](int col, int idx) { return h->slots + (long long)e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
     const int ldg = 2 * bs;
-    const BPtr aug = bp_chain(h->aug, h->aug + (long long)bs * ldg, 2LL * bs * ldg);
-    const BPtr aop = bp_chain(h->aop, h->aop + B2, 2 * B2);
+    const long long s_aug_e = 2LL * bs * ldg;
+    const BPtr aug = bp_chain(h->aug + e0 * s_aug_e, h->aug + e0 * s_aug_e + (long long)bs * ldg, s_aug_e);
+    const BPtr aop = bp_chain(h->aop + e0 * 2 * B2, h->aop + e0 * 2 * B2 + B2, 2 * B2);
+    const cplx* E = h->E_dev + e0;
+    const int blk_chain = (int)cdiv(bs, 128);
     LuWork w;
-    w.tinv = h->tinv; w.tinv_blocks = h->tinv_blocks_total; w.ipiv = h->ipiv; w.ipiv_stride = 2 * bs; w.info = h->info;
+    w.tinv = h->tinv + (long long)2 * e0 * blk_chain * 128 * 128; w.tinv_blocks = batch * blk_chain;
+    w.ipiv = h->ipiv + (long long)2 * e0 * 2 * bs; w.ipiv_stride = 2 * bs; w.info = h->info + 2 * e0;
     const int info_stride = 2 * bs + 2;
 
-    for (int s = 0; s < nb; s++) {
-        const int i_f = nb - s, i_m = s + 1;                       // 1-based block index of each chain
-        // right-hand sides: A_{i,i-1} (column 0) / A_{i,i+1} (column 1); identity at the ends (L164, reading c1)
-        FormSide r0 = (i_f > 1) ? FormSide{h->Su + (long long)(i_f - 2) * B2, h->Hu + (long long)(i_f - 2) * B2, FORM_CONJT}
-                                : FormSide{nullptr, nullptr, FORM_IDENT};
-        FormSide r1 = (i_m < nb) ? FormSide{h->Su + (long long)(i_m - 1) * B2, h->Hu + (long long)(i_m - 1) * B2, FORM_PLAIN}
-                                 : FormSide{nullptr, nullptr, FORM_IDENT};
-        launch_form(ctx, r0, r1, h->E_dev, bp_offset(aug, bs), ldg, bs, batch);
-        GemmArgs g{};
-        g.M = bs; g.N = bs; g.K = 0;
-        g.A = aop; g.lda = bs; g.B = aop; g.ldb = bs;
-        if (s > 0) {
-            // left operands: A_{i,i+1} (column 0) / A_{i,i-1} (column 1)
-            FormSide a0{h->Su + (long long)(i_f - 1) * B2, h->Hu + (long long)(i_f - 1) * B2, FORM_PLAIN};
-            FormSide a1{h->Su + (long long)(i_m - 2) * B2, h->Hu + (long long)(i_m - 2) * B2, FORM_CONJT};
-            launch_form(ctx, a0, a1, h->E_dev, aop, bs, bs, batch);
-            g.K = bs;
-            g.B = bp_chain(slot(0, i_f + 1), slot(1, i_m - 2), s_slot_e);   // X_{i+1} / Y_{i-1}
-        }
-        // a1 (+ a0 for the diagonal block, fused in the epilogue): D = E S_ii - H_ii - A_op * X_prev
-        g.C = aug; g.ldc = ldg; g.Cin = aug; g.ldcin = ldg; g.alpha = 1.0; g.beta = 0.0;
-        g.S = bp_chain(h->Sd + (long long)(i_f - 1) * B2, h->Sd + (long long)(i_m - 1) * B2, 0);
-        g.H = bp_chain(h->Hd + (long long)(i_f - 1) * B2, h->Hd + (long long)(i_m - 1) * B2, 0);
-        g.lds = bs; g.E = h->E_dev;
-        gemm_run(ctx, g, batch, GEMM_BIG, EPI_SCHUR);
-        // a2 + the L half of a3
-        lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, h->nb_lu, w, s * info_stride);
-        // U half of a3: X_i / Y_i into its slot
-        BPtr out = bp_chain(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
-        back_substitute(ctx, aug, ldg, bs, bs, out, bs, batch, w);
+    const int i_f = nb - s, i_m = s + 1;                       // 1-based block index of each chain
+    ctx.use(CLS_HI);
+    // right-hand sides: A_{i,i-1} (column 0) / A_{i,i+1} (column 1); identity at the ends (L164, reading c1)
+    FormSide r0 = (i_f > 1) ? FormSide{h->Su + (long long)(i_f - 2) * B2, h->Hu + (long long)(i_f - 2) * B2, FORM_CONJT}
+                            : FormSide{nullptr, nullptr, FORM_IDENT};
+    FormSide r1 = (i_m < nb) ? FormSide{h->Su + (long long)(i_m - 1) * B2, h->Hu + (long long)(i_m - 1) * B2, FORM_PLAIN}
+                             : FormSide{nullptr, nullptr, FORM_IDENT};
+    launch_form(ctx, r0, r1, E, bp_offset(aug, bs), ldg, bs, batch);
+    GemmArgs g{};
+    g.M = bs; g.N = bs; g.K = 0;
+    g.A = aop; g.lda = bs; g.B = aop; g.ldb = bs;
+    if (s > 0) {
+        // left operands: A_{i,i+1} (column 0) / A_{i,i-1} (column 1)
+        FormSide a0{h->Su + (long long)(i_f - 1) * B2, h->Hu + (long long)(i_f - 1) * B2, FORM_PLAIN};
+        FormSide a1{h->Su + (long long)(i_m - 2) * B2, h->Hu + (long long)(i_m - 2) * B2, FORM_CONJT};
+        launch_form(ctx, a0, a1, E, aop, bs, bs, batch);
+        g.K = bs;
+        g.B = bp_chain(slot(0, i_f + 1), slot(1, i_m - 2), s_slot_e);   // X_{i+1} / Y_{i-1}
     }
-    // a4: Q_i = -X_i Q_{i-1} (i = 2..nb), P_i = -Y_i P_{i+1} (i = nb-1..1)
-    for (int r = 1; r < nb; r++) {
-        const int i0 = r + 1, i1 = nb - r;
-        GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_chain(slot(0, i0), slot(1, i1 - 1), s_slot_e), bs,
-                              bp_chain(slot(0, i0 - 2), slot(1, i1 + 1), s_slot_e), bs, 0.0,
-                              bp_chain(slot(0, i0 - 1), slot(1, i1), s_slot_e), bs);
-        gemm_run(ctx, g, batch, GEMM_BIG, EPI_STD);
-    }
+    // a1 (+ a0 for the diagonal block, fused in the epilogue): D = E S_ii - H_ii - A_op * X_prev
+    ctx.use(CLS_LO);
+    g.C = aug; g.ldc = ldg; g.Cin = aug; g.ldcin = ldg; g.alpha = 1.0; g.beta = 0.0;
+    g.S = bp_chain(h->Sd + (long long)(i_f - 1) * B2, h->Sd + (long long)(i_m - 1) * B2, 0);
+    g.H = bp_chain(h->Hd + (long long)(i_f - 1) * B2, h->Hd + (long long)(i_m - 1) * B2, 0);
+    g.lds = bs; g.E = E;
+    gemm_run(ctx, g, batch, GEMM_BIG, EPI_SCHUR);
+    // a2 + the L half of a3
+    lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, h->nb_lu, w, s * info_stride);
+    // U half of a3: X_i / Y_i into its slot
+    BPtr out = bp_chain(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
+    back_substitute(ctx, aug, ldg, bs, bs, out, bs, batch, w);
+}
+
+// a4: Q_i = -X_i Q_{i-1} (i = 2..nb), P_i = -Y_i P_{i+1} (i = nb-1..1); r = 1..nb-1
+static void recursion_step(ss_handle_t h, Group& G, int r) {
+    const int nb = h->nb, bs = h->bs, batch = 2 * G.nE;
+    const long long B2 = (long long)bs * bs;
+    const long long s_slot_e = 2LL * (nb + 1) * B2;
+    auto slot = [&](int col, int idx) { return h->slots + (long long)G.e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
+    const int i0 = r + 1, i1 = nb - r;
+    G.ctx.use(CLS_LO);
+    GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_chain(slot(0, i0), slot(1, i1 - 1), s_slot_e), bs,
+                          bp_chain(slot(0, i0 - 2), slot(1, i1 + 1), s_slot_e), bs, 0.0,
+                          bp_chain(slot(0, i0 - 1), slot(1, i1), s_slot_e), bs);
+    gemm_run(G.ctx, g, batch, GEMM_BIG, EPI_STD);
 }
 
 // a5-a7: corner system, solution, transmission (north_star for T).
-static void run_post(ss_handle_t h, Ctx& ctx, const cplx* SigL, const cplx* SigR, const cplx* inj1, const cplx* inj2,
+static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR, const cplx* inj1, const cplx* inj2,
                      int m, cplx* X) {
-    const int nb = h->nb, bs = h->bs, nE = h->n_energy;
+    Ctx& ctx = G.ctx;
+    const int nb = h->nb, bs = h->bs, nE = G.nE, e0 = G.e0;
     const long long B2 = (long long)bs * bs;
     const long long s_slot_e = 2LL * (nb + 1) * B2;
-    auto slot = [&](int col, int idx) { return h->slots + ((long long)col * (nb + 1) + idx) * B2; };
+    auto slot = [&](int col, int idx) { return h->slots + (long long)e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
     const int zc = h->want_T ? bs : 0;                // columns of e_2 (for (R^-1)_{12}, (R^-1)_{22})
     const int W = 2 * bs + m + zc;
     const int nr = m + zc;
     const long long s_r = 2LL * bs * W, s_w = 2LL * bs * nr;
+    cplx* raug = h->raug + e0 * s_r;
+    cplx* wz = h->wz + e0 * s_w;
+    SigL += e0 * B2; SigR += e0 * B2;
+    if (inj1) inj1 += (long long)e0 * bs * m;
+    if (inj2) inj2 += (long long)e0 * bs * m;
+    if (X) X += (long long)e0 * nb * bs * m;
+    cplx *g1n = h->g1n + e0 * B2, *w1 = h->w1 + e0 * B2, *w2 = h->w2 + e0 * B2;
+    cplx *gam_l = h->gam_l + e0 * B2, *gam_r = h->gam_r + e0 * B2;
+    ctx.use(CLS_HI);
     {
         dim3 grid((unsigned)min((long long)8, cdiv(W, 256)), (unsigned)(2 * bs), (unsigned)nE);
-        corner_init_kernel<<<grid, 256, 0, ctx.st>>>(h->raug, s_r, W, bs, m, inj1, inj2);
+        corner_init_kernel<<<grid, 256, 0, ctx.st>>>(raug, s_r, W, bs, m, inj1, inj2);
         ctx.note(cudaGetLastError());
     }
+    ctx.use(CLS_LO);
     // R = 1 - C [Q P]:  R11 -= Sigma_L Q_1, R12 -= Sigma_L P_1, R21 -= Sigma_R Q_nb, R22 -= Sigma_R P_nb
     const cplx* sig[2] = {SigL, SigR};
     for (int br = 0; br < 2; br++)
         for (int bc = 0; bc < 2; bc++) {
             const cplx* Bsrc = (bc == 0) ? slot(0, br == 0 ? 0 : nb - 1) : slot(1, br == 0 ? 1 : nb);
             GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(Bsrc, s_slot_e), bs, 1.0,
-                                  bp_strided(h->raug + (long long)br * bs * W + (long long)bc * bs, s_r), W);
+                                  bp_strided(raug + (long long)br * bs * W + (long long)bc * bs, s_r), W);
             gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         }
+    const int blk_corner = (int)cdiv(2 * bs, 128);
     LuWork w;
-    w.tinv = h->tinv; w.tinv_blocks = h->tinv_blocks_total;
-    w.ipiv = h->ipiv + (long long)2 * nE * 2 * bs; w.ipiv_stride = 2 * bs; w.info = h->info + 2 * nE;
-    lu_factor(ctx, bp_strided(h->raug, s_r), W, 2 * bs, W, nE, h->nb_lu, w, 0);
-    back_substitute(ctx, bp_strided(h->raug, s_r), W, 2 * bs, nr, bp_strided(h->wz, s_w), nr, nE, w);
+    w.tinv = h->tinv + (long long)e0 * blk_corner * 128 * 128; w.tinv_blocks = nE * blk_corner;
+    w.ipiv = h->ipiv + (long long)2 * h->n_energy * 2 * bs + (long long)e0 * 2 * bs; w.ipiv_stride = 2 * bs;
+    w.info = h->info + 2 * h->n_energy + e0;
+    lu_factor(ctx, bp_strided(raug, s_r), W, 2 * bs, W, nE, h->nb_lu, w, 0);
+    back_substitute(ctx, bp_strided(raug, s_r), W, 2 * bs, nr, bp_strided(wz, s_w), nr, nE, w);
     // a6: X_i = Q_i w_top + P_i w_bot, batch z = e*nb + (i-1)
     if (m > 0) {
         GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(0, 0), nb, B2, s_slot_e), bs,
-                              bp_two_level(h->wz, nb, 0, s_w), nr, 0.0,
+                              bp_two_level(wz, nb, 0, s_w), nr, 0.0,
                               bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
         gemm_run(ctx, g, nE * nb, GEMM_BIG, EPI_STD);
         GemmArgs g2 = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(1, 1), nb, B2, s_slot_e), bs,
-                               bp_two_level(h->wz + (long long)bs * nr, nb, 0, s_w), nr, 1.0,
+                               bp_two_level(wz + (long long)bs * nr, nb, 0, s_w), nr, 1.0,
                                bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
         gemm_run(ctx, g2, nE * nb, GEMM_BIG, EPI_STD);
     }
     // a7: G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22;  T = Re Tr(Gamma_L G Gamma_R G^H)
     if (h->want_T) {
-        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(0, 0), s_slot_e), bs, bp_strided(h->wz + m, s_w), nr, 0.0,
-                              bp_strided(h->g1n, B2), bs);
+        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(0, 0), s_slot_e), bs, bp_strided(wz + m, s_w), nr, 0.0,
+                              bp_strided(g1n, B2), bs);
         gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(1, 1), s_slot_e), bs,
-                               bp_strided(h->wz + (long long)bs * nr + m, s_w), nr, 1.0, bp_strided(h->g1n, B2), bs);
+                               bp_strided(wz + (long long)bs * nr + m, s_w), nr, 1.0, bp_strided(g1n, B2), bs);
         gemm_run(ctx, g2, nE, GEMM_BIG, EPI_STD);
         dim3 gg((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)nE);
-        gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigL, h->gam_l, bs); ctx.note(cudaGetLastError());
-        gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigR, h->gam_r, bs); ctx.note(cudaGetLastError());
-        GemmArgs g3 = gemm_std(bs, bs, bs, 1.0, bp_strided(h->gam_l, B2), bs, bp_strided(h->g1n, B2), bs, 0.0,
-                               bp_strided(h->w1, B2), bs);
+        gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigL, gam_l, bs); ctx.note(cudaGetLastError());
+        gamma_kernel<<<gg, 256, 0, ctx.st>>>(SigR, gam_r, bs); ctx.note(cudaGetLastError());
+        GemmArgs g3 = gemm_std(bs, bs, bs, 1.0, bp_strided(gam_l, B2), bs, bp_strided(g1n, B2), bs, 0.0,
+                               bp_strided(w1, B2), bs);
         gemm_run(ctx, g3, nE, GEMM_BIG, EPI_STD);
-        GemmArgs g4 = gemm_std(bs, bs, bs, 1.0, bp_strided(h->w1, B2), bs, bp_strided(h->gam_r, B2), bs, 0.0,
-                               bp_strided(h->w2, B2), bs);
+        GemmArgs g4 = gemm_std(bs, bs, bs, 1.0, bp_strided(w1, B2), bs, bp_strided(gam_r, B2), bs, 0.0,
+                               bp_strided(w2, B2), bs);
         gemm_run(ctx, g4, nE, GEMM_BIG, EPI_STD);
         int parts = (int)min((long long)TRACE_PARTS, cdiv(B2, 256));
-        trace_partial_kernel<<<dim3((unsigned)parts, (unsigned)nE), 256, 0, ctx.st>>>(h->w2, h->g1n, B2, B2, h->tpart);
+        trace_partial_kernel<<<dim3((unsigned)parts, (unsigned)nE), 256, 0, ctx.st>>>(w2, g1n, B2, B2,
+                                                                                       h->tpart + (long long)e0 * TRACE_PARTS);
         ctx.note(cudaGetLastError());
-        trace_final_kernel<<<nE, 32, 0, ctx.st>>>(h->tpart, parts, h->T_dev);
+        trace_final_kernel<<<nE, 32, 0, ctx.st>>>(h->tpart + (long long)e0 * TRACE_PARTS, parts, h->T_dev + e0);
         ctx.note(cudaGetLastError());
     }
+}
+
+static bool ensure_groups(ss_handle_t h, int n) {
+    if (!h->ev_fork && cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess) return false;
+    int lo_prio = 0, hi_prio = 0;
+    cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio);     // numerically lower = higher priority
+    while ((int)h->groups.size() < n) {
+        ss_handle_s::GroupRes g;
+        bool ok = cudaStreamCreateWithPriority(&g.hi, cudaStreamNonBlocking, hi_prio) == cudaSuccess &&
+                  cudaStreamCreateWithPriority(&g.lo, cudaStreamNonBlocking, lo_prio) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&g.ev_sw, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&g.ev_mark, cudaEventDisableTiming) == cudaSuccess;
+        h->groups.push_back(g);                               // pushed even on failure so that ss_destroy frees the parts
+        if (!ok) return false;
+    }
+    return true;
 }
 
 extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L, const ss_cplx* Sigma_R,
@@ -358,23 +425,71 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     if (h->solved) cudaEventSynchronize(h->ev[2]);        // E_pinned of the previous call is free again
     memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
-    Ctx ctx; ctx.st = stream; ctx.variant = h->gemm_variant;
     h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
-    ctx.prof = h->profile_gemm ? &h->prof : nullptr;
     if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
         cudaMemsetAsync(h->info, 0, sizeof(int) * 3 * (size_t)h->n_energy, stream) != cudaSuccess) {
         cudaGetLastError(); return SS_ERR_CUDA;
     }
+    // Energy points are independent: split them over stream groups.  Group g owns the energies
+    // [e0, e0 + nE); the host interleaves the groups' launches step by step so that every group's streams stay fed.
+    const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
+    if (nG > 1 && !ensure_groups(h, nG)) { cudaGetLastError(); return SS_ERR_CUDA; }
+    std::vector<Group> G((size_t)nG);
+    for (int g = 0; g < nG; g++) {
+        G[g].e0 = (int)((long long)h->n_energy * g / nG);
+        G[g].nE = (int)((long long)h->n_energy * (g + 1) / nG) - G[g].e0;
+        Ctx& c = G[g].ctx;
+        c.variant = h->gemm_variant;
+        c.group = g;
+        c.prof = h->profile_gemm ? &h->prof : nullptr;
+        c.st = stream;
+    }
     cudaEventRecord(h->ev[0], stream);
-    run_sweep(h, ctx);
+    if (nG > 1) {
+        cudaEventRecord(h->ev_fork, stream);
+        for (int g = 0; g < nG; g++) {
+            Ctx& c = G[g].ctx;
+            c.s_hi = h->groups[g].hi; c.s_lo = h->groups[g].lo; c.ev_sw = h->groups[g].ev_sw;
+            c.st = c.s_lo; c.cls = CLS_LO;
+            cudaStreamWaitEvent(c.s_lo, h->ev_fork, 0);
+        }
+    }
+    for (auto& r : h->trace) { cudaEventDestroy(r.t0); cudaEventDestroy(r.t1); }
+    h->trace.clear();
+    if (h->want_trace)
+        for (int g = 0; g < nG; g++) { G[g].ctx.trace = &h->trace; G[g].ctx.trace_open(); }
+    const int nb = h->nb;
+    for (int s = 0; s < nb; s++)
+        for (int g = 0; g < nG; g++) sweep_step(h, G[g], s);
+    for (int r = 1; r < nb; r++)
+        for (int g = 0; g < nG; g++) recursion_step(h, G[g], r);
+    if (nG > 1)
+        for (int g = 0; g < nG; g++) {                     // marks the end of the sweep phase; the groups do not wait
+            G[g].ctx.use(CLS_LO);
+            cudaEventRecord(h->groups[g].ev_mark, G[g].ctx.st);
+            cudaStreamWaitEvent(stream, h->groups[g].ev_mark, 0);
+        }
     cudaEventRecord(h->ev[1], stream);
-    run_post(h, ctx, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first, (const cplx*)Inj_last, nrhs, (cplx*)X);
+    for (int g = 0; g < nG; g++)
+        run_post(h, G[g], (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first, (const cplx*)Inj_last, nrhs, (cplx*)X);
+    if (nG > 1)
+        for (int g = 0; g < nG; g++) {
+            G[g].ctx.use(CLS_LO);
+            cudaEventRecord(h->groups[g].ev_mark, G[g].ctx.st);
+            cudaStreamWaitEvent(stream, h->groups[g].ev_mark, 0);
+        }
+    for (int g = 0; g < nG; g++) G[g].ctx.trace_close();
     cudaEventRecord(h->ev[2], stream);
-    h->launches = ctx.launches;
+    h->launches = 0;
+    cudaError_t err = cudaSuccess;
+    for (int g = 0; g < nG; g++) {
+        h->launches += G[g].ctx.launches;
+        if (err == cudaSuccess) err = G[g].ctx.err;
+    }
     h->last_stream = stream;
     h->last_nrhs = nrhs;
     h->solved = true;
-    if (ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }
 
@@ -484,6 +599,31 @@ extern "C" ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops,
 }
 
 extern "C" long long ss_launch_count(ss_handle_t h) { return h ? h->launches : 0; }
+
+extern "C" ss_status_t ss_trace_write(ss_handle_t h, const char* path) {
+    if (!h || !path) return SS_ERR_INVALID_ARG;
+    if (!h->solved) return SS_ERR_NOT_READY;
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    FILE* f = fopen(path, "w");
+    if (!f) return SS_ERR_INVALID_ARG;
+    fprintf(f, "group,class,start_ms,end_ms\n");
+    for (auto& r : h->trace) {
+        float a = 0.f, b = 0.f;
+        if (cudaEventElapsedTime(&a, h->ev[0], r.t0) != cudaSuccess || cudaEventElapsedTime(&b, h->ev[0], r.t1) != cudaSuccess) {
+            cudaGetLastError(); continue;
+        }
+        fprintf(f, "%d,%s,%.4f,%.4f\n", r.group, r.cls == CLS_HI ? "hi" : "lo", a, b);
+    }
+    if (h->profile_gemm)                                   // every GEMM launch of the solve: class "gemm", group -1
+        for (size_t i = 0; i + 1 < h->prof.used; i += 2) {
+            float a = 0.f, b = 0.f;
+            if (cudaEventElapsedTime(&a, h->ev[0], h->prof.ev[i]) != cudaSuccess ||
+                cudaEventElapsedTime(&b, h->ev[0], h->prof.ev[i + 1]) != cudaSuccess) { cudaGetLastError(); continue; }
+            fprintf(f, "-1,gemm,%.4f,%.4f\n", a, b);
+        }
+    fclose(f);
+    return SS_OK;
+}
 
 extern "C" ss_status_t ss_solve_host(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* SigL, const ss_cplx* SigR,
                                      const ss_cplx* Inj1, const ss_cplx* Inj2, int nrhs, ss_cplx* X_host, double* T_host) {

@@ -157,6 +157,152 @@ lu_leaf_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restri
     }
 }
 
+// ---- leaf panel, version 2: 256 rows per CTA (cluster of up to 16 CTAs = 4096 rows), one __syncthreads and one
+// cluster barrier per column.  Warp arg-max by three redux.sync on the bit pattern of |re|+|im| (non-negative doubles
+// order like unsigned integers) and the row position; the warp winner deposits (value, position, row) in shared
+// memory, warp 0 picks the CTA winner and all its lanes push that candidate to every CTA of the cluster through
+// distributed shared memory; after the cluster barrier every thread scans the <= 16 candidates and updates its row.
+constexpr int LEAF2_TPB = 256;
+constexpr int LEAF2_MAXC = 16;
+
+__device__ __forceinline__ cplx crecip_fast(cplx a) {
+    double n = fma(a.re, a.re, a.im * a.im);
+    if (n > 1e-280 && n < 1e280) {
+        double r = 1.0 / n;
+        return make_c(a.re * r, -a.im * r);
+    }
+    return crecip(a);
+}
+
+// (value, position) arg-max over the lanes of a warp; ties -> lowest position.  value >= 0 or -1 (no row).
+// Returns true on the single winning lane (false on all lanes if no lane has a row).
+__device__ __forceinline__ bool warp_argmax(double v, int pos, double& wv, int& wp) {
+    unsigned long long key = (v >= 0.0) ? ((unsigned long long)__double_as_longlong(v) + 1ull) : 0ull;
+    unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
+    unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+    unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
+    bool cand = (hi == mh) && (lo == ml);
+    unsigned mp = __reduce_min_sync(0xffffffffu, cand ? (unsigned)pos : 0xffffffffu);
+    unsigned long long mk = ((unsigned long long)mh << 32) | ml;
+    wv = mk ? __longlong_as_double((long long)(mk - 1ull)) : -1.0;
+    wp = (int)mp;
+    return cand && (unsigned)pos == mp && mk != 0ull;
+}
+
+#ifdef LEAF_PROFILE
+__device__ long long g_leaf_prof[8];
+#define LEAF_TICK(i) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { long long t_ = clock64(); g_leaf_prof[i] += t_ - tprev_; tprev_ = t_; } } while (0)
+#else
+#define LEAF_TICK(i) do { } while (0)
+#endif
+
+__global__ void __launch_bounds__(LEAF2_TPB, 1)
+lu_leaf2_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restrict__ ipiv, int ipiv_stride,
+                int* __restrict__ info, int info_base) {
+    cg::cluster_group cluster = cg::this_cluster();
+    const int csize = (int)cluster.num_blocks();
+    const int crank = (int)cluster.block_rank();
+    const int z = blockIdx.y;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = LEAF2_TPB / 32;
+    constexpr int CH = (int)(sizeof(LeafCand) / 16);            // 16-byte chunks per candidate
+
+    __shared__ __align__(16) LeafCand slots[2][LEAF2_MAXC];
+    __shared__ __align__(16) LeafCand wcand[NW];
+
+    cplx* __restrict__ A = bptr(Ab, z) + (long long)row0 * ld + col0;
+    const int r = crank * LEAF2_TPB + tid;       // my row inside the panel
+    const bool valid = r < m;
+
+    cplx a[LEAF_JB];
+#pragma unroll
+    for (int k = 0; k < LEAF_JB; k++) a[k] = make_c(0.0, 0.0);
+    if (valid) {
+        const cplx* src = A + (long long)r * ld;
+#pragma unroll
+        for (int k = 0; k < LEAF_JB; k++)
+            if (k < jb) a[k] = src[k];
+    }
+    int cur_pos = r;
+    bool done = !valid;
+    int final_pos = r;
+
+#pragma unroll
+    for (int j = 0; j < LEAF_JB; j++) {
+        if (j < jb) {
+            const int buf = j & 1;
+            double wv; int wp;
+#ifdef LEAF_PROFILE
+            long long tprev_ = clock64();
+#endif
+            const double myv = done ? -1.0 : (fabs(a[j].re) + fabs(a[j].im));
+            if (warp_argmax(myv, cur_pos, wv, wp)) {
+                LeafCand* c = &wcand[warp];
+                c->val = myv; c->pos = cur_pos;
+#pragma unroll
+                for (int k = 0; k < LEAF_JB; k++) c->row[k] = a[k];
+            }
+            if (lane == 0 && wv < 0.0) { wcand[warp].val = -1.0; wcand[warp].pos = 0x7fffffff; }
+            LEAF_TICK(0);
+            __syncthreads();
+            LEAF_TICK(1);
+            if (warp == 0) {
+                double v2 = lane < NW ? wcand[lane].val : -1.0;
+                int p2 = lane < NW ? wcand[lane].pos : 0x7fffffff;
+                double cv; int cp;
+                bool win = warp_argmax(v2, p2, cv, cp);
+                unsigned bal = __ballot_sync(0xffffffffu, win);
+                const int w = bal ? (__ffs(bal) - 1) : 0;        // no rows in this CTA: wcand[0] already says (-1, max)
+                const uint4* src = reinterpret_cast<const uint4*>(&wcand[w]);
+                for (int idx = lane; idx < CH * csize; idx += 32) {
+                    int c = idx / CH, ch = idx - c * CH;
+                    uint4* dst = reinterpret_cast<uint4*>(cluster.map_shared_rank(&slots[buf][crank], c));
+                    dst[ch] = src[ch];
+                }
+            }
+            LEAF_TICK(2);
+            cluster.sync();
+            LEAF_TICK(3);
+            // ---- winner among the csize candidates
+            int win = 0; double gv = slots[buf][0].val; int gp = slots[buf][0].pos;
+            for (int c = 1; c < csize; c++) {
+                double cv = slots[buf][c].val; int cp = slots[buf][c].pos;
+                if (cv > gv || (cv == gv && cp < gp)) { gv = cv; gp = cp; win = c; }
+            }
+            if (gv < 0.0) { gp = j; }                     // no rows left (m < jb): nothing to do
+            const bool singular = !(gv > 0.0);
+            if (crank == 0 && tid == 0) {
+                ipiv[(long long)z * ipiv_stride + row0 + j] = row0 + gp;
+                if (singular && gv >= 0.0) atomicCAS(&info[z], 0, info_base + row0 + j + 1);
+            }
+            LEAF_TICK(4);
+            if (!done) {
+                if (cur_pos == gp && gv >= 0.0) {
+                    done = true; final_pos = j;           // I am the pivot row: becomes row j of U
+                } else {
+                    if (cur_pos == j) cur_pos = gp;       // LAPACK swap bookkeeping
+                    if (!singular) {
+                        const cplx* prow = slots[buf][win].row;
+                        cplx rinv = crecip_fast(prow[j]);
+                        cplx l = cmul(a[j], rinv);
+                        a[j] = l;
+#pragma unroll
+                        for (int k = j + 1; k < LEAF_JB; k++) a[k] = cfnma(a[k], l, prow[k]);
+                    }
+                }
+            }
+            LEAF_TICK(5);
+        }
+    }
+    if (valid) {
+        if (!done) final_pos = cur_pos;
+        cplx* dst = A + (long long)final_pos * ld;
+#pragma unroll
+        for (int k = 0; k < LEAF_JB; k++)
+            if (k < jb) dst[k] = a[k];
+    }
+}
+
 // Apply the row interchanges ipiv[row0 .. row0+jb) to columns [0, skip_lo) U [skip_hi, ncols) of each matrix.
 // One thread per column: consecutive threads touch consecutive elements of a row (coalesced in row-major).
 __global__ void __launch_bounds__(256)
@@ -310,13 +456,49 @@ struct GemmProfile {                 // optional per-launch CUDA-event timing of
     long long launches = 0;
 };
 
+// Launch context of one group of chains.  With stream groups (splitsolve.cu) every group owns two streams: a
+// HIGH-priority one for the short latency-bound kernels of the panel factorisation (leaf, row swaps, small
+// triangular solves and inverses, rank-16 updates) and a LOW-priority one for the large GEMMs, so that one group's
+// panel runs in the shadow of another group's GEMMs (the block scheduler places pending high-priority CTAs first).
+// use() moves the launch point between the two, ordering them with an event.  Without groups both are the caller's
+// stream and use() does nothing.
+enum { CLS_LO = 0, CLS_HI = 1 };
+struct TraceRec { int group, cls; cudaEvent_t t0, t1; };      // one phase of one group (option "trace")
 struct Ctx {
+    std::vector<TraceRec>* trace = nullptr;
+    int group = 0;
+    void trace_open() {
+        if (!trace) return;
+        TraceRec r{group, cls, nullptr, nullptr};
+        cudaEventCreate(&r.t0); cudaEventCreate(&r.t1);
+        cudaEventRecord(r.t0, st);
+        trace->push_back(r);
+    }
+    void trace_close() {
+        if (!trace) return;
+        for (size_t i = trace->size(); i-- > 0;)
+            if ((*trace)[i].group == group) { cudaEventRecord((*trace)[i].t1, st); break; }
+    }
     cudaStream_t st = nullptr;
+    cudaStream_t s_hi = nullptr, s_lo = nullptr;
+    cudaEvent_t ev_sw = nullptr;
+    int cls = CLS_LO;
     long long launches = 0;
     cudaError_t err = cudaSuccess;
     GemmProfile* prof = nullptr;
     int variant = GV_4M;            // GEMM arithmetic / tile variant (zgemm3m.cuh)
     void note(cudaError_t e) { if (err == cudaSuccess && e != cudaSuccess) err = e; launches++; }
+    void use(int c) {
+        if (c == cls) return;
+        if (!ev_sw) { trace_close(); cls = c; trace_open(); return; }      // single stream: phases only marked
+        cudaStream_t to = (c == CLS_HI) ? s_hi : s_lo;
+        trace_close();
+        cudaError_t e = cudaEventRecord(ev_sw, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(to, ev_sw, 0);
+        if (err == cudaSuccess && e != cudaSuccess) err = e;
+        st = to; cls = c;
+        trace_open();
+    }
 };
 
 static void gemm_run(Ctx& ctx, const GemmArgs& g, int batch, int cfg, int epi) {
@@ -354,19 +536,24 @@ static inline GemmArgs gemm_std(int M, int N, int K, double alpha, BPtr A, int l
     return g;
 }
 
+static int g_leaf_version = 2;       // 1 = lu_leaf_kernel (512 rows / CTA), 2 = lu_leaf2_kernel (256 rows / CTA)
+
 static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, int jb, const LuWork& w, int info_base,
                         int batch) {
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(lu_leaf_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        cudaFuncSetAttribute(lu_leaf2_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         configured = true;
     }
-    int need = (m + LEAF_TPB - 1) / LEAF_TPB;
+    const bool v2 = (g_leaf_version == 2) && m <= 4 * LEAF2_TPB;     // measured: v2 wins up to 4 CTAs per cluster
+    const int tpb = v2 ? LEAF2_TPB : LEAF_TPB;
+    int need = (m + tpb - 1) / tpb;
     int csize = 1;
     while (csize < need) csize <<= 1;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)csize, (unsigned)batch, 1);
-    cfg.blockDim = dim3(LEAF_TPB, 1, 1);
+    cfg.blockDim = dim3((unsigned)tpb, 1, 1);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = ctx.st;
     cudaLaunchAttribute attr[1];
@@ -376,7 +563,10 @@ static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, in
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
+    if (v2)
+        ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf2_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
+    else
+        ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
 }
 
 // LU with partial pivoting of the leading n x n part of the n x ncols matrices; interchanges and L-solve applied
@@ -385,6 +575,7 @@ static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, in
                       int info_base) {
     for (int j0 = 0; j0 < n; j0 += nb_lu) {
         const int nbw = min(nb_lu, n - j0);
+        ctx.use(CLS_HI);
         for (int c = j0; c < j0 + nbw; c += LEAF_JB) {
             const int jb = min(LEAF_JB, j0 + nbw - c);
             const int m = n - c;
@@ -417,6 +608,7 @@ static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, in
             t.out = w.tinv; t.nblocks = 1; t.upper = 0; t.unit = 1;
             trtri_kernel<<<dim3(8, 1, (unsigned)batch), 256, 0, ctx.st>>>(t);
             ctx.note(cudaGetLastError());
+            ctx.use(CLS_LO);
             BPtr A12 = bp_offset(Ab, (long long)j0 * ld + j0 + nbw);
             GemmArgs g = gemm_std(nbw, rest, nbw, 1.0, bp_strided(w.tinv, 128 * 128), 128, A12, ld, 0.0, A12, ld);
             gemm_run(ctx, g, batch, GEMM_TALL, EPI_STD);
@@ -438,8 +630,10 @@ static void back_substitute(Ctx& ctx, BPtr Ab, int ld, int n, int nrhs, BPtr X, 
     TrtriArgs t{};
     t.T = Ab; t.ld = ld; t.t_step = (long long)P * ld + P; t.n_total = n; t.out = w.tinv; t.nblocks = nblk;
     t.upper = 1; t.unit = 0;
+    ctx.use(CLS_HI);
     trtri_kernel<<<dim3(8, (unsigned)nblk, (unsigned)batch), 256, 0, ctx.st>>>(t);
     ctx.note(cudaGetLastError());
+    ctx.use(CLS_LO);
     for (int jb = nblk - 1; jb >= 0; jb--) {
         const int j = jb * P, nbj = min(P, n - j), kk = n - j - nbj;
         BPtr Yj = bp_offset(Ab, (long long)j * ld + n);
