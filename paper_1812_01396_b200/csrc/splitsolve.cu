@@ -54,6 +54,11 @@ static const int TRACE_PARTS = 592;   // 4 x 148 CTAs per energy for the trace r
 
 static inline long long cdiv(long long a, long long b) { return (a + b - 1) / b; }
 
+// Leading dimension of a handle-owned row-major work matrix with n columns.  A byte stride that is a multiple of 2 KB
+// maps the rows a panel kernel walks down (one thread per row) onto the same cache sets: measured, the 16-column
+// leaf panel ran 1.5x slower at ld = 4096 than at ld = 4112.  So such strides get 16 elements (256 B) of padding.
+static inline int pad_ld(long long n) { return (int)((n >= 128 && n % 128 == 0) ? n + 16 : n); }
+
 static void free_dev(void* p) { if (p) cudaFree(p); }
 
 static void free_workspace(ss_handle_t h) {
@@ -76,12 +81,13 @@ static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
     WsSizes w;
     const size_t B2 = (size_t)bs * bs, C = sizeof(cplx);
     w.slots = (size_t)nE * 2 * (nb + 1) * B2 * C;
-    w.aug = (size_t)nE * 2 * bs * 2 * bs * C;
+    w.aug = (size_t)nE * 2 * bs * pad_ld(2 * bs) * C;
     w.aop = (size_t)nE * 2 * B2 * C;
     int blk_sweep = 2 * nE * (int)cdiv(bs, 128), blk_corner = nE * (int)cdiv(2 * bs, 128);
     w.tinv_blocks = blk_sweep > blk_corner ? blk_sweep : blk_corner;
     w.tinv = (size_t)w.tinv_blocks * 128 * 128 * C;
-    const size_t W = (size_t)3 * bs + nrhs;
+    size_t W = (size_t)pad_ld(3LL * bs + nrhs), W2 = (size_t)pad_ld(2LL * bs + nrhs);   // with / without the e_2 columns
+    if (W2 > W) W = W2;
     w.raug = (size_t)nE * 2 * bs * W * C;
     w.wz = (size_t)nE * 2 * bs * ((size_t)nrhs + bs) * C;
     w.sq = (size_t)nE * B2 * C;
@@ -260,7 +266,7 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
     const long long B2 = (long long)bs * bs;
     const long long s_slot_e = 2LL * (nb + 1) * B2;
     auto slot = [&](int col, int idx) { return h->slots + (long long)e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
-    const int ldg = 2 * bs;
+    const int ldg = pad_ld(2 * bs);
     const long long s_aug_e = 2LL * bs * ldg;
     const BPtr aug = bp_chain(h->aug + e0 * s_aug_e, h->aug + e0 * s_aug_e + (long long)bs * ldg, s_aug_e);
     const BPtr aop = bp_chain(h->aop + e0 * 2 * B2, h->aop + e0 * 2 * B2 + B2, 2 * B2);
@@ -329,7 +335,8 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     const int zc = h->want_T ? bs : 0;                // columns of e_2 (for (R^-1)_{12}, (R^-1)_{22})
     const int W = 2 * bs + m + zc;
     const int nr = m + zc;
-    const long long s_r = 2LL * bs * W, s_w = 2LL * bs * nr;
+    const int ldW = pad_ld(W);
+    const long long s_r = 2LL * bs * ldW, s_w = 2LL * bs * nr;
     cplx* raug = h->raug + e0 * s_r;
     cplx* wz = h->wz + e0 * s_w;
     SigL += e0 * B2; SigR += e0 * B2;
@@ -341,7 +348,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     ctx.use(CLS_HI);
     {
         dim3 grid((unsigned)min((long long)8, cdiv(W, 256)), (unsigned)(2 * bs), (unsigned)nE);
-        corner_init_kernel<<<grid, 256, 0, ctx.st>>>(raug, s_r, W, bs, m, inj1, inj2);
+        corner_init_kernel<<<grid, 256, 0, ctx.st>>>(raug, s_r, W, ldW, bs, m, inj1, inj2);
         ctx.note(cudaGetLastError());
     }
     ctx.use(CLS_LO);
@@ -351,7 +358,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
         for (int bc = 0; bc < 2; bc++) {
             const cplx* Bsrc = (bc == 0) ? slot(0, br == 0 ? 0 : nb - 1) : slot(1, br == 0 ? 1 : nb);
             GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(Bsrc, s_slot_e), bs, 1.0,
-                                  bp_strided(raug + (long long)br * bs * W + (long long)bc * bs, s_r), W);
+                                  bp_strided(raug + (long long)br * bs * ldW + (long long)bc * bs, s_r), ldW);
             gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         }
     const int blk_corner = (int)cdiv(2 * bs, 128);
@@ -359,8 +366,8 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     w.tinv = h->tinv + (long long)e0 * blk_corner * 128 * 128; w.tinv_blocks = nE * blk_corner;
     w.ipiv = h->ipiv + (long long)2 * h->n_energy * 2 * bs + (long long)e0 * 2 * bs; w.ipiv_stride = 2 * bs;
     w.info = h->info + 2 * h->n_energy + e0;
-    lu_factor(ctx, bp_strided(raug, s_r), W, 2 * bs, W, nE, h->nb_lu, w, 0);
-    back_substitute(ctx, bp_strided(raug, s_r), W, 2 * bs, nr, bp_strided(wz, s_w), nr, nE, w);
+    lu_factor(ctx, bp_strided(raug, s_r), ldW, 2 * bs, W, nE, h->nb_lu, w, 0);
+    back_substitute(ctx, bp_strided(raug, s_r), ldW, 2 * bs, nr, bp_strided(wz, s_w), nr, nE, w);
     // a6: X_i = Q_i w_top + P_i w_bot, batch z = e*nb + (i-1)
     if (m > 0) {
         GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(0, 0), nb, B2, s_slot_e), bs,

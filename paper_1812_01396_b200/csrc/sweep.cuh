@@ -67,13 +67,13 @@ form_kernel(FormSide s0, FormSide s1, const cplx* __restrict__ E, BPtr dst, int 
     }
 }
 
-// Raug[e] : 2bs x W row-major, W = 2bs + m + bs:  [ 1_{2bs} | Inj_first ; Inj_last | 0 ; 1_bs ]
+// Raug[e] : 2bs x W row-major (leading dimension ld >= W), W = 2bs + m + bs:  [ 1_{2bs} | Inj_first ; Inj_last | 0 ; 1_bs ]
 __global__ void __launch_bounds__(256)
-corner_init_kernel(cplx* __restrict__ Raug, long long stride, int W, int bs, int m, const cplx* __restrict__ inj_first,
+corner_init_kernel(cplx* __restrict__ Raug, long long stride, int W, int ld, int bs, int m, const cplx* __restrict__ inj_first,
                    const cplx* __restrict__ inj_last) {
     const int e = blockIdx.z;
     const int r = blockIdx.y;
-    cplx* __restrict__ row = Raug + (long long)e * stride + (long long)r * W;
+    cplx* __restrict__ row = Raug + (long long)e * stride + (long long)r * ld;
     for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < W; c += gridDim.x * blockDim.x) {
         cplx v = make_c(0.0, 0.0);
         if (c < 2 * bs) {

@@ -241,11 +241,13 @@ using C3_64x32s3 = Gemm3Cfg<64, 32, 2, 2, 8, 3, 3>;      // same, 3-stage ring
 using C3_64x64 = Gemm3Cfg<64, 64, 2, 4, 16, 3, 1>;       // 8 warps of 32x16, 1 CTA/SM
 using C3_64x96 = Gemm3Cfg<64, 96, 2, 4, 16, 3, 1>;       // 8 warps of 32x24
 using C3_128x48 = Gemm3Cfg<128, 48, 4, 2, 16, 3, 1>;     // 8 warps of 32x24
+using C3_64x48 = Gemm3Cfg<64, 48, 2, 2, 8, 4, 2>;        // 4 warps of 32x24, 2 CTAs/SM
+using C3_96x32 = Gemm3Cfg<96, 32, 2, 2, 8, 4, 2>;        // 4 warps of 48x16, 2 CTAs/SM
 using C3_Tall = Gemm3Cfg<128, 32, 4, 2, 16, 3, 1>;       // one CTA owns all (<=128) rows of its columns: in-place L^-1 * A12
 
 // GEMM variants: 0 = 4M (zgemm.cuh), 1.. = 3M tile shapes.  GEMM_TALL always maps to the one-CTA-per-column
 // configuration of the same arithmetic.
-enum { GV_4M = 0, GV_3M_64x32s4 = 1, GV_3M_64x32s3 = 2, GV_3M_64x64 = 3, GV_3M_64x96 = 4, GV_3M_128x48 = 5, GV_COUNT = 6 };
+enum { GV_4M = 0, GV_3M_64x32s4 = 1, GV_3M_64x32s3 = 2, GV_3M_64x64 = 3, GV_3M_64x96 = 4, GV_3M_128x48 = 5, GV_3M_64x48 = 6, GV_3M_96x32 = 7, GV_3M_64x32s4_FIXED = 8, GV_COUNT = 9 };
 
 template <class Cfg>
 static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_t st) {
@@ -256,11 +258,16 @@ static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_
 static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st, int variant) {
     if (variant == GV_4M) return gemm4m_launch(a, batch, cfg, epi, st);
     if (cfg == GEMM_TALL) return gemm3m_launch_t<C3_Tall, EPI_STD>(a, batch, st);
+    // default (GV_3M_64x32s4): the 64x32 tile, except for long-K products of large matrices, where the 32x24 warp tile
+    // (7 instead of 6 fragment sums per 36 instead of 24 DMMA) is 2 % faster (profiles/r01_gemm_variants.md)
+    if (variant == GV_3M_64x32s4 && a.K >= 1024 && a.M >= 512 && a.N >= 512) variant = GV_3M_64x48;
     switch (variant) {
         case GV_3M_64x32s3: return gemm3m_epi<C3_64x32s3>(a, batch, epi, st);
         case GV_3M_64x64: return gemm3m_epi<C3_64x64>(a, batch, epi, st);
         case GV_3M_64x96: return gemm3m_epi<C3_64x96>(a, batch, epi, st);
         case GV_3M_128x48: return gemm3m_epi<C3_128x48>(a, batch, epi, st);
+        case GV_3M_64x48: return gemm3m_epi<C3_64x48>(a, batch, epi, st);
+        case GV_3M_96x32: return gemm3m_epi<C3_96x32>(a, batch, epi, st);
         default: return gemm3m_epi<C3_64x32s4>(a, batch, epi, st);
     }
 }

@@ -157,11 +157,9 @@ lu_leaf_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restri
     }
 }
 
-// ---- leaf panel, version 2: 256 rows per CTA (cluster of up to 16 CTAs = 4096 rows), one __syncthreads and one
-// cluster barrier per column.  Warp arg-max by three redux.sync on the bit pattern of |re|+|im| (non-negative doubles
-// order like unsigned integers) and the row position; the warp winner deposits (value, position, row) in shared
-// memory, warp 0 picks the CTA winner and all its lanes push that candidate to every CTA of the cluster through
-// distributed shared memory; after the cluster barrier every thread scans the <= 16 candidates and updates its row.
+// ---- helpers of the second leaf panel kernel (lu_leaf3_kernel below): 256 rows per CTA, cluster of up to 16 CTAs = 4096
+// rows.  Warp arg-max by three redux.sync on the bit pattern of |re|+|im| (non-negative doubles order like unsigned
+// integers) and the row position.
 constexpr int LEAF2_TPB = 256;
 constexpr int LEAF2_MAXC = 16;
 
@@ -189,15 +187,17 @@ __device__ __forceinline__ bool warp_argmax(double v, int pos, double& wv, int& 
     return cand && (unsigned)pos == mp && mk != 0ull;
 }
 
-#ifdef LEAF_PROFILE
-__device__ long long g_leaf_prof[8];
-#define LEAF_TICK(i) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { long long t_ = clock64(); g_leaf_prof[i] += t_ - tprev_; tprev_ = t_; } } while (0)
-#else
-#define LEAF_TICK(i) do { } while (0)
-#endif
+// ---- leaf panel for up to 4096 rows: one thread = one row, 16 columns in registers, sized to run in the shadow of the
+// GEMM kernel of other stream groups (256 threads x 80 registers = one GEMM CTA slot).  Per column: the warp winner
+// deposits (value, position, row) in shared memory; warp 0 picks the CTA winner and pushes only its 16-byte key (value,
+// position, warp slot) to every CTA of the cluster (distributed shared memory); one cluster barrier; each warp finds the
+// global winner with one redux pass over the keys and warp 0 PULLS the winner's row (16 x 16 B) out of the winning
+// CTA's shared memory; rank-1 update in registers.  Measured 2.7 (4 CTAs) - 4.3 (16 CTAs) us per column against 4.9 - 9.0
+// for lu_leaf_kernel, which remains for panels of more than 4096 rows (the 2bs corner system at bs = 4096).
+struct LeafKey { double val; int pos; int warp; };
 
-__global__ void __launch_bounds__(LEAF2_TPB, 1)
-lu_leaf2_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restrict__ ipiv, int ipiv_stride,
+__global__ void __launch_bounds__(LEAF2_TPB, 3)
+lu_leaf3_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restrict__ ipiv, int ipiv_stride,
                 int* __restrict__ info, int info_base) {
     cg::cluster_group cluster = cg::this_cluster();
     const int csize = (int)cluster.num_blocks();
@@ -205,10 +205,10 @@ lu_leaf2_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restr
     const int z = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = LEAF2_TPB / 32;
-    constexpr int CH = (int)(sizeof(LeafCand) / 16);            // 16-byte chunks per candidate
 
-    __shared__ __align__(16) LeafCand slots[2][LEAF2_MAXC];
-    __shared__ __align__(16) LeafCand wcand[NW];
+    __shared__ __align__(16) LeafCand wcand[2][NW];
+    __shared__ __align__(16) LeafKey keys[2][LEAF2_MAXC];
+    __shared__ __align__(16) cplx prow[LEAF_JB];
 
     cplx* __restrict__ A = bptr(Ab, z) + (long long)row0 * ld + col0;
     const int r = crank * LEAF2_TPB + tid;       // my row inside the panel
@@ -230,59 +230,50 @@ lu_leaf2_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restr
 #pragma unroll
     for (int j = 0; j < LEAF_JB; j++) {
         if (j < jb) {
-            const int buf = j & 1;
+            const int par = j & 1;
             double wv; int wp;
-#ifdef LEAF_PROFILE
-            long long tprev_ = clock64();
-#endif
             const double myv = done ? -1.0 : (fabs(a[j].re) + fabs(a[j].im));
             if (warp_argmax(myv, cur_pos, wv, wp)) {
-                LeafCand* c = &wcand[warp];
+                LeafCand* c = &wcand[par][warp];
                 c->val = myv; c->pos = cur_pos;
 #pragma unroll
                 for (int k = 0; k < LEAF_JB; k++) c->row[k] = a[k];
             }
-            if (lane == 0 && wv < 0.0) { wcand[warp].val = -1.0; wcand[warp].pos = 0x7fffffff; }
-            LEAF_TICK(0);
+            if (lane == 0 && wv < 0.0) { wcand[par][warp].val = -1.0; wcand[par][warp].pos = 0x7fffffff; }
             __syncthreads();
-            LEAF_TICK(1);
             if (warp == 0) {
-                double v2 = lane < NW ? wcand[lane].val : -1.0;
-                int p2 = lane < NW ? wcand[lane].pos : 0x7fffffff;
+                double v2 = lane < NW ? wcand[par][lane].val : -1.0;
+                int p2 = lane < NW ? wcand[par][lane].pos : 0x7fffffff;
                 double cv; int cp;
                 bool win = warp_argmax(v2, p2, cv, cp);
                 unsigned bal = __ballot_sync(0xffffffffu, win);
-                const int w = bal ? (__ffs(bal) - 1) : 0;        // no rows in this CTA: wcand[0] already says (-1, max)
-                const uint4* src = reinterpret_cast<const uint4*>(&wcand[w]);
-                for (int idx = lane; idx < CH * csize; idx += 32) {
-                    int c = idx / CH, ch = idx - c * CH;
-                    uint4* dst = reinterpret_cast<uint4*>(cluster.map_shared_rank(&slots[buf][crank], c));
-                    dst[ch] = src[ch];
-                }
+                LeafKey k; k.val = cv; k.pos = cp; k.warp = bal ? (__ffs(bal) - 1) : 0;
+                if (lane < csize) *cluster.map_shared_rank(&keys[par][crank], lane) = k;
             }
-            LEAF_TICK(2);
             cluster.sync();
-            LEAF_TICK(3);
-            // ---- winner among the csize candidates
-            int win = 0; double gv = slots[buf][0].val; int gp = slots[buf][0].pos;
-            for (int c = 1; c < csize; c++) {
-                double cv = slots[buf][c].val; int cp = slots[buf][c].pos;
-                if (cv > gv || (cv == gv && cp < gp)) { gv = cv; gp = cp; win = c; }
-            }
+            // ---- winner among the csize keys (every warp, one redux pass)
+            double kv = -1.0; int kp = 0x7fffffff, kw = 0;
+            if (lane < csize) { LeafKey k = keys[par][lane]; kv = k.val; kp = k.pos; kw = k.warp; }
+            double gv; int gp;
+            bool gwin = warp_argmax(kv, kp, gv, gp);
+            unsigned gbal = __ballot_sync(0xffffffffu, gwin);
+            const int wcta = gbal ? (__ffs(gbal) - 1) : 0;
+            const int wslot = __shfl_sync(0xffffffffu, kw, wcta);
+            if (warp == 0 && lane < LEAF_JB && gv >= 0.0)
+                prow[lane] = cluster.map_shared_rank(&wcand[par][wslot], wcta)->row[lane];
             if (gv < 0.0) { gp = j; }                     // no rows left (m < jb): nothing to do
             const bool singular = !(gv > 0.0);
             if (crank == 0 && tid == 0) {
                 ipiv[(long long)z * ipiv_stride + row0 + j] = row0 + gp;
                 if (singular && gv >= 0.0) atomicCAS(&info[z], 0, info_base + row0 + j + 1);
             }
-            LEAF_TICK(4);
+            __syncthreads();
             if (!done) {
                 if (cur_pos == gp && gv >= 0.0) {
                     done = true; final_pos = j;           // I am the pivot row: becomes row j of U
                 } else {
                     if (cur_pos == j) cur_pos = gp;       // LAPACK swap bookkeeping
                     if (!singular) {
-                        const cplx* prow = slots[buf][win].row;
                         cplx rinv = crecip_fast(prow[j]);
                         cplx l = cmul(a[j], rinv);
                         a[j] = l;
@@ -291,9 +282,9 @@ lu_leaf2_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restr
                     }
                 }
             }
-            LEAF_TICK(5);
         }
     }
+    cluster.sync();                                   // no CTA may exit while another still reads its shared memory
     if (valid) {
         if (!done) final_pos = cur_pos;
         cplx* dst = A + (long long)final_pos * ld;
@@ -361,7 +352,9 @@ trsm_leaf_kernel(BPtr Ab, int ld, int row0, int jb, int c0, int w) {
 }
 
 // Inverse of an nt x nt (nt <= 128) triangular block T (row-major, ld) into Tinv (row-major, ldo = 128-padded):
-// lower (unit or not) or upper.  16x16 blocked forward substitution, one CTA (256 threads) per (block column, matrix).
+// lower (unit or not) or upper.  16x16 blocked forward substitution, one CTA (256 threads) per (block column, matrix):
+// the 8 diagonal 16x16 blocks are inverted up front (one thread per block column of each), the off-diagonal block rows
+// are prefetched one step ahead, every step is two 16x16 products out of shared memory.
 // Upper is handled as the index-reversed lower problem.  Everything outside the triangle of Tinv (up to the
 // padded size pad) is written as zero, the padded diagonal as one.
 struct TrtriArgs {
@@ -376,9 +369,12 @@ struct TrtriArgs {
 __global__ void __launch_bounds__(256)
 trtri_kernel(TrtriArgs p) {
     constexpr int B = 16, NBK = 8, P = 128;
-    __shared__ cplx X[NBK][B][B + 1];    // inverse blocks of my block column
-    __shared__ cplx D[B][B + 1];
-    __shared__ cplx S[B][B + 1];
+    extern __shared__ __align__(16) unsigned char trtri_smem[];
+    typedef cplx Tile[B][B + 1];
+    Tile* X = reinterpret_cast<Tile*>(trtri_smem);          // [NBK] inverse blocks of my block column
+    Tile* Di = X + NBK;                                     // [NBK] first the diagonal blocks, then their inverses
+    Tile* Lr = Di + NBK;                                    // [NBK-1] block row ib of the matrix, columns jbk .. ib-1
+    Tile& S = *(Lr + (NBK - 1));
     const int jbk = blockIdx.x, yb = blockIdx.y, z = blockIdx.z;
     const int nt = min(P, p.n_total - P * yb);
     const cplx* __restrict__ T = bptr(p.T, z) + (long long)yb * p.t_step;
@@ -393,47 +389,70 @@ trtri_kernel(TrtriArgs p) {
         int ii = upper ? nt - 1 - i : i, jj = upper ? nt - 1 - j : j;
         return T[(long long)ii * p.ld + jj];
     };
-    auto diag_inverse = [&](int bk) {      // D <- inverse of diagonal block bk (lower, 16x16)
-        S[tr][tc] = elem(bk * B + tr, bk * B + tc);
-        __syncthreads();
-        if (tid < B) {
-            int c = tid;
-            cplx x[B];
+    // ---- all diagonal blocks jbk .. 7 at once: load, then one thread per (block, column) inverts by substitution
+    for (int bk = jbk; bk < NBK; bk++) Di[bk][tr][tc] = elem(bk * B + tr, bk * B + tc);
+    cplx pre[NBK - 1];                     // prefetch of block row jbk + 1
 #pragma unroll
-            for (int i = 0; i < B; i++) x[i] = make_c(0.0, 0.0);
+    for (int kb = 0; kb < NBK - 1; kb++)
+        pre[kb] = (jbk + 1 < NBK && jbk + kb < jbk + 1) ? elem((jbk + 1) * B + tr, (jbk + kb) * B + tc) : make_c(0.0, 0.0);
+    __syncthreads();
+    {
+        const int bk = jbk + tid / B, c = tid % B;
+        cplx x[B];
+#pragma unroll
+        for (int i = 0; i < B; i++) x[i] = make_c(0.0, 0.0);
+        if (bk < NBK) {
 #pragma unroll
             for (int i = 0; i < B; i++) {
                 if (i >= c) {
                     cplx s = make_c(i == c ? 1.0 : 0.0, 0.0);
 #pragma unroll
                     for (int k = 0; k < B; k++)
-                        if (k >= c && k < i) s = cfnma(s, S[i][k], x[k]);
-                    x[i] = cmul(s, crecip(S[i][i]));
+                        if (k >= c && k < i) s = cfnma(s, Di[bk][i][k], x[k]);
+                    x[i] = cmul(s, crecip(Di[bk][i][i]));
                 }
             }
-#pragma unroll
-            for (int i = 0; i < B; i++) D[i][c] = x[i];
         }
-        __syncthreads();
-    };
-    diag_inverse(jbk);
-    X[jbk][tr][tc] = D[tr][tc];
-    __syncthreads();
-    for (int ib = jbk + 1; ib < NBK; ib++) {
-        cplx s = make_c(0.0, 0.0);
-        for (int kb = jbk; kb < ib; kb++) {
+        __syncthreads();                   // everyone has read the blocks: overwrite them with the inverses
+        if (bk < NBK) {
 #pragma unroll
-            for (int k = 0; k < B; k++) s = cfma(s, elem(ib * B + tr, kb * B + k), X[kb][k][tc]);
+            for (int i = 0; i < B; i++) Di[bk][i][c] = x[i];
         }
-        diag_inverse(ib);                  // syncs inside; S is overwritten there, so stash s afterwards
-        S[tr][tc] = s;
-        __syncthreads();
-        cplx o = make_c(0.0, 0.0);
-#pragma unroll
-        for (int k = 0; k < B; k++) o = cfnma(o, D[tr][k], S[k][tc]);
-        X[ib][tr][tc] = o;
-        __syncthreads();
     }
+    __syncthreads();
+    X[jbk][tr][tc] = Di[jbk][tr][tc];
+    // ---- block forward substitution down my block column; block row ib + 1 is prefetched while row ib is used
+    for (int ib = jbk + 1; ib < NBK; ib++) {
+        const int nk = ib - jbk;
+#pragma unroll
+        for (int kb = 0; kb < NBK - 1; kb++)
+            if (kb < nk) Lr[kb][tr][tc] = pre[kb];
+        if (ib + 1 < NBK) {
+#pragma unroll
+            for (int kb = 0; kb < NBK - 1; kb++)
+                if (kb < nk + 1) pre[kb] = elem((ib + 1) * B + tr, (jbk + kb) * B + tc);
+        }
+        __syncthreads();
+        cplx s0 = make_c(0.0, 0.0), s1 = make_c(0.0, 0.0);
+        for (int kb = 0; kb < nk; kb++) {
+#pragma unroll
+            for (int k = 0; k < B; k += 2) {
+                s0 = cfma(s0, Lr[kb][tr][k], X[jbk + kb][k][tc]);
+                s1 = cfma(s1, Lr[kb][tr][k + 1], X[jbk + kb][k + 1][tc]);
+            }
+        }
+        S[tr][tc] = make_c(s0.re + s1.re, s0.im + s1.im);
+        __syncthreads();
+        cplx o0 = make_c(0.0, 0.0), o1 = make_c(0.0, 0.0);
+#pragma unroll
+        for (int k = 0; k < B; k += 2) {
+            o0 = cfnma(o0, Di[ib][tr][k], S[k][tc]);
+            o1 = cfnma(o1, Di[ib][tr][k + 1], S[k + 1][tc]);
+        }
+        X[ib][tr][tc] = make_c(o0.re + o1.re, o0.im + o1.im);
+        // the next iteration's first barrier orders these writes before anyone reads X[ib] or rewrites Lr / S
+    }
+    __syncthreads();
     // write block column jbk of the inverse (zeros above the diagonal blocks), undoing the index reversal.
     // Reversal applies to the nt x nt part only; the identity padding stays in place.
     for (int ib = 0; ib < NBK; ib++) {
@@ -444,6 +463,17 @@ trtri_kernel(TrtriArgs p) {
         if (upper && ((i < nt) != (j < nt))) v = make_c(0.0, 0.0);
         O[(long long)oi * P + oj] = v;
     }
+}
+
+constexpr int TRTRI_SMEM = (8 + 8 + 7 + 1) * 16 * 17 * (int)sizeof(cplx);
+
+static void launch_trtri(cudaStream_t st, const TrtriArgs& t, int yblocks, int batch) {
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(trtri_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRTRI_SMEM);
+        configured = true;
+    }
+    trtri_kernel<<<dim3(8, (unsigned)yblocks, (unsigned)batch), 256, TRTRI_SMEM, st>>>(t);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -536,18 +566,18 @@ static inline GemmArgs gemm_std(int M, int N, int K, double alpha, BPtr A, int l
     return g;
 }
 
-static int g_leaf_version = 2;       // 1 = lu_leaf_kernel (512 rows / CTA), 2 = lu_leaf2_kernel (256 rows / CTA)
+static int g_leaf_version = 3;       // 1 = always lu_leaf_kernel (512 rows / CTA), 3 = lu_leaf3_kernel (256 rows / CTA) up to 4096 rows
 
 static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, int jb, const LuWork& w, int info_base,
                         int batch) {
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(lu_leaf_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        cudaFuncSetAttribute(lu_leaf2_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        cudaFuncSetAttribute(lu_leaf3_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         configured = true;
     }
-    const bool v2 = (g_leaf_version == 2) && m <= 4 * LEAF2_TPB;     // measured: v2 wins up to 4 CTAs per cluster
-    const int tpb = v2 ? LEAF2_TPB : LEAF_TPB;
+    const bool v3 = (g_leaf_version == 3) && m <= LEAF2_TPB * LEAF2_MAXC;
+    const int tpb = v3 ? LEAF2_TPB : LEAF_TPB;
     int need = (m + tpb - 1) / tpb;
     int csize = 1;
     while (csize < need) csize <<= 1;
@@ -563,8 +593,8 @@ static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, in
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (v2)
-        ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf2_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
+    if (v3)
+        ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf3_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
     else
         ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
 }
@@ -606,7 +636,7 @@ static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, in
             TrtriArgs t{};
             t.T = bp_offset(Ab, (long long)j0 * ld + j0); t.ld = ld; t.t_step = 0; t.n_total = nbw;
             t.out = w.tinv; t.nblocks = 1; t.upper = 0; t.unit = 1;
-            trtri_kernel<<<dim3(8, 1, (unsigned)batch), 256, 0, ctx.st>>>(t);
+            launch_trtri(ctx.st, t, 1, batch);
             ctx.note(cudaGetLastError());
             ctx.use(CLS_LO);
             BPtr A12 = bp_offset(Ab, (long long)j0 * ld + j0 + nbw);
@@ -631,7 +661,7 @@ static void back_substitute(Ctx& ctx, BPtr Ab, int ld, int n, int nrhs, BPtr X, 
     t.T = Ab; t.ld = ld; t.t_step = (long long)P * ld + P; t.n_total = n; t.out = w.tinv; t.nblocks = nblk;
     t.upper = 1; t.unit = 0;
     ctx.use(CLS_HI);
-    trtri_kernel<<<dim3(8, (unsigned)nblk, (unsigned)batch), 256, 0, ctx.st>>>(t);
+    launch_trtri(ctx.st, t, nblk, batch);
     ctx.note(cudaGetLastError());
     ctx.use(CLS_LO);
     for (int jb = nblk - 1; jb >= 0; jb--) {
