@@ -76,3 +76,51 @@ def test_product_does_not_import_oracle():
         if f.endswith(".py"):
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(from|import)\s+(paper_1812_01396_b200|ctypes)\b", src, flags=re.M), f
+
+
+def test_host_side_argument_logic_without_a_device(libpath):
+    """Calls that must answer from host logic alone (no CUDA work): argument validation, closed forms, strings."""
+    from ctypes import byref, c_void_p
+    from paper_1812_01396_b200 import binding
+    lib = binding.load()
+    h = c_void_p()
+    # nb >= 2, 1 <= bs <= 4096, n_energy >= 1 (include/splitsolve.h "Limits"); rejected before any CUDA call
+    for nb, bs, ne in ((1, 8, 1), (2, 0, 1), (2, 4097, 1), (2, 8, 0)):
+        assert lib.ss_create(nb, bs, ne, byref(h)) == binding.SS_ERR_INVALID_ARG
+        assert not h.value
+    assert lib.ss_create(2, 8, 1, None) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_destroy(None) == binding.SS_OK
+    assert lib.ss_solve(None, None, None, None, None, None, 0, None, None) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_transmission(None, None) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_set_option(None, b"nb_lu", 64) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_strerror(binding.SS_OK) == b"ok" and lib.ss_strerror(binding.SS_ERR_SINGULAR) == b"exactly zero pivot"
+    assert lib.ss_workspace_bytes(1, 8, 1, 1) == 0 and lib.ss_workspace_bytes(2, 8, 1, -1) == 0
+    # workspace grows with every size argument and is dominated by the 2 (nb+1) bs^2 slots per energy
+    w = lib.ss_workspace_bytes(32, 2048, 8, 256)
+    assert w >= 8 * 2 * 33 * 2048 * 2048 * 16
+    assert lib.ss_workspace_bytes(32, 2048, 8, 512) > w and lib.ss_workspace_bytes(33, 2048, 8, 256) > w
+    assert w < 100e9                                   # config C3 fits a B200 (DESIGN.md section 5)
+    assert lib.ss_workspace_bytes(24, 4096, 4, 512) < 100e9
+    assert lib.ss_flops(None, 1) == 0.0 and lib.ss_flops_sweep(None) == 0.0
+    d = binding.get_default_gemm_variant()
+    assert lib.ss_set_default_gemm_variant(-1) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_set_default_gemm_variant(len(binding.GEMM_VARIANTS)) == binding.SS_ERR_INVALID_ARG
+    assert binding.get_default_gemm_variant() == d
+    assert lib.ss_zgemm_batched(-1, 1, 1, 1.0, None, 1, 0, None, 1, 0, 0.0, None, 1, 0, 1, None) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_zgetrf_batched(0, 0, None, 0, 0, None, None, 1, None) == binding.SS_ERR_INVALID_ARG
+
+
+def test_closed_form_flop_counts_match_survey_table():
+    """F_sweep = (160/3 nb - 32) bs^3; per-energy totals 0.505 / 16.0 / 97.4 TFLOP for C2-C4.
+    (ss_flops needs a handle, hence a device; the same closed form is restated here against the table.)"""
+    def f_sweep(nb, bs):
+        return (160.0 / 3.0 * nb - 32.0) * bs ** 3
+
+    def f_total(nb, bs, m):
+        return f_sweep(nb, bs) + (32 + 64 / 3) * bs ** 3 + 32 * bs * bs * m + 16 * nb * bs * bs * m + 64 * bs ** 3 + 8 * bs * bs
+    assert abs(f_sweep(64, 512) / 1e12 - 0.454) < 5e-4
+    assert abs(f_sweep(32, 2048) / 1e12 - 14.4) < 5e-2
+    assert abs(f_sweep(24, 4096) / 1e12 - 85.8) < 5e-2
+    assert abs(f_total(64, 512, 128) / 1e12 - 0.505) < 1e-3
+    assert abs(f_total(32, 2048, 256) / 1e12 - 16.0) < 5e-2
+    assert abs(f_total(24, 4096, 512) / 1e12 - 97.4) < 5e-2
