@@ -174,6 +174,13 @@ ss_status_t ss_zgetrf_batched(int n, int ncols, ss_cplx* AB_dev, int ld, long lo
 ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB_dev, int ld, long long stride, ss_cplx* X_dev, int ldx,
                              long long strideX, int* ipiv_dev, int* info_dev, int batch, void* cuda_stream);
 
+/* Carrier density from the solution ("charge and current densities can be directly
+ * derived from ... c(E)"):  rho[i] = sum_e w[e] * sum_c |X[e][i][c]|^2,  i = 0..n-1.
+ *   X_dev [n_energy][n][nrhs] (the output of ss_solve, n = nb*bs), w_dev [n_energy] doubles (occupation x energy
+ *   integration weight) or NULL = all ones, rho_dev out [n] doubles.  Deterministic (no atomics); enqueued on cuda_stream. */
+ss_status_t ss_density(const ss_cplx* X_dev, int n_energy, long long n, int nrhs, const double* w_dev, double* rho_dev,
+                       void* cuda_stream);
+
 /* Arithmetic / tile shape of the complex GEMM kernel (north_star: "4M or 3M ... whichever reaches the higher fraction
  * of the chip's FP64 peak"):  0 = 4M (four real products per complex product, 64x64 tile);  1..8 = 3M (three real
  * products, P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi); 6 instead of 8 real flops per complex multiply-add; rounding

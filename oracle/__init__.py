@@ -34,5 +34,6 @@ Pin status (tests/test_oracle_pins.py, all `-m "not gpu"`):
   banded.*                               : pinned to dense.* on C0-sized and medium inputs + closed form C1
   residual.backward_error                : pinned to the dense residual on small inputs
   stepwise.*                             : pinned to dense.* (it is itself only a cross-check)
+  observables.density                    : pinned (closed-form perfect chain rho_i = sum_e w_e; brute-force loop)
 No function here is "parity unpinned".
 """

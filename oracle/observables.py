@@ -1,0 +1,22 @@
+"""Observables derived from the wave functions c(E) = X.  TEST INFRASTRUCTURE.
+
+PAPER.md L85: "charge and current densities can be directly derived from G^R(E) or c(E)".  In the wave-function
+formalism the carrier density on orbital i is the occupation-weighted sum over energies and injected modes of the
+squared modulus of the wave-function coefficient (Datta [21]); occupations and integration weights are
+inputs here (they come from the contacts' Fermi functions and the energy grid, which OMEN builds: L250).
+
+Pin status: density -- pinned (tests/test_oracle_pins.py: perfect chain X_j = e^{ikj} 1 gives rho_i = sum_e w_e exactly;
+brute-force python loop on tiny inputs).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def density(X, w=None) -> np.ndarray:
+    """rho[i] = sum_e w[e] * sum_c |X[e, i, c]|^2 ;  X [n_energy, n, nrhs] complex, w [n_energy] real (default ones)."""
+    X = np.asarray(X, dtype=np.complex128)
+    p = (X.real ** 2 + X.imag ** 2).sum(axis=2)              # [n_energy, n]
+    if w is None:
+        return p.sum(axis=0)
+    return np.tensordot(np.asarray(w, dtype=np.float64), p, axes=(0, 0))

@@ -43,6 +43,7 @@ SIGNATURES = {
     "ss_zgesv_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong, c_void_p,
                                  c_void_p, c_int, c_void_p]),
     "ss_fp64_peak_tflops": (c_int, [c_double, POINTER(c_double)]),
+    "ss_density": (c_int, [c_void_p, c_int, c_longlong, c_int, c_void_p, c_void_p, c_void_p]),
     "ss_set_default_gemm_variant": (c_int, [c_int]),
     "ss_get_default_gemm_variant": (c_int, []),
 }
@@ -246,6 +247,18 @@ def zgesv_batched(AB, n):
     _check(load().ss_zgesv_batched(n, nrhs, _dev(AB, "AB"), ncols, n * ncols, _dev(X, "X"), nrhs, n * nrhs,
                                    ipiv.data_ptr(), info.data_ptr(), batch, _stream()), "ss_zgesv_batched")
     return X, ipiv, info
+
+
+def density(X, w=None):
+    """rho[i] = sum_e w[e] sum_c |X[e, i, c]|^2 for X [n_energy, n, nrhs] (CUDA complex128); w CUDA float64 [n_energy] or None."""
+    import torch
+    n_energy, n, nrhs = X.shape
+    rho = torch.empty(n, dtype=torch.float64, device=X.device)
+    if w is not None and not (w.is_cuda and w.dtype == torch.float64 and w.is_contiguous() and w.numel() == n_energy):
+        raise TypeError("w: expected a contiguous CUDA float64 tensor [n_energy]")
+    _check(load().ss_density(_dev(X, "X"), n_energy, n, nrhs, None if w is None else w.data_ptr(), rho.data_ptr(), _stream()),
+           "ss_density")
+    return rho
 
 
 GEMM_VARIANTS = {0: "4M 64x64", 1: "3M auto (64x32 s4 / 64x48 for K>=1024)", 2: "3M 64x32 s3", 3: "3M 64x64", 4: "3M 64x96", 5: "3M 128x48", 6: "3M 64x48", 7: "3M 96x32", 8: "3M 64x32 s4"}

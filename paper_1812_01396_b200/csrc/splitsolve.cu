@@ -717,6 +717,15 @@ extern "C" ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB, int ld, lo
     return lu_common(n, nrhs, n + nrhs, AB, ld, stride, X, ldx, sX, ipiv, info, batch, stream);
 }
 
+extern "C" ss_status_t ss_density(const ss_cplx* X, int n_energy, long long n, int nrhs, const double* w, double* rho,
+                                  void* stream) {
+    if (!X || !rho || n_energy < 1 || n < 1 || nrhs < 1) return SS_ERR_INVALID_ARG;
+    const unsigned blocks = (unsigned)cdiv(n, 8);
+    density_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>((const cplx*)X, n_energy, n, nrhs, w, rho);
+    if (cudaGetLastError() != cudaSuccess) return SS_ERR_CUDA;
+    return SS_OK;
+}
+
 extern "C" ss_status_t ss_set_default_gemm_variant(int variant) {
     if (variant < 0 || variant >= GV_COUNT) return SS_ERR_INVALID_ARG;
     g_default_variant = variant;

@@ -149,6 +149,31 @@ __global__ void trace_final_kernel(const double* __restrict__ partial, int npart
     if (threadIdx.x == 0) T[e] = acc;
 }
 
+// carrier density from the wave functions c(E) = X ("charge and current densities can be
+// directly derived from ... c(E)"):  rho[i] = sum_e w[e] sum_c |X[e][i][c]|^2  (w = occupation x integration weight,
+// supplied by the caller).  HBM-bound: every element of X is read once, 16-byte coalesced; one warp per orbital row,
+// energies accumulated in order in a register (deterministic, no atomics).
+__global__ void __launch_bounds__(256)
+density_kernel(const cplx* __restrict__ X, int n_energy, long long n, int m, const double* __restrict__ w, double* __restrict__ rho) {
+    const int lane = threadIdx.x & 31;
+    const long long row = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= n) return;
+    double total = 0.0;
+    for (int e = 0; e < n_energy; e++) {
+        const double2* __restrict__ x = reinterpret_cast<const double2*>(X + ((long long)e * n + row) * m);
+        double acc = 0.0;
+        for (int c = lane; c < m; c += 32) {
+            double2 v = x[c];
+            acc = fma(v.x, v.x, acc);
+            acc = fma(v.y, v.y, acc);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        total = fma(w ? w[e] : 1.0, acc, total);
+    }
+    if (lane == 0) rho[row] = total;
+}
+
 // FP64 pipe microbenchmark: register-resident DMMA chains (the roofline denominator, measured live).
 __global__ void __launch_bounds__(128) fp64_peak_kernel(double* out, int iters) {
     double c[8][2];

@@ -340,3 +340,28 @@ def test_golden_config0_is_reproducible():
     assert np.allclose(p.E.real, tab[:, 0], atol=1e-15) and np.allclose(p.E.imag, tab[:, 1], atol=1e-18)
     assert np.allclose(T, tab[:, 2], rtol=1e-10)
     assert np.allclose(np.linalg.norm(X, axis=(1, 2)), tab[:, 3], rtol=1e-10)
+
+
+# ------------------------------------------------------------------------------------------------------
+# observables
+# ------------------------------------------------------------------------------------------------------
+def test_density_closed_form_on_the_perfect_chain_and_brute_force():
+    """X_j = e^{ikj} 1 (reading c11) has exactly one unit-modulus entry per row: rho_i = sum_e w_e for every orbital."""
+    from oracle import observables
+    p = inputs.perfect_chain_problem(4, 6, 5)
+    X = np.stack([dense.solve_energy(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e],
+                                     p.Inj_first[e], None)["X"] for e in range(5)])
+    w = np.array([0.5, 1.0, 2.0, 0.25, 3.0])
+    rho = observables.density(X, w)
+    assert np.allclose(rho, w.sum(), rtol=0, atol=1e-11)
+    assert np.allclose(observables.density(X), 5.0, rtol=0, atol=1e-11)
+    # brute force on random data
+    rng = np.random.default_rng(3)
+    Y = rng.standard_normal((3, 7, 4)) + 1j * rng.standard_normal((3, 7, 4))
+    w3 = np.array([1.5, -0.5, 2.0])
+    want = np.zeros(7)
+    for e in range(3):
+        for i in range(7):
+            for c in range(4):
+                want[i] += w3[e] * abs(Y[e, i, c]) ** 2
+    assert np.allclose(observables.density(Y, w3), want, rtol=1e-14, atol=1e-14)

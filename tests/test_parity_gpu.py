@@ -344,3 +344,33 @@ def test_config3_full_size(lib):
 @pytest.mark.slow
 def test_config4_full_size(lib):
     _full_size_check(lib, "C4", n_res=1)
+
+
+# ------------------------------------------------------------------------------------------------------
+# carrier density from X
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb,n_e,nrhs", [(16, 8, 4, 4), (33, 5, 3, 70), (1, 2, 1, 1), (130, 3, 2, 257)])
+def test_density_vs_oracle(lib, bs, nb, n_e, nrhs):
+    from oracle import observables
+    p = inputs.random_problem(bs, nb, n_e, nrhs, seed=14)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    X = ss.solve(p.E, dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first))
+    ss.synchronize()
+    w = np.linspace(0.25, 2.0, n_e)
+    rho = lib.density(X, torch.from_numpy(w).cuda()).cpu().numpy()
+    rho1 = lib.density(X).cpu().numpy()
+    Xo, _ = dense.solve_all(p)
+    want = observables.density(Xo, w)
+    assert np.abs(rho - want).max() <= 1e-9 * np.abs(want).max()
+    # the kernel's own arithmetic on the GPU's X: accumulation order differs from numpy's, values agree to rounding
+    Xg = X.cpu().numpy()
+    assert np.abs(rho - observables.density(Xg, w)).max() <= 1e-13 * np.abs(want).max()
+    assert np.abs(rho1 - observables.density(Xg)).max() <= 1e-13 * np.abs(rho1).max()
+
+
+def test_density_perfect_chain_closed_form(lib):
+    p = inputs.perfect_chain_problem(8, 12, 6)
+    out = run_gpu(lib, p)
+    rho = lib.density(torch.from_numpy(out["X"]).cuda()).cpu().numpy()
+    assert np.abs(rho - 6.0).max() <= 1e-9
