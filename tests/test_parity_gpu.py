@@ -374,3 +374,48 @@ def test_density_perfect_chain_closed_form(lib):
     out = run_gpu(lib, p)
     rho = lib.density(torch.from_numpy(out["X"]).cuda()).cpu().numpy()
     assert np.abs(rho - 6.0).max() <= 1e-9
+
+
+# ------------------------------------------------------------------------------------------------------
+# stream groups: the split of the energies over groups must not change a single bit
+# ------------------------------------------------------------------------------------------------------
+def test_stream_groups_do_not_change_results(lib):
+    """5 energies over 1, 2, 3, 5 and 8 (> n_energy) groups: ragged group sizes, every chain's arithmetic is independent
+    of which launch carries it, so X and T(E) are bit-identical; and all match the oracle."""
+    p = inputs.random_problem(70, 4, 5, 9, seed=15, inj_last=True)
+    ref = run_gpu(lib, p, options={"stream_groups": 1})
+    check_against_oracle(p, ref)
+    for g in (2, 3, 5, 8):
+        out = run_gpu(lib, p, options={"stream_groups": g})
+        assert np.array_equal(out["X"], ref["X"]) and np.array_equal(out["T"], ref["T"]), g
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    for bad in (0, 17):
+        with pytest.raises(lib.SplitSolveError):
+            ss.set_option("stream_groups", bad)
+    ss.close()
+
+
+def test_repeated_solves_on_one_handle_and_other_streams(lib):
+    """Same handle, three solves: default stream, a side stream, default again with other energies; the fork/join of the
+    group streams must order each solve after the previous one."""
+    p = inputs.random_problem(40, 3, 4, 6, seed=16)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    sl, sr, inj = dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first)
+    X1 = ss.solve(p.E, sl, sr, inj).clone()
+    T1 = ss.transmission()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        X2 = ss.solve(p.E, sl, sr, inj)
+        T2 = ss.transmission()
+    side.synchronize()
+    assert torch.equal(X1, X2) and np.array_equal(T1, T2)
+    E2 = p.E[::-1].copy()
+    X3 = ss.solve(E2, sl, sr, inj)
+    T3 = ss.transmission()
+    for e in range(p.n_energy):
+        a = (E2[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], None)
+        r = dense.solve_energy(*a)
+        assert residual.rel_frobenius(X3[e].cpu().numpy(), r["X"]) <= TOL_X
+        assert residual.rel_T(T3[e], r["T_LR"]) <= TOL_T
+    ss.close()
