@@ -142,7 +142,9 @@ ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long*
 
 /* Options: "nb_lu" (outer LU block, 16..128, multiple of 16; default 128), "transmission" (0/1, default 1:
  * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0), "gemm_variant" (see ss_set_default_gemm_variant;
- * default = the process-wide default at ss_create), "trace" (0/1, default 0: record a CUDA-event
+ * default = the process-wide default at ss_create), "cuda_graph" (0/1, default 0: when 1, the second solve with the
+ * same buffers, sizes and options captures the whole launch sequence, all group streams included, into a CUDA graph that
+ * later identical solves replay; measured 2-4 % slower than direct launches on configs C2 and C3, hence off), "trace" (0/1, default 0: record a CUDA-event
  * timeline of every group's high-/low-priority phases, see ss_trace_write), "stream_groups" (1..16,
  * default 4: the energy points are split
  * over that many groups, each with a high-priority stream for the latency-bound panel kernels and a low-priority

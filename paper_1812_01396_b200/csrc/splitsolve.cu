@@ -26,6 +26,15 @@ struct ss_handle_s {
     int stream_groups = 4;
     int want_trace = 0;
     std::vector<TraceRec> trace;
+    // CUDA graph of the solve
+    struct SolveKey { const void *sl, *sr, *i1, *i2, *x; int nrhs, groups, variant, nb_lu, want_T, pad; const void *hd, *hu, *sd, *su; };   // no padding bytes: compared with memcmp
+    int use_graph = 0;       // measured slower than direct launches on every config: off by default
+    SolveKey key{};
+    bool direct_done = false;
+    cudaGraphExec_t graph_exec = nullptr;
+    long long graph_launches = 0;
+    cudaStream_t main_stream = nullptr;
+    cudaEvent_t ev_in = nullptr, ev_out = nullptr;
     GemmProfile prof;
     // stream groups (created on first use): per group a high- and a low-priority stream and two events
     struct GroupRes { cudaStream_t hi = nullptr, lo = nullptr; cudaEvent_t ev_sw = nullptr, ev_mark = nullptr; };
@@ -173,6 +182,10 @@ extern "C" ss_status_t ss_destroy(ss_handle_t h) {
         if (g.ev_mark) cudaEventDestroy(g.ev_mark);
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+    if (h->main_stream) cudaStreamDestroy(h->main_stream);
+    if (h->ev_in) cudaEventDestroy(h->ev_in);
+    if (h->ev_out) cudaEventDestroy(h->ev_out);
     delete h;
     return SS_OK;
 }
@@ -216,6 +229,7 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         h->stream_groups = value; return SS_OK;
     }
     if (!strcmp(name, "trace")) { h->want_trace = value ? 1 : 0; return SS_OK; }
+    if (!strcmp(name, "cuda_graph")) { h->use_graph = value ? 1 : 0; if (!value) { if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; } return SS_OK; }
     if (!strcmp(name, "gemm_variant")) {
         if (value < 0 || value >= GV_COUNT) return SS_ERR_INVALID_ARG;
         h->gemm_variant = value; return SS_OK;
@@ -421,26 +435,20 @@ static bool ensure_groups(ss_handle_t h, int n) {
     return true;
 }
 
-extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L, const ss_cplx* Sigma_R,
-                                const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs, ss_cplx* X,
-                                void* cuda_stream) {
-    if (!h || !E_host || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
-    if (nrhs > 0 && (!Inj_first || !X)) return SS_ERR_INVALID_ARG;
-    if (!h->have_h) return SS_ERR_NOT_READY;
-    ss_status_t st = ensure_workspace(h, nrhs);
-    if (st != SS_OK) return st;
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
-    if (h->solved) cudaEventSynchronize(h->ev[2]);        // E_pinned of the previous call is free again
-    memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
-    h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
+// Everything ss_solve puts on the device, enqueued on `stream` (a non-default stream the handle owns).  With
+// `capturing`, `stream` is in stream-capture mode: the group streams join the capture through the fork event, and the
+// three phase-timing events are recorded as external event nodes so that they carry real timestamps at every replay.
+static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx* Sigma_L, const cplx* Sigma_R,
+                                 const cplx* Inj_first, const cplx* Inj_last, int nrhs, cplx* X, bool capturing) {
+    auto mark = [&](cudaEvent_t ev) {
+        return capturing ? cudaEventRecordWithFlags(ev, stream, cudaEventRecordExternal) : cudaEventRecord(ev, stream);
+    };
     if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-        cudaMemsetAsync(h->info, 0, sizeof(int) * 3 * (size_t)h->n_energy, stream) != cudaSuccess) {
-        cudaGetLastError(); return SS_ERR_CUDA;
-    }
+        cudaMemsetAsync(h->info, 0, sizeof(int) * 3 * (size_t)h->n_energy, stream) != cudaSuccess)
+        return cudaErrorUnknown;
     // Energy points are independent: split them over stream groups.  Group g owns the energies
     // [e0, e0 + nE); the host interleaves the groups' launches step by step so that every group's streams stay fed.
     const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
-    if (nG > 1 && !ensure_groups(h, nG)) { cudaGetLastError(); return SS_ERR_CUDA; }
     std::vector<Group> G((size_t)nG);
     for (int g = 0; g < nG; g++) {
         G[g].e0 = (int)((long long)h->n_energy * g / nG);
@@ -451,7 +459,7 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
         c.prof = h->profile_gemm ? &h->prof : nullptr;
         c.st = stream;
     }
-    cudaEventRecord(h->ev[0], stream);
+    mark(h->ev[0]);
     if (nG > 1) {
         cudaEventRecord(h->ev_fork, stream);
         for (int g = 0; g < nG; g++) {
@@ -476,9 +484,8 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
             cudaEventRecord(h->groups[g].ev_mark, G[g].ctx.st);
             cudaStreamWaitEvent(stream, h->groups[g].ev_mark, 0);
         }
-    cudaEventRecord(h->ev[1], stream);
-    for (int g = 0; g < nG; g++)
-        run_post(h, G[g], (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first, (const cplx*)Inj_last, nrhs, (cplx*)X);
+    mark(h->ev[1]);
+    for (int g = 0; g < nG; g++) run_post(h, G[g], Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X);
     if (nG > 1)
         for (int g = 0; g < nG; g++) {
             G[g].ctx.use(CLS_LO);
@@ -486,14 +493,89 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
             cudaStreamWaitEvent(stream, h->groups[g].ev_mark, 0);
         }
     for (int g = 0; g < nG; g++) G[g].ctx.trace_close();
-    cudaEventRecord(h->ev[2], stream);
+    mark(h->ev[2]);
     h->launches = 0;
     cudaError_t err = cudaSuccess;
     for (int g = 0; g < nG; g++) {
         h->launches += G[g].ctx.launches;
         if (err == cudaSuccess) err = G[g].ctx.err;
     }
-    h->last_stream = stream;
+    return err;
+}
+
+static void drop_graph(ss_handle_t h) {
+    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
+    h->direct_done = false;
+}
+
+extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L, const ss_cplx* Sigma_R,
+                                const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs, ss_cplx* X,
+                                void* cuda_stream) {
+    if (!h || !E_host || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
+    if (nrhs > 0 && (!Inj_first || !X)) return SS_ERR_INVALID_ARG;
+    if (!h->have_h) return SS_ERR_NOT_READY;
+    const int ws_before = h->ws_nrhs;
+    ss_status_t st = ensure_workspace(h, nrhs);
+    if (st != SS_OK) return st;
+    if (h->ws_nrhs != ws_before) drop_graph(h);
+    const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
+    if (nG > 1 && !ensure_groups(h, nG)) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (!h->main_stream) {
+        if (cudaStreamCreateWithFlags(&h->main_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    }
+    cudaStream_t user = (cudaStream_t)cuda_stream, main = h->main_stream;
+    if (h->solved) cudaEventSynchronize(h->ev[2]);        // E_pinned of the previous call is free again
+    memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
+    h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
+    // the solve runs on a stream of the handle (a capture cannot start on the legacy default stream), ordered after the
+    // caller's stream and joined back to it
+    cudaEventRecord(h->ev_in, user);
+    cudaStreamWaitEvent(main, h->ev_in, 0);
+
+    // CUDA graph: the launch sequence of a solve depends only on the sizes, the options and the buffer addresses.  The
+    // first call with a given set enqueues directly; the second identical call captures the same sequence (all group
+    // streams included) into a graph; later calls replay it -- one graph launch instead of 10^4..10^5 kernel launches.
+    ss_handle_s::SolveKey key{Sigma_L, Sigma_R, Inj_first, Inj_last, X, nrhs, nG, h->gemm_variant, h->nb_lu, h->want_T, 0,
+                              h->Hd, h->Hu, h->Sd, h->Su};
+    const bool can_graph = h->use_graph && !h->profile_gemm && !h->want_trace;
+    const bool same = h->direct_done && !memcmp(&key, &h->key, sizeof(key));
+    cudaError_t err = cudaSuccess;
+    bool done = false;
+    if (can_graph && same && h->graph_exec) {
+        err = cudaGraphLaunch(h->graph_exec, main);
+        h->launches = h->graph_launches;
+        done = true;
+    } else if (can_graph && same) {
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(main, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            cudaError_t e1 = enqueue_solve(h, main, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first,
+                                           (const cplx*)Inj_last, nrhs, (cplx*)X, true);
+            cudaError_t e2 = cudaStreamEndCapture(main, &graph);
+            if (e1 == cudaSuccess && e2 == cudaSuccess && graph &&
+                cudaGraphInstantiate(&h->graph_exec, graph, 0) == cudaSuccess) {
+                h->graph_launches = h->launches;
+                err = cudaGraphLaunch(h->graph_exec, main);
+                done = true;
+            } else {
+                h->graph_exec = nullptr;
+                h->use_graph = 0;                           // capture is not possible here: stay with direct launches
+            }
+            if (graph) cudaGraphDestroy(graph);
+        }
+        cudaGetLastError();
+    }
+    if (!done) {
+        if (!same) { if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; } }
+        err = enqueue_solve(h, main, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first, (const cplx*)Inj_last,
+                            nrhs, (cplx*)X, false);
+        h->key = key;
+        h->direct_done = true;
+    }
+    cudaEventRecord(h->ev_out, main);
+    cudaStreamWaitEvent(user, h->ev_out, 0);
+    h->last_stream = user;
     h->last_nrhs = nrhs;
     h->solved = true;
     if (err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }

@@ -395,6 +395,32 @@ def test_stream_groups_do_not_change_results(lib):
     ss.close()
 
 
+def test_cuda_graph_replay_matches_direct_launches(lib):
+    """Option cuda_graph: first solve direct, second captured (all group streams) and launched, third and fourth replayed,
+    the fourth with other energies (E is read from device memory at replay time).  Bit-identical to direct launches."""
+    p = inputs.random_problem(70, 4, 5, 9, seed=17)
+    ref = run_gpu(lib, p)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_option("cuda_graph", 1)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    sl, sr, inj = dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first)
+    X = torch.empty((p.n_energy, p.nb * p.bs, 9), dtype=torch.complex128, device="cuda")
+    for it in range(3):
+        X.zero_()
+        ss.solve(p.E, sl, sr, inj, None, X)
+        T = ss.transmission()
+        assert np.array_equal(X.cpu().numpy(), ref["X"]) and np.array_equal(T, ref["T"]), it
+        assert ss.launch_count() == ref["ss"].launch_count() and ss.phase_ms(2) > 0.0
+    E2 = p.E[::-1].copy()
+    ss.solve(E2, sl, sr, inj, None, X)
+    T = ss.transmission()
+    for e in range(p.n_energy):
+        a = (E2[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], None)
+        r = dense.solve_energy(*a)
+        assert residual.rel_frobenius(X[e].cpu().numpy(), r["X"]) <= TOL_X and residual.rel_T(T[e], r["T_LR"]) <= TOL_T
+    ss.close()
+
+
 def test_repeated_solves_on_one_handle_and_other_streams(lib):
     """Same handle, three solves: default stream, a side stream, default again with other energies; the fork/join of the
     group streams must order each solve after the previous one."""
