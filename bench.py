@@ -37,7 +37,7 @@ EXECUTED_RATIO = {False: 1.0, True: 0.75}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant GEMM shape (a1/a4 of C3: M=N=K=2048,
 # batch 16; algorithmic bytes 3 x 16 x 67.1 MB = 3.22e9) from the committed `ncu --set full` captures
 NCU_TRAFFIC = {False: {"bytes": 7.14e9, "note": "profiles/r01_zgemm_ncu_full.md (4M, 2048^3 x16 launch; algorithmic 3.22e9 B)"},
-               True: {"bytes": 7.48e9, "note": "profiles/r01_zgemm3m_ncu_full.md (3M 64x48, 2048^3 x16 launch; algorithmic 3.22e9 B)"}}
+               True: {"bytes": 7.48e9, "note": "profiles/r01_zgemm3m_ncu_full.md (3M, 2048^3 x16 launch; algorithmic 3.22e9 B)"}}
 
 
 def parse():

@@ -261,7 +261,8 @@ def density(X, w=None):
     return rho
 
 
-GEMM_VARIANTS = {0: "4M 64x64", 1: "3M auto (64x32 s4 / 64x48 for K>=1024)", 2: "3M 64x32 s3", 3: "3M 64x64", 4: "3M 64x96", 5: "3M 128x48", 6: "3M 64x48", 7: "3M 96x32", 8: "3M 64x32 s4"}
+GEMM_VARIANTS = {0: "4M 64x64", 1: "3M auto (64x32: 3 CTAs/SM for K<512, prefetching 2 CTAs/SM above)", 2: "3M 64x32 s3", 3: "3M 64x64", 4: "3M 64x96",
+                 5: "3M 128x48", 6: "3M 64x48", 7: "3M 96x32", 8: "3M 64x32 s4", 9: "3M 64x32 pf"}
 
 
 def set_default_gemm_variant(variant: int):

@@ -21,9 +21,11 @@
 
 namespace ss {
 
-template <int BM_, int BN_, int WARPS_M_, int WARPS_N_, int KC_, int STAGES_, int MINB_>
+template <int BM_, int BN_, int WARPS_M_, int WARPS_N_, int KC_, int STAGES_, int MINB_, int PF_ = 0>
 struct Gemm3Cfg {
     static constexpr int BM = BM_, BN = BN_, WARPS_M = WARPS_M_, WARPS_N = WARPS_N_, KC = KC_, STAGES = STAGES_, MINB = MINB_;
+    static constexpr int PF = PF_;     // 1: fragments of the next k-step are prefetched across the stage boundary
+    static_assert(PF_ == 0 || STAGES_ >= 3, "cross-stage prefetch shortens the cp.async distance by one stage");
     static constexpr int NT = WARPS_M * WARPS_N * 32;
     static constexpr int WM = BM / WARPS_M, WN = BN / WARPS_N;   // warp tile, complex elements
     static constexpr int MI = WM / 8, NJ = WN / 8;               // m8 / n8 tiles per warp
@@ -129,36 +131,91 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
         cp_async_commit();
     }
 
-    for (int kt = 0; kt < KT; kt++) {
-        cp_async_wait<STAGES - 2>();
-        __syncthreads();
-        {
-            int nk = kt + STAGES - 1;
-            if (nk < KT) load_stage(nk, nk % STAGES);
-            cp_async_commit();
+    if (Cfg::PF == 0) {
+        for (int kt = 0; kt < KT; kt++) {
+            cp_async_wait<STAGES - 2>();
+            __syncthreads();
+            {
+                int nk = kt + STAGES - 1;
+                if (nk < KT) load_stage(nk, nk % STAGES);
+                cp_async_commit();
+            }
+            const double* sS = smem + (kt % STAGES) * STAGE_D;
+    #pragma unroll
+            for (int ks = 0; ks < KC / 4; ks++) {
+                double ar[MI], ai[MI], as[MI], br[NJ], bi[NJ], bs[NJ];
+    #pragma unroll
+                for (int i = 0; i < MI; i++) {
+                    double2 v = *reinterpret_cast<const double2*>(sS + a_off + 8 * i * LDA_S + 8 * ks);
+                    ar[i] = v.x; ai[i] = v.y; as[i] = v.x + v.y;
+                }
+    #pragma unroll
+                for (int j = 0; j < NJ; j++) {
+                    double2 v = *reinterpret_cast<const double2*>(sS + b_off + 16 * j + 4 * ks * LDB_S);
+                    br[j] = v.x; bi[j] = v.y; bs[j] = v.x + v.y;
+                }
+    #pragma unroll
+                for (int i = 0; i < MI; i++)
+    #pragma unroll
+                    for (int j = 0; j < NJ; j++) {
+                        dmma884(P1[i][j][0], P1[i][j][1], ar[i], br[j]);
+                        dmma884(P2[i][j][0], P2[i][j][1], ai[i], bi[j]);
+                        dmma884(P3[i][j][0], P3[i][j][1], as[i], bs[j]);
+                    }
+            }
         }
-        const double* sS = smem + (kt % STAGES) * STAGE_D;
-#pragma unroll
-        for (int ks = 0; ks < KC / 4; ks++) {
-            double ar[MI], ai[MI], as[MI], br[NJ], bi[NJ], bs[NJ];
+    } else {
+        // Same product, software-pipelined across the stage boundary: the CTA barrier that publishes stage kt+1 sits
+        // BEFORE the last k-step of stage kt, so that the first fragments of stage kt+1 are already in registers when
+        // stage kt's last DMMAs issue -- no warp starts a stage by waiting for its LDS.
+        constexpr int KS = KC / 4;
+        double fa[2][MI][2], fb[2][NJ][2];
+        auto load_frag = [&](int buf, const double* sS, int ks) {
 #pragma unroll
             for (int i = 0; i < MI; i++) {
                 double2 v = *reinterpret_cast<const double2*>(sS + a_off + 8 * i * LDA_S + 8 * ks);
-                ar[i] = v.x; ai[i] = v.y; as[i] = v.x + v.y;
+                fa[buf][i][0] = v.x; fa[buf][i][1] = v.y;
             }
 #pragma unroll
             for (int j = 0; j < NJ; j++) {
                 double2 v = *reinterpret_cast<const double2*>(sS + b_off + 16 * j + 4 * ks * LDB_S);
-                br[j] = v.x; bi[j] = v.y; bs[j] = v.x + v.y;
+                fb[buf][j][0] = v.x; fb[buf][j][1] = v.y;
             }
+        };
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        if (KT > 0) load_frag(0, smem, 0);
+        int cur = 0;
+        for (int kt = 0; kt < KT; kt++) {
+            const double* sS = smem + (kt % STAGES) * STAGE_D;
 #pragma unroll
-            for (int i = 0; i < MI; i++)
-#pragma unroll
-                for (int j = 0; j < NJ; j++) {
-                    dmma884(P1[i][j][0], P1[i][j][1], ar[i], br[j]);
-                    dmma884(P2[i][j][0], P2[i][j][1], ai[i], bi[j]);
-                    dmma884(P3[i][j][0], P3[i][j][1], as[i], bs[j]);
+            for (int ks = 0; ks < KS; ks++) {
+                if (ks == KS - 1) {
+                    // stage kt+1 must have landed (groups committed so far: STAGES-1+kt; needed complete: kt+2)
+                    cp_async_wait<STAGES - 3>();
+                    __syncthreads();
+                    int nk = kt + STAGES - 1;
+                    if (nk < KT) load_stage(nk, nk % STAGES);      // slot (kt-1) % STAGES: everyone is past stage kt-1
+                    cp_async_commit();
+                    if (kt + 1 < KT) load_frag(cur ^ 1, smem + ((kt + 1) % STAGES) * STAGE_D, 0);
+                } else {
+                    load_frag(cur ^ 1, sS, ks + 1);
                 }
+                double as[MI], bs[NJ];
+#pragma unroll
+                for (int i = 0; i < MI; i++) as[i] = fa[cur][i][0] + fa[cur][i][1];
+#pragma unroll
+                for (int j = 0; j < NJ; j++) bs[j] = fb[cur][j][0] + fb[cur][j][1];
+#pragma unroll
+                for (int i = 0; i < MI; i++)
+#pragma unroll
+                    for (int j = 0; j < NJ; j++) {
+                        dmma884(P1[i][j][0], P1[i][j][1], fa[cur][i][0], fb[cur][j][0]);
+                        dmma884(P2[i][j][0], P2[i][j][1], fa[cur][i][1], fb[cur][j][1]);
+                        dmma884(P3[i][j][0], P3[i][j][1], as[i], bs[j]);
+                    }
+                cur ^= 1;
+            }
         }
     }
     cp_async_wait<0>();
@@ -234,8 +291,9 @@ static cudaError_t gemm3m_launch_t(GemmArgs a, int batch, cudaStream_t st) {
 }
 
 // tile configurations.  Measured on B200 at M=N=K=2048 x 16 (profiles/r01_gemm_variants.md): the small tile with
-// three independent CTAs per SM wins (42.0 TFLOP/s LAPACK-convention vs 34.1 for 4M): with one CTA per SM every
-// __syncthreads idles the whole DMMA pipe, and the larger warp tiles do not fit 3 accumulator sets in registers.
+// several independent CTAs per SM wins (42.0 TFLOP/s LAPACK-convention, 44.2 with the prefetching main loop, vs 34.1
+// for 4M): with one CTA per SM every __syncthreads idles the whole DMMA pipe, and the larger warp tiles do not fit 3
+// accumulator sets in registers.
 using C3_64x32s4 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3>;      // 4 warps of 32x16, 4-stage ring, 3 CTAs/SM   (default)
 using C3_64x32s3 = Gemm3Cfg<64, 32, 2, 2, 8, 3, 3>;      // same, 3-stage ring
 using C3_64x64 = Gemm3Cfg<64, 64, 2, 4, 16, 3, 1>;       // 8 warps of 32x16, 1 CTA/SM
@@ -243,11 +301,12 @@ using C3_64x96 = Gemm3Cfg<64, 96, 2, 4, 16, 3, 1>;       // 8 warps of 32x24
 using C3_128x48 = Gemm3Cfg<128, 48, 4, 2, 16, 3, 1>;     // 8 warps of 32x24
 using C3_64x48 = Gemm3Cfg<64, 48, 2, 2, 8, 4, 2>;        // 4 warps of 32x24, 2 CTAs/SM
 using C3_96x32 = Gemm3Cfg<96, 32, 2, 2, 8, 4, 2>;        // 4 warps of 48x16, 2 CTAs/SM
+using C3_64x32pf = Gemm3Cfg<64, 32, 2, 2, 8, 4, 2, 1>;   // 4 warps of 32x16, cross-stage fragment prefetch, 220 registers, 2 CTAs/SM
 using C3_Tall = Gemm3Cfg<128, 32, 4, 2, 16, 3, 1>;       // one CTA owns all (<=128) rows of its columns: in-place L^-1 * A12
 
 // GEMM variants: 0 = 4M (zgemm.cuh), 1.. = 3M tile shapes.  GEMM_TALL always maps to the one-CTA-per-column
 // configuration of the same arithmetic.
-enum { GV_4M = 0, GV_3M_64x32s4 = 1, GV_3M_64x32s3 = 2, GV_3M_64x64 = 3, GV_3M_64x96 = 4, GV_3M_128x48 = 5, GV_3M_64x48 = 6, GV_3M_96x32 = 7, GV_3M_64x32s4_FIXED = 8, GV_COUNT = 9 };
+enum { GV_4M = 0, GV_3M_64x32s4 = 1, GV_3M_64x32s3 = 2, GV_3M_64x64 = 3, GV_3M_64x96 = 4, GV_3M_128x48 = 5, GV_3M_64x48 = 6, GV_3M_96x32 = 7, GV_3M_64x32s4_FIXED = 8, GV_3M_64x32pf = 9, GV_COUNT = 10 };
 
 template <class Cfg>
 static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_t st) {
@@ -258,9 +317,10 @@ static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_
 static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st, int variant) {
     if (variant == GV_4M) return gemm4m_launch(a, batch, cfg, epi, st);
     if (cfg == GEMM_TALL) return gemm3m_launch_t<C3_Tall, EPI_STD>(a, batch, st);
-    // default (GV_3M_64x32s4): the 64x32 tile, except for long-K products of large matrices, where the 32x24 warp tile
-    // (7 instead of 6 fragment sums per 36 instead of 24 DMMA) is 2 % faster (profiles/r01_gemm_variants.md)
-    if (variant == GV_3M_64x32s4 && a.K >= 1024 && a.M >= 512 && a.N >= 512) variant = GV_3M_64x48;
+    // default (GV_3M_64x32s4): the 64x32 tile at 3 CTAs/SM for short K; from K = 512 on the software-pipelined main loop
+    // (fragments of the next k-step prefetched across the stage boundary, 2 CTAs/SM) is 3-6 % faster (44.2 vs 42.0
+    // TFLOP/s at 2048^3 x 16) while at K = 128 its longer prologue loses 10 % (profiles/r01_gemm_variants.md)
+    if (variant == GV_3M_64x32s4 && a.K >= 512) variant = GV_3M_64x32pf;
     switch (variant) {
         case GV_3M_64x32s3: return gemm3m_epi<C3_64x32s3>(a, batch, epi, st);
         case GV_3M_64x64: return gemm3m_epi<C3_64x64>(a, batch, epi, st);
@@ -268,6 +328,7 @@ static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, c
         case GV_3M_128x48: return gemm3m_epi<C3_128x48>(a, batch, epi, st);
         case GV_3M_64x48: return gemm3m_epi<C3_64x48>(a, batch, epi, st);
         case GV_3M_96x32: return gemm3m_epi<C3_96x32>(a, batch, epi, st);
+        case GV_3M_64x32pf: return gemm3m_epi<C3_64x32pf>(a, batch, epi, st);
         default: return gemm3m_epi<C3_64x32s4>(a, batch, epi, st);
     }
 }

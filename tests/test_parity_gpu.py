@@ -57,7 +57,7 @@ def check_against_oracle(p, out, energies=None, solver=dense):
 @pytest.mark.parametrize("M,N,K,batch", [(64, 64, 64, 1), (1, 1, 1, 2), (37, 53, 29, 3), (130, 70, 200, 2),
                                          (200, 16, 3, 2), (5, 300, 17, 1), (64, 64, 0, 1),
                                          (520, 530, 1030, 1)])
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9])
 def test_zgemm_batched_vs_numpy(lib, M, N, K, batch, variant):
     """Every GEMM variant (0 = 4M, 1..5 = 3M tile shapes) against numpy.matmul, normwise bound (3M's error bound is
     normwise, not componentwise: Higham, Accuracy and Stability of Numerical Algorithms, §23.2.4)."""
@@ -77,7 +77,7 @@ def test_zgemm_batched_vs_numpy(lib, M, N, K, batch, variant):
         lib.set_default_gemm_variant(default)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9])
 def test_hot_path_with_every_gemm_variant(lib, variant):
     p = inputs.random_problem(150, 3, 2, 37, seed=13, inj_last=True)
     out = run_gpu(lib, p, options={"gemm_variant": variant})
