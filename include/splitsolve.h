@@ -183,6 +183,13 @@ ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB_dev, int ld, long long
 ss_status_t ss_density(const ss_cplx* X_dev, int n_energy, long long n, int nrhs, const double* w_dev, double* rho_dev,
                        void* cuda_stream);
 
+/* Bond (spectral) current through every block interface, from the solution X of the LAST ss_solve
+ * on this handle (its energies and H, S are used):
+ *     J[e][i] = 2 Im Tr( X_i^H A_{i,i+1}(E_e) X_{i+1} ),   i = 0..nb-2,   A_{i,i+1} = E_e S_{i,i+1} - H_{i,i+1}  (Eq. 5).
+ * At Im E = 0 the interior equations give J[e][i] = J[e][i+1] (current conservation).  X_dev [n_energy][nb*bs][nrhs] as
+ * returned by that solve (nrhs <= its nrhs), J_host out [n_energy][nb-1].  Overwrites handle scratch; synchronises. */
+ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X_dev, int nrhs, double* J_host);
+
 /* Arithmetic / tile shape of the complex GEMM kernel (north_star: "4M or 3M ... whichever reaches the higher fraction
  * of the chip's FP64 peak"):  0 = 4M (four real products per complex product, 64x64 tile);  1..9 = 3M (three real
  * products, P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi); 6 instead of 8 real flops per complex multiply-add; rounding

@@ -35,5 +35,6 @@ Pin status (tests/test_oracle_pins.py, all `-m "not gpu"`):
   residual.backward_error                : pinned to the dense residual on small inputs
   stepwise.*                             : pinned to dense.* (it is itself only a cross-check)
   observables.density                    : pinned (closed-form perfect chain rho_i = sum_e w_e; brute-force loop)
+  observables.bond_current               : pinned (conservation at Im E = 0; perfect chain J = 2 bs sin k; brute-force loop)
 No function here is "parity unpinned".
 """

@@ -44,6 +44,7 @@ SIGNATURES = {
                                  c_void_p, c_int, c_void_p]),
     "ss_fp64_peak_tflops": (c_int, [c_double, POINTER(c_double)]),
     "ss_density": (c_int, [c_void_p, c_int, c_longlong, c_int, c_void_p, c_void_p, c_void_p]),
+    "ss_bond_current": (c_int, [c_void_p, c_void_p, c_int, c_void_p]),
     "ss_set_default_gemm_variant": (c_int, [c_int]),
     "ss_get_default_gemm_variant": (c_int, []),
 }
@@ -188,6 +189,13 @@ class SplitSolve:
         ms, fl, n = c_double(), c_double(), c_longlong()
         _check(load().ss_gemm_profile(self._h, byref(ms), byref(fl), byref(n)), "ss_gemm_profile")
         return float(ms.value), float(fl.value), int(n.value)
+
+    def bond_current(self, X):
+        """J[e, i] = 2 Im Tr(X_i^H A_{i,i+1}(E_e) X_{i+1}) for the X of the last solve: numpy float64 [n_energy, nb-1]."""
+        import numpy as np
+        J = np.empty((self.n_energy, self.nb - 1), dtype=np.float64)
+        _check(load().ss_bond_current(self._h, _dev(X, "X"), int(X.shape[-1]), J.ctypes.data), "ss_bond_current")
+        return J
 
     def trace_write(self, path: str):
         _check(load().ss_trace_write(self._h, str(path).encode()), "ss_trace_write")

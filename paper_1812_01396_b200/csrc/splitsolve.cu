@@ -411,7 +411,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
                                bp_strided(w2, B2), bs);
         gemm_run(ctx, g4, nE, GEMM_BIG, EPI_STD);
         int parts = (int)min((long long)TRACE_PARTS, cdiv(B2, 256));
-        trace_partial_kernel<<<dim3((unsigned)parts, (unsigned)nE), 256, 0, ctx.st>>>(w2, g1n, B2, B2,
+        trace_partial_kernel<<<dim3((unsigned)parts, (unsigned)nE), 256, 0, ctx.st>>>(w2, B2, g1n, B2, B2, 0,
                                                                                        h->tpart + (long long)e0 * TRACE_PARTS);
         ctx.note(cudaGetLastError());
         trace_final_kernel<<<nE, 32, 0, ctx.st>>>(h->tpart + (long long)e0 * TRACE_PARTS, parts, h->T_dev + e0);
@@ -805,6 +805,39 @@ extern "C" ss_status_t ss_density(const ss_cplx* X, int n_energy, long long n, i
     const unsigned blocks = (unsigned)cdiv(n, 8);
     density_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>((const cplx*)X, n_energy, n, nrhs, w, rho);
     if (cudaGetLastError() != cudaSuccess) return SS_ERR_CUDA;
+    return SS_OK;
+}
+
+// bond (spectral) current through every block interface, from the wave functions of the last solve:
+//   J[e][i] = 2 Im Tr( X_i^H A_{i,i+1}(E_e) X_{i+1} ),  A_{i,i+1} = E S_{i,i+1} - H_{i,i+1}   (Eq. 5; L85).
+// Per interface: a0's form kernel for all energies, one batched GEMM W = A_{i,i+1} X_{i+1}, one conj-dot reduction.
+extern "C" ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X, int nrhs, double* J_host) {
+    if (!h || !X || !J_host || nrhs < 1) return SS_ERR_INVALID_ARG;
+    if (!h->solved || nrhs > h->ws_nrhs) return SS_ERR_NOT_READY;
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    const int nb = h->nb, bs = h->bs, nE = h->n_energy, m = nrhs;
+    const long long B2 = (long long)bs * bs, sX = (long long)nb * bs * m, sW = (long long)bs * m;
+    double* J_dev = nullptr;
+    if (cudaMalloc((void**)&J_dev, sizeof(double) * (size_t)nE * (nb - 1)) != cudaSuccess) { cudaGetLastError(); return SS_ERR_ALLOC; }
+    Ctx ctx; ctx.st = h->main_stream ? h->main_stream : h->last_stream; ctx.variant = h->gemm_variant;
+    const BPtr aop = bp_chain(h->aop, h->aop + B2, 2 * B2);
+    const int parts = (int)min((long long)TRACE_PARTS, cdiv(sW, 256));
+    for (int i = 0; i + 1 < nb; i++) {
+        FormSide up{h->Su + (long long)i * B2, h->Hu + (long long)i * B2, FORM_PLAIN}, none{nullptr, nullptr, FORM_NONE};
+        launch_form(ctx, up, none, h->E_dev, aop, bs, bs, 2 * nE);
+        GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_strided(h->aop, 2 * B2), bs,
+                              bp_strided((const cplx*)X + (long long)(i + 1) * bs * m, sX), m, 0.0, bp_strided(h->wz, sW), m);
+        gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
+        trace_partial_kernel<<<dim3((unsigned)parts, (unsigned)nE), 256, 0, ctx.st>>>(
+            h->wz, sW, (const cplx*)X + (long long)i * bs * m, sX, sW, 1, h->tpart);
+        ctx.note(cudaGetLastError());
+        trace_final_kernel<<<nE, 32, 0, ctx.st>>>(h->tpart, parts, J_dev + i, nb - 1, 2.0);
+        ctx.note(cudaGetLastError());
+    }
+    cudaError_t e = cudaMemcpyAsync(J_host, J_dev, sizeof(double) * (size_t)nE * (nb - 1), cudaMemcpyDeviceToHost, ctx.st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx.st);
+    cudaFree(J_dev);
+    if (e != cudaSuccess || ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }
 

@@ -115,18 +115,25 @@ gamma_kernel(const cplx* __restrict__ Sigma, cplx* __restrict__ out, int bs) {
     }
 }
 
-// partial[e][blockIdx.x] = sum over this block's grid-stride slice of Re(W conj(G)) = W.re G.re + W.im G.im
+// partial[e][blockIdx.x] = sum over this block's grid-stride slice of
+//   mode 0:  Re(W conj(G)) = W.re G.re + W.im G.im        (a7: T = Re Tr(W G^H))
+//   mode 1:  Im(conj(G) W) = G.re W.im - G.im W.re        (f3: bond current, Im Tr(X_i^H W))
 __global__ void __launch_bounds__(256)
-trace_partial_kernel(const cplx* __restrict__ Wm, const cplx* __restrict__ G, long long count, long long stride,
-                     double* __restrict__ partial) {
+trace_partial_kernel(const cplx* __restrict__ Wm, long long strideW, const cplx* __restrict__ G, long long strideG,
+                     long long count, int mode, double* __restrict__ partial) {
     const int e = blockIdx.y;
-    const double2* __restrict__ w = reinterpret_cast<const double2*>(Wm + (long long)e * stride);
-    const double2* __restrict__ g = reinterpret_cast<const double2*>(G + (long long)e * stride);
+    const double2* __restrict__ w = reinterpret_cast<const double2*>(Wm + (long long)e * strideW);
+    const double2* __restrict__ g = reinterpret_cast<const double2*>(G + (long long)e * strideG);
     double acc = 0.0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
         double2 a = w[i], b = g[i];
-        acc = fma(a.x, b.x, acc);
-        acc = fma(a.y, b.y, acc);
+        if (mode == 0) {
+            acc = fma(a.x, b.x, acc);
+            acc = fma(a.y, b.y, acc);
+        } else {
+            acc = fma(b.x, a.y, acc);
+            acc = fma(-b.y, a.x, acc);
+        }
     }
     __shared__ double red[8];
 #pragma unroll
@@ -140,13 +147,15 @@ trace_partial_kernel(const cplx* __restrict__ Wm, const cplx* __restrict__ G, lo
     }
 }
 
-__global__ void trace_final_kernel(const double* __restrict__ partial, int nparts, double* __restrict__ T) {
+// T[e * t_stride] = scale * sum of the nparts partials of e
+__global__ void trace_final_kernel(const double* __restrict__ partial, int nparts, double* __restrict__ T, int t_stride = 1,
+                                   double scale = 1.0) {
     const int e = blockIdx.x;
     double acc = 0.0;
     for (int i = threadIdx.x; i < nparts; i += 32) acc += partial[(long long)e * nparts + i];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (threadIdx.x == 0) T[e] = acc;
+    if (threadIdx.x == 0) T[(long long)e * t_stride] = scale * acc;
 }
 
 // carrier density from the wave functions c(E) = X ("charge and current densities can be

@@ -365,3 +365,37 @@ def test_density_closed_form_on_the_perfect_chain_and_brute_force():
             for c in range(4):
                 want[i] += w3[e] * abs(Y[e, i, c]) ** 2
     assert np.allclose(observables.density(Y, w3), want, rtol=1e-14, atol=1e-14)
+
+
+def test_bond_current_conservation_closed_form_and_brute_force():
+    """(1) conservation at Im E = 0 on a random device (follows from the interior block rows, not from the oracle's code);
+    (2) perfect chain: X_j = e^{ikj} 1, A_{i,i+1} = -t 1  =>  J = 2 bs (-t) sin k for every interface;
+    (3) element-by-element python loop on tiny data."""
+    from oracle import observables
+    p = inputs.random_problem(5, 6, 2, 3, seed=21, eta=0.0)
+    for e in range(2):
+        r = dense.solve_energy(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], None)
+        J = observables.bond_current(p.E[e], p.H_upper, p.S_upper, r["X"])
+        assert np.abs(J - J[0]).max() <= 1e-11 * max(1.0, abs(J[0]))
+        assert abs(J[0]) > 1e-6                      # a current does flow (left injection, absorbing right contact)
+    pc = inputs.perfect_chain_problem(3, 7, 4)
+    k = inputs.chain_wavevector(pc.E, -1.0)
+    for e in range(4):
+        r = dense.solve_energy(pc.E[e], pc.H_diag, pc.H_upper, pc.S_diag, pc.S_upper, pc.Sigma_L[e], pc.Sigma_R[e], pc.Inj_first[e], None)
+        J = observables.bond_current(pc.E[e], pc.H_upper, pc.S_upper, r["X"])
+        assert np.allclose(J, 2.0 * 3 * np.sin(k[e]), rtol=0, atol=1e-10)
+    rng = np.random.default_rng(5)
+    bs, nb, m = 2, 3, 2
+    Hu = rng.standard_normal((nb - 1, bs, bs)) + 1j * rng.standard_normal((nb - 1, bs, bs))
+    Su = rng.standard_normal((nb - 1, bs, bs)) + 1j * rng.standard_normal((nb - 1, bs, bs))
+    X = rng.standard_normal((nb * bs, m)) + 1j * rng.standard_normal((nb * bs, m))
+    E = 0.3 + 0.1j
+    want = np.zeros(nb - 1)
+    for i in range(nb - 1):
+        acc = 0.0 + 0.0j
+        for c in range(m):
+            for a in range(bs):
+                for b in range(bs):
+                    acc += np.conj(X[i * bs + a, c]) * (E * Su[i, a, b] - Hu[i, a, b]) * X[(i + 1) * bs + b, c]
+        want[i] = 2.0 * acc.imag
+    assert np.allclose(observables.bond_current(E, Hu, Su, X), want, rtol=1e-13, atol=1e-13)

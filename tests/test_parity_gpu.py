@@ -445,3 +445,22 @@ def test_repeated_solves_on_one_handle_and_other_streams(lib):
         assert residual.rel_frobenius(X3[e].cpu().numpy(), r["X"]) <= TOL_X
         assert residual.rel_T(T3[e], r["T_LR"]) <= TOL_T
     ss.close()
+
+
+@pytest.mark.parametrize("bs,nb,n_e,nrhs,eta", [(16, 8, 4, 4, 1e-3), (33, 5, 3, 70, 0.0), (130, 3, 2, 40, 1e-3)])
+def test_bond_current_vs_oracle(lib, bs, nb, n_e, nrhs, eta):
+    from oracle import observables
+    p = inputs.random_problem(bs, nb, n_e, nrhs, seed=18, eta=eta)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    X = ss.solve(p.E, dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first))
+    J = ss.bond_current(X)
+    T = ss.transmission()                              # still available after the call
+    Xo, To = dense.solve_all(p)
+    for e in range(n_e):
+        want = observables.bond_current(p.E[e], p.H_upper, p.S_upper, Xo[e])
+        assert np.abs(J[e] - want).max() <= 1e-9 * np.abs(want).max(), (e, J[e], want)
+        assert residual.rel_T(T[e], To[e]) <= TOL_T
+        if eta == 0.0:
+            assert np.abs(J[e] - J[e, 0]).max() <= 1e-9 * abs(J[e, 0])     # conservation
+    ss.close()
