@@ -225,6 +225,10 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
     if (EPI == EPI_STD) {
         const cplx* Cin = (p.beta != 0.0) ? bptr(p.Cin, z) : nullptr;
         const double alpha = p.alpha, beta = p.beta;
+        // C += alpha A B in place (the LU / TRSM updates): red.global.add.f64 instead of load-add-store.  Every element
+        // is written by exactly one thread and receives exactly one addition, so the result is the same correctly
+        // rounded c + alpha*acc, deterministic -- but no warp waits for a global load at the end of its tile.
+        const bool red = (beta == 1.0) && (Cin == Cg) && (p.ldcin == p.ldc);
 #pragma unroll
         for (int i = 0; i < MI; i++) {
             int row = m0 + wm0 + 8 * i + g;
@@ -238,6 +242,12 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
                     double re = P1[i][j][h] - P2[i][j][h];
                     double im = P3[i][j][h] - P1[i][j][h] - P2[i][j][h];
                     cplx o = make_c(alpha * re, alpha * im);
+                    if (red) {
+                        double* dst = reinterpret_cast<double*>(Cg + (long long)row * p.ldc + col);
+                        atomicAdd(dst, o.re);
+                        atomicAdd(dst + 1, o.im);
+                        continue;
+                    }
                     if (Cin) {
                         cplx c = Cin[(long long)row * p.ldcin + col];
                         o.re = fma(beta, c.re, o.re);
@@ -317,10 +327,11 @@ static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_
 static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st, int variant) {
     if (variant == GV_4M) return gemm4m_launch(a, batch, cfg, epi, st);
     if (cfg == GEMM_TALL) return gemm3m_launch_t<C3_Tall, EPI_STD>(a, batch, st);
-    // default (GV_3M_64x32s4): the 64x32 tile at 3 CTAs/SM for short K; from K = 512 on the software-pipelined main loop
-    // (fragments of the next k-step prefetched across the stage boundary, 2 CTAs/SM) is 3-6 % faster (44.2 vs 42.0
-    // TFLOP/s at 2048^3 x 16) while at K = 128 its longer prologue loses 10 % (profiles/r01_gemm_variants.md)
-    if (variant == GV_3M_64x32s4 && a.K >= 512) variant = GV_3M_64x32pf;
+    // default (GV_3M_64x32s4): the 64x32 tile at 3 CTAs/SM for short K; from K = 640 on the software-pipelined main loop
+    // (fragments of the next k-step prefetched across the stage boundary, 2 CTAs/SM) is faster (44.2 vs 42.0 TFLOP/s at
+    // 2048^3 x 16; measured crossover between K = 512 and 640) while at K = 128 its longer prologue loses 15 %
+    // (profiles/r01_gemm_variants.md)
+    if (variant == GV_3M_64x32s4 && a.K >= 640) variant = GV_3M_64x32pf;
     switch (variant) {
         case GV_3M_64x32s3: return gemm3m_epi<C3_64x32s3>(a, batch, epi, st);
         case GV_3M_64x64: return gemm3m_epi<C3_64x64>(a, batch, epi, st);
