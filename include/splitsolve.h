@@ -27,6 +27,9 @@
  *   - A handle is not thread-safe.  Device work is enqueued on the stream given to ss_solve (NULL = the
  *     legacy default stream); ss_solve returns after enqueueing, results are complete after
  *     ss_synchronize / ss_transmission or a synchronisation of that stream by the caller.
+ *   - ss_solve first waits (on the host) for the previous ss_solve of the SAME handle to finish: its per-solve scratch
+ *     and the staged energies are reused.  Use one handle per concurrently running solve.
+ *   - One process drives one GPU (the device current at ss_create); kernel attributes are set once per process.
  *   - Limits of this version: 2 <= nb, 1 <= bs <= 4096, 1 <= n_energy, 0 <= nrhs.
  */
 #ifndef SPLITSOLVE_H
