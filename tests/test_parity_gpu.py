@@ -464,3 +464,29 @@ def test_bond_current_vs_oracle(lib, bs, nb, n_e, nrhs, eta):
         if eta == 0.0:
             assert np.abs(J[e] - J[e, 0]).max() <= 1e-9 * abs(J[e, 0])     # conservation
     ss.close()
+
+
+def test_transmission_option_off_and_lu_block_sizes(lib):
+    p = inputs.random_problem(90, 3, 2, 11, seed=19, inj_last=True)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_option("transmission", 0)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    X = ss.solve(p.E, dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first), dev(p.Inj_last)).cpu().numpy()
+    ss.synchronize()
+    with pytest.raises(lib.SplitSolveError) as ei:
+        ss.transmission()
+    assert ei.value.status == lib.SS_ERR_NOT_READY
+    Xo, _ = dense.solve_all(p)
+    for e in range(2):
+        assert residual.rel_frobenius(X[e], Xo[e]) <= TOL_X
+    ss.close()
+    for nb_lu in (16, 64, 128):
+        out = run_gpu(lib, p, options={"nb_lu": nb_lu})
+        check_against_oracle(p, out)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    for bad in (8, 24, 256):
+        with pytest.raises(lib.SplitSolveError):
+            ss.set_option("nb_lu", bad)
+    with pytest.raises(lib.SplitSolveError):
+        ss.set_option("no_such_option", 1)
+    ss.close()
