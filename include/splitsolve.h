@@ -71,7 +71,10 @@ ss_status_t ss_destroy(ss_handle_t h);
 ss_status_t ss_set_hamiltonian(ss_handle_t h, const ss_cplx* H_diag_dev, const ss_cplx* H_upper_dev,
                                const ss_cplx* S_diag_dev, const ss_cplx* S_upper_dev);
 
-/* Same, from HOST buffers: the handle allocates device copies it owns and uploads (synchronous). */
+/* Same, from HOST buffers: the handle allocates device copies it owns and uploads them ASYNCHRONOUSLY, block by block in the
+ * order the sweeps consume them; the next ss_solve waits per block step, so with pinned host memory the upload overlaps
+ * the first block steps.  The host buffers must stay valid and unchanged until that solve has completed (ss_synchronize,
+ * ss_transmission or ss_solve_host returned); pageable buffers are staged before the call returns. */
 ss_status_t ss_set_hamiltonian_host(ss_handle_t h, const ss_cplx* H_diag_host, const ss_cplx* H_upper_host,
                                     const ss_cplx* S_diag_host, const ss_cplx* S_upper_host);
 

@@ -123,7 +123,9 @@ class SplitSolve:
                                          _dev(S_diag, "S_diag"), _dev(S_upper, "S_upper")), "ss_set_hamiltonian")
 
     def set_hamiltonian_host(self, H_diag, H_upper, S_diag, S_upper):
-        """Host buffers: numpy complex128 arrays or CPU torch tensors (C-contiguous)."""
+        """Host buffers: numpy complex128 arrays or CPU torch tensors (C-contiguous).  Uploaded asynchronously (pinned
+        memory): kept alive here until replaced."""
+        self._keep = [H_diag, H_upper, S_diag, S_upper]
         _check(load().ss_set_hamiltonian_host(self._h, _host(H_diag), _host(H_upper), _host(S_diag), _host(S_upper)),
                "ss_set_hamiltonian_host")
 

@@ -18,6 +18,7 @@ struct ss_handle_s {
     const cplx *Hd = nullptr, *Hu = nullptr, *Sd = nullptr, *Su = nullptr;
     cplx* own_hs[4] = {nullptr, nullptr, nullptr, nullptr};
     bool have_h = false, solved = false;
+    bool launched = false;           // some ss_solve has been enqueued: ev[2] is a valid event to wait on
     // options
     int nb_lu = 128;
     int want_T = 1;
@@ -35,6 +36,12 @@ struct ss_handle_s {
     long long graph_launches = 0;
     cudaStream_t main_stream = nullptr;
     cudaEvent_t ev_in = nullptr, ev_out = nullptr;
+    // asynchronous upload of H, S from host buffers (ss_set_hamiltonian_host)
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> up_ev;
+    bool upload_pending = false;
+    cudaEvent_t ev_sig = nullptr;    // ss_solve_host: Sigma / Inj uploads done (only the post-processing waits for it)
+    bool post_wait = false;
     GemmProfile prof;
     // stream groups (created on first use): per group a high- and a low-priority stream and two events
     struct GroupRes { cudaStream_t hi = nullptr, lo = nullptr; cudaEvent_t ev_sw = nullptr, ev_mark = nullptr; };
@@ -184,6 +191,9 @@ extern "C" ss_status_t ss_destroy(ss_handle_t h) {
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
     if (h->main_stream) cudaStreamDestroy(h->main_stream);
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    for (cudaEvent_t e : h->up_ev) cudaEventDestroy(e);
+    if (h->ev_sig) cudaEventDestroy(h->ev_sig);
     if (h->ev_in) cudaEventDestroy(h->ev_in);
     if (h->ev_out) cudaEventDestroy(h->ev_out);
     delete h;
@@ -195,25 +205,50 @@ extern "C" ss_status_t ss_set_hamiltonian(ss_handle_t h, const ss_cplx* Hd, cons
     if (!h || !Hd || !Hu || !Sd || !Su) return SS_ERR_INVALID_ARG;
     h->Hd = (const cplx*)Hd; h->Hu = (const cplx*)Hu; h->Sd = (const cplx*)Sd; h->Su = (const cplx*)Su;
     h->have_h = true; h->solved = false;
+    h->upload_pending = false;
     return SS_OK;
 }
 
+// Host buffers: the blocks are uploaded asynchronously on a copy stream of the handle, in the order the two sweeps
+// consume them (from both ends of the device towards the middle), with one event per pair of ends; block step s of the
+// sweep waits for event s only, so that with pinned host memory the upload runs under the first block steps instead of
+// in front of the solve.  (From pageable memory cudaMemcpyAsync stages synchronously: same result, no overlap.)
 extern "C" ss_status_t ss_set_hamiltonian_host(ss_handle_t h, const ss_cplx* Hd, const ss_cplx* Hu, const ss_cplx* Sd,
                                                const ss_cplx* Su) {
     if (!h || !Hd || !Hu || !Sd || !Su) return SS_ERR_INVALID_ARG;
-    const size_t B2 = (size_t)h->bs * h->bs * sizeof(cplx);
-    const size_t bytes[4] = {B2 * h->nb, B2 * (h->nb - 1), B2 * h->nb, B2 * (h->nb - 1)};
-    const ss_cplx* src[4] = {Hd, Hu, Sd, Su};
-    for (int i = 0; i < 4; i++) {
-        if (!h->own_hs[i] && cudaMalloc((void**)&h->own_hs[i], bytes[i]) != cudaSuccess) {
-            cudaGetLastError(); return SS_ERR_ALLOC;
-        }
-        if (cudaMemcpy(h->own_hs[i], src[i], bytes[i], cudaMemcpyHostToDevice) != cudaSuccess) {
-            cudaGetLastError(); return SS_ERR_CUDA;
-        }
+    const int nb = h->nb;
+    const size_t B2e = (size_t)h->bs * h->bs, B2 = B2e * sizeof(cplx);
+    const size_t bytes[4] = {B2 * nb, B2 * (nb - 1), B2 * nb, B2 * (nb - 1)};
+    for (int i = 0; i < 4; i++)
+        if (!h->own_hs[i] && cudaMalloc((void**)&h->own_hs[i], bytes[i]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_ALLOC; }
+    if (!h->copy_stream && cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
     }
-    return ss_set_hamiltonian(h, (ss_cplx*)h->own_hs[0], (ss_cplx*)h->own_hs[1], (ss_cplx*)h->own_hs[2],
-                              (ss_cplx*)h->own_hs[3]);
+    while ((int)h->up_ev.size() < nb) {
+        cudaEvent_t e;
+        if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+        h->up_ev.push_back(e);
+    }
+    if (h->launched) cudaEventSynchronize(h->ev[2]);      // the previous solve may still read the old blocks
+    std::vector<char> done_d((size_t)nb, 0), done_u((size_t)(nb > 1 ? nb - 1 : 0), 0);
+    bool ok = true;
+    auto put = [&](int which, const ss_cplx* src, int idx) {
+        if (ok && cudaMemcpyAsync(h->own_hs[which] + (size_t)idx * B2e, src + (size_t)idx * B2e, B2, cudaMemcpyHostToDevice,
+                                  h->copy_stream) != cudaSuccess) ok = false;
+    };
+    for (int k = 0; k < nb; k++) {
+        const int dl[2] = {nb - 1 - k, k}, ul[2] = {nb - 2 - k, k};
+        for (int q = 0; q < 2; q++) {
+            if (dl[q] >= 0 && dl[q] < nb && !done_d[dl[q]]) { done_d[dl[q]] = 1; put(0, Hd, dl[q]); put(2, Sd, dl[q]); }
+            if (ul[q] >= 0 && ul[q] < nb - 1 && !done_u[ul[q]]) { done_u[ul[q]] = 1; put(1, Hu, ul[q]); put(3, Su, ul[q]); }
+        }
+        if (ok && cudaEventRecord(h->up_ev[k], h->copy_stream) != cudaSuccess) ok = false;
+    }
+    if (!ok) { cudaGetLastError(); return SS_ERR_CUDA; }
+    ss_status_t st = ss_set_hamiltonian(h, (ss_cplx*)h->own_hs[0], (ss_cplx*)h->own_hs[1], (ss_cplx*)h->own_hs[2],
+                                        (ss_cplx*)h->own_hs[3]);
+    h->upload_pending = true;
+    return st;
 }
 
 extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value) {
@@ -293,6 +328,7 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
 
     const int i_f = nb - s, i_m = s + 1;                       // 1-based block index of each chain
     ctx.use(CLS_HI);
+    if (h->upload_pending) cudaStreamWaitEvent(ctx.st, h->up_ev[s], 0);   // H, S blocks of this step (ss_set_hamiltonian_host)
     // right-hand sides: A_{i,i-1} (column 0) / A_{i,i+1} (column 1); identity at the ends (L164, reading c1)
     FormSide r0 = (i_f > 1) ? FormSide{h->Su + (long long)(i_f - 2) * B2, h->Hu + (long long)(i_f - 2) * B2, FORM_CONJT}
                             : FormSide{nullptr, nullptr, FORM_IDENT};
@@ -360,6 +396,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     cplx *g1n = h->g1n + e0 * B2, *w1 = h->w1 + e0 * B2, *w2 = h->w2 + e0 * B2;
     cplx *gam_l = h->gam_l + e0 * B2, *gam_r = h->gam_r + e0 * B2;
     ctx.use(CLS_HI);
+    if (h->post_wait) cudaStreamWaitEvent(ctx.st, h->ev_sig, 0);          // Sigma, Inj uploaded by ss_solve_host
     {
         dim3 grid((unsigned)min((long long)8, cdiv(W, 256)), (unsigned)(2 * bs), (unsigned)nE);
         corner_init_kernel<<<grid, 256, 0, ctx.st>>>(raug, s_r, W, ldW, bs, m, inj1, inj2);
@@ -526,7 +563,7 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
             cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     }
     cudaStream_t user = (cudaStream_t)cuda_stream, main = h->main_stream;
-    if (h->solved) cudaEventSynchronize(h->ev[2]);        // E_pinned of the previous call is free again
+    if (h->launched) cudaEventSynchronize(h->ev[2]);      // E_pinned of the previous call is free again
     memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
     h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
     // the solve runs on a stream of the handle (a capture cannot start on the legacy default stream), ordered after the
@@ -539,7 +576,7 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
     // streams included) into a graph; later calls replay it -- one graph launch instead of 10^4..10^5 kernel launches.
     ss_handle_s::SolveKey key{Sigma_L, Sigma_R, Inj_first, Inj_last, X, nrhs, nG, h->gemm_variant, h->nb_lu, h->want_T, 0,
                               h->Hd, h->Hu, h->Sd, h->Su};
-    const bool can_graph = h->use_graph && !h->profile_gemm && !h->want_trace;
+    const bool can_graph = h->use_graph && !h->profile_gemm && !h->want_trace && !h->upload_pending && !h->post_wait;
     const bool same = h->direct_done && !memcmp(&key, &h->key, sizeof(key));
     cudaError_t err = cudaSuccess;
     bool done = false;
@@ -578,6 +615,7 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
     h->last_stream = user;
     h->last_nrhs = nrhs;
     h->solved = true;
+    h->launched = true;
     if (err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }
@@ -733,13 +771,26 @@ extern "C" ss_status_t ss_solve_host(ss_handle_t h, const ss_cplx* E_host, const
         h->hp_nrhs = nrhs;
     }
     cudaStream_t st = h->own_stream;
-    bool ok = cudaMemcpyAsync(h->hp_sigl, SigL, nE * B2 * C, cudaMemcpyHostToDevice, st) == cudaSuccess &&
-              cudaMemcpyAsync(h->hp_sigr, SigR, nE * B2 * C, cudaMemcpyHostToDevice, st) == cudaSuccess;
-    if (ok && nrhs > 0) ok = cudaMemcpyAsync(h->hp_inj1, Inj1, inj_bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
-    if (ok && nrhs > 0 && Inj2) ok = cudaMemcpyAsync(h->hp_inj2, Inj2, inj_bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    // Sigma and Inj go up on the copy stream (behind a pending H, S upload, which shares the copy engine anyway); only the
+    // post-processing waits for them, so the sweep starts at once (pre-/post-processing split of PAPER.md L150-152).
+    if (!h->copy_stream && cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    if (!h->ev_sig && cudaEventCreateWithFlags(&h->ev_sig, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_CUDA;
+    }
+    if (h->launched) cudaEventSynchronize(h->ev[2]);      // the previous solve may still read the staging buffers
+    cudaStream_t cs = h->copy_stream;
+    bool ok = cudaMemcpyAsync(h->hp_sigl, SigL, nE * B2 * C, cudaMemcpyHostToDevice, cs) == cudaSuccess &&
+              cudaMemcpyAsync(h->hp_sigr, SigR, nE * B2 * C, cudaMemcpyHostToDevice, cs) == cudaSuccess;
+    if (ok && nrhs > 0) ok = cudaMemcpyAsync(h->hp_inj1, Inj1, inj_bytes, cudaMemcpyHostToDevice, cs) == cudaSuccess;
+    if (ok && nrhs > 0 && Inj2) ok = cudaMemcpyAsync(h->hp_inj2, Inj2, inj_bytes, cudaMemcpyHostToDevice, cs) == cudaSuccess;
+    if (ok) ok = cudaEventRecord(h->ev_sig, cs) == cudaSuccess;
     if (!ok) { cudaGetLastError(); return SS_ERR_CUDA; }
+    h->post_wait = true;
     ss_status_t s = ss_solve(h, E_host, (ss_cplx*)h->hp_sigl, (ss_cplx*)h->hp_sigr, nrhs ? (ss_cplx*)h->hp_inj1 : nullptr,
                              (nrhs && Inj2) ? (ss_cplx*)h->hp_inj2 : nullptr, nrhs, nrhs ? (ss_cplx*)h->hp_x : nullptr, st);
+    h->post_wait = false;
     if (s != SS_OK) return s;
     if (X_host && nrhs > 0 && cudaMemcpyAsync(X_host, h->hp_x, x_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) {
         cudaGetLastError(); return SS_ERR_CUDA;
