@@ -199,8 +199,8 @@ ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X_dev, int nrhs, doubl
 /* Arithmetic / tile shape of the complex GEMM kernel (north_star: "4M or 3M ... whichever reaches the higher fraction
  * of the chip's FP64 peak"):  0 = 4M (four real products per complex product, 64x64 tile);  1..9 = 3M (three real
  * products, P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi); 6 instead of 8 real flops per complex multiply-add; rounding
- * differs, normwise error stays O(u)) with CTA tiles: 1 = 64x32 (3 CTAs/SM for K < 640, software-pipelined main loop at 2 CTAs/SM
- * from K = 640) = the default, 2 = 64x32 (3-stage), 3 = 64x64, 4 = 64x96, 5 = 128x48, 6 = 64x48, 7 = 96x32, 8 / 9 = the two
+ * differs, normwise error stays O(u)) with CTA tiles: 1 = 64x32 (3 CTAs/SM for K < 768, software-pipelined main loop at 2 CTAs/SM
+ * from K = 768) = the default, 2 = 64x32 (3-stage), 3 = 64x64, 4 = 64x96, 5 = 128x48, 6 = 64x48, 7 = 96x32, 8 / 9 = the two
  * 64x32 kernels of the default for every shape.  The process-wide default
  * (initially 1) applies to handles created afterwards and to the handle-less building blocks above. */
 ss_status_t ss_set_default_gemm_variant(int variant);

@@ -70,7 +70,75 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
     const cplx* __restrict__ Ag = bptr(p.A, z);
     const cplx* __restrict__ Bg = bptr(p.B, z);
 
-    // ---- per-thread staging descriptors (chunk c of the A tile: row c / KC, k c % KC; of the B tile: k c / BN, col c % BN)
+    // ---- per-thread staging state (chunk c of the A tile: row c / KC, k c % KC; of the B tile: k c / BN, col c % BN).
+    // Stages are loaded in increasing k order, so each chunk keeps a running global pointer; shared-memory destinations
+    // are 32-bit shared-space addresses; the per-chunk size (16 or 0 = zero fill for rows / columns beyond M / N) is loop
+    // invariant, and only the last, partial k-chunk takes the predicated path.  (The first version recomputed pointers,
+    // predicates and selects for every chunk of every stage: ~85 integer instructions per 48 DMMA.)
+    const cplx* a_p[Cfg::ITER_A]; unsigned a_sd[Cfg::ITER_A]; int a_sz[Cfg::ITER_A];
+    const unsigned smem_u32 = (unsigned)__cvta_generic_to_shared(smem);
+#pragma unroll
+    for (int q = 0; q < Cfg::ITER_A; q++) {
+        int c = tid + q * NT;
+        int row = c / KC, kc = c % KC;
+        bool in = (c < Cfg::CH_A);
+        bool ok = in && (m0 + row) < M;
+        a_sz[q] = ok ? 16 : (in ? 0 : -1);                   // -1: no such chunk
+        a_p[q] = Ag + (long long)(ok ? (m0 + row) : 0) * p.lda + kc;
+        a_sd[q] = smem_u32 + 8u * (unsigned)(row * LDA_S + 2 * kc);
+    }
+    const cplx* b_p[Cfg::ITER_B]; unsigned b_sd[Cfg::ITER_B]; int b_sz[Cfg::ITER_B];
+#pragma unroll
+    for (int q = 0; q < Cfg::ITER_B; q++) {
+        int c = tid + q * NT;
+        int kr = c / BN, col = c % BN;
+        bool in = (c < Cfg::CH_B);
+        bool ok = in && (n0 + col) < N;
+        b_sz[q] = ok ? 16 : (in ? 0 : -1);
+        b_p[q] = Bg + (long long)kr * p.ldb + (ok ? (n0 + col) : 0);
+        b_sd[q] = smem_u32 + 8u * (unsigned)(BM * LDA_S + kr * LDB_S + 2 * col);
+    }
+    const long long b_step = (long long)KC * p.ldb;
+
+    auto cp16 = [](unsigned sdst, const void* g, int bytes) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(sdst), "l"(g), "r"(bytes));
+    };
+    auto load_stage_lean = [&](int kt, int stage) {            // called with kt = 0, 1, 2, ... in order
+        const unsigned soff = (unsigned)(stage * STAGE_D * 8);
+        const int k0 = kt * KC;
+        if (__builtin_expect(k0 + KC <= K, 1)) {
+#pragma unroll
+            for (int q = 0; q < Cfg::ITER_A; q++) {
+                if (a_sz[q] >= 0) cp16(a_sd[q] + soff, a_p[q], a_sz[q]);
+                a_p[q] += KC;
+            }
+#pragma unroll
+            for (int q = 0; q < Cfg::ITER_B; q++) {
+                if (b_sz[q] >= 0) cp16(b_sd[q] + soff, b_p[q], b_sz[q]);
+                b_p[q] += b_step;
+            }
+        } else {                                               // last, partial k-chunk: zero-fill k >= K
+            asm volatile("" ::: "memory");                       // keep this rare path a real branch
+#pragma unroll
+            for (int q = 0; q < Cfg::ITER_A; q++) {
+                int kc = (tid + q * NT) % KC;
+                bool ok = (k0 + kc < K);
+                if (a_sz[q] >= 0) cp16(a_sd[q] + soff, ok ? (const void*)a_p[q] : (const void*)Ag, ok ? a_sz[q] : 0);
+                a_p[q] += KC;
+            }
+#pragma unroll
+            for (int q = 0; q < Cfg::ITER_B; q++) {
+                int kr = (tid + q * NT) / BN;
+                bool ok = (k0 + kr < K);
+                if (b_sz[q] >= 0) cp16(b_sd[q] + soff, ok ? (const void*)b_p[q] : (const void*)Bg, ok ? b_sz[q] : 0);
+                b_p[q] += b_step;
+            }
+        }
+    };
+
+    // ---- the first version of the staging code: descriptors recomputed per stage.  The software-pipelined main loop
+    // (PF = 1) is measurably faster with it (44.2 vs 43.6 TFLOP/s at 2048^3 x 16), the plain loop with the lean one above
+    // (43.6 vs 42.0); unused state of the other version is dead code per instantiation.
     const cplx* a_src[Cfg::ITER_A]; int a_dst[Cfg::ITER_A]; int a_kc[Cfg::ITER_A]; bool a_ok[Cfg::ITER_A];
 #pragma unroll
     for (int q = 0; q < Cfg::ITER_A; q++) {
@@ -92,7 +160,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
         b_dst[q] = (c < Cfg::CH_B) ? BM * LDA_S + kr * LDB_S + 2 * col : -1;
     }
 
-    auto load_stage = [&](int kt, int stage) {
+    auto load_stage_desc = [&](int kt, int stage) {
         double* sbase = smem + stage * STAGE_D;
         const int k0 = kt * KC;
 #pragma unroll
@@ -107,6 +175,10 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
             bool ok = b_ok[q] && (k0 + b_kr[q] < K);
             cp_async16(sbase + b_dst[q], ok ? (const void*)(b_src[q] + (long long)k0 * p.ldb) : (const void*)Bg, ok ? 16 : 0);
         }
+    };
+
+    auto load_stage = [&](int kt, int stage) {
+        if (Cfg::PF) load_stage_desc(kt, stage); else load_stage_lean(kt, stage);
     };
 
     // ---- fragment offsets (doubles, within a stage)
@@ -327,11 +399,11 @@ static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_
 static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st, int variant) {
     if (variant == GV_4M) return gemm4m_launch(a, batch, cfg, epi, st);
     if (cfg == GEMM_TALL) return gemm3m_launch_t<C3_Tall, EPI_STD>(a, batch, st);
-    // default (GV_3M_64x32s4): the 64x32 tile at 3 CTAs/SM for short K; from K = 640 on the software-pipelined main loop
-    // (fragments of the next k-step prefetched across the stage boundary, 2 CTAs/SM) is faster (44.2 vs 42.0 TFLOP/s at
-    // 2048^3 x 16; measured crossover between K = 512 and 640) while at K = 128 its longer prologue loses 15 %
-    // (profiles/r01_gemm_variants.md)
-    if (variant == GV_3M_64x32s4 && a.K >= 640) variant = GV_3M_64x32pf;
+    // default (GV_3M_64x32s4): the 64x32 tile at 3 CTAs/SM (lean staging code: 43.6 TFLOP/s at 2048^3 x 16, 38.9 at K = 128);
+    // for long K the software-pipelined main loop (fragments of the next k-step prefetched across the stage boundary,
+    // 2 CTAs/SM) is another 1-2 % faster (44.2 / 44.6 at 2048^3 / 4096^3); the crossover measured on isolated launches lies
+    // near K = 1200, inside the solve (4 stream groups) K >= 768 is at least as good (profiles/r01_gemm_variants.md)
+    if (variant == GV_3M_64x32s4 && a.K >= 768) variant = GV_3M_64x32pf;
     switch (variant) {
         case GV_3M_64x32s3: return gemm3m_epi<C3_64x32s3>(a, batch, epi, st);
         case GV_3M_64x64: return gemm3m_epi<C3_64x64>(a, batch, epi, st);
