@@ -311,9 +311,16 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
                 for (int h = 0; h < 2; h++) {
                     int col = n0 + wn0 + 8 * j + 2 * t + h;
                     if (col >= N) continue;
-                    double re = P1[i][j][h] - P2[i][j][h];
-                    double im = P3[i][j][h] - P1[i][j][h] - P2[i][j][h];
-                    cplx o = make_c(alpha * re, alpha * im);
+                    // alpha = +-1 (every product of the path): no multiplies -- each FP64 instruction of the epilogue
+                    // costs the DMMA pipe ~6 cycles, 5 per element were 8 % of a K = 128 tile.  -(x) is exact, so the
+                    // results are bit-identical to alpha * (...)
+                    cplx o;
+                    if (alpha == -1.0) {
+                        o = make_c(P2[i][j][h] - P1[i][j][h], (P1[i][j][h] - P3[i][j][h]) + P2[i][j][h]);
+                    } else {
+                        o = make_c(P1[i][j][h] - P2[i][j][h], (P3[i][j][h] - P1[i][j][h]) - P2[i][j][h]);
+                        if (alpha != 1.0) { o.re *= alpha; o.im *= alpha; }
+                    }
                     if (red) {
                         double* dst = reinterpret_cast<double*>(Cg + (long long)row * p.ldc + col);
                         atomicAdd(dst, o.re);
