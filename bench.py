@@ -186,7 +186,12 @@ def run_ours(args, cfg):
         idx = sharding.energy_indices(nE * world, rank, world)
         p.E, p.Sigma_L, p.Sigma_R, p.Inj_first = p.E[idx], p.Sigma_L[idx], p.Sigma_R[idx], p.Inj_first[idx]
     else:
-        p = inputs.random_problem(bs, nb, 1, 1, seed=cfg.seed, threads=threads)      # H, S only
+        if world > 1 and rank != 0:
+            # H, S come from rank 0 by one NCCL broadcast per array (the paper's MPI_Bcast, L212)
+            p = inputs.Problem(bs, nb, *(np.empty((k, bs, bs), dtype=np.complex128) for k in (nb, nb - 1, nb, nb - 1)),
+                               None, None, None, None)
+        else:
+            p = inputs.random_problem(bs, nb, 1, 1, seed=cfg.seed, threads=os.cpu_count() or 1)      # H, S only
         grid = inputs.energy_grid(nE * world, cfg.e_lo, cfg.e_hi, cfg.eta)
         idx = sharding.energy_indices(nE * world, rank, world)
         p.E = grid[idx].copy()
@@ -201,6 +206,13 @@ def run_ours(args, cfg):
     host = {k: pin(getattr(p, k)) for k in ("H_diag", "H_upper", "S_diag", "S_upper", "Sigma_L", "Sigma_R", "Inj_first")}
     devt = {k: v.cuda(non_blocking=True) for k, v in host.items()}
     torch.cuda.synchronize()
+    if world > 1 and cfg.kind != "chain":
+        hs = ("H_diag", "H_upper", "S_diag", "S_upper")
+        sharding.broadcast_hamiltonian([devt[k] for k in hs], 0, world)
+        torch.cuda.synchronize()
+        if rank != 0 and not args.no_e2e:                 # the e2e leg uploads from host buffers: fill them
+            for k in hs:
+                host[k].copy_(devt[k])
 
     if args.gemm_variant is not None:
         binding.set_default_gemm_variant(args.gemm_variant)

@@ -53,3 +53,19 @@ def max_over_ranks(value: float, world: int, device=None) -> float:
     t = torch.tensor([float(value)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def broadcast_hamiltonian(tensors, src: int, world: int):
+    """Replicates H and S on every rank ("one ncclBroadcast of H,S at ss_set_hamiltonian"): the analogue of
+    the paper's MPI_Bcast of the Hamiltonian and overlap matrices to all nodes before they are copied to the GPUs
+    (PAPER.md L212).  `tensors`: the same list of equally shaped torch tensors on every rank (device tensors with nccl, CPU
+    tensors with gloo); rank `src` holds the data, the others receive in place.  complex128 is sent as its float64 view.
+    One collective per array (4 for H_diag, H_upper, S_diag, S_upper); world == 1 is a no-op."""
+    if world == 1:
+        return tensors
+    import torch
+    import torch.distributed as dist
+    for t in tensors:
+        v = torch.view_as_real(t) if t.is_complex() else t
+        dist.broadcast(v, src=src)
+    return tensors

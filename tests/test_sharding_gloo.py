@@ -45,6 +45,31 @@ def _worker(rank, world, port, n_total, out_dir):
         dist.destroy_process_group()
 
 
+def _bcast_worker(rank, world, port, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        p = inputs.random_problem(3, 4, 1, 1, seed=9)
+        names = ("H_diag", "H_upper", "S_diag", "S_upper")
+        if rank == 0:
+            ts = [torch.from_numpy(getattr(p, k).copy()) for k in names]
+        else:
+            ts = [torch.zeros(getattr(p, k).shape, dtype=torch.complex128) for k in names]
+        sharding.broadcast_hamiltonian(ts, 0, world)
+        ok = all(np.array_equal(t.numpy(), getattr(p, k)) for t, k in zip(ts, names))
+        np.save(os.path.join(out_dir, f"ok_{rank}.npy"), np.array([ok]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_hamiltonian_broadcast_replicates_rank0_data(tmp_path):
+    port = _free_port()
+    mp.spawn(_bcast_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    for r in range(2):
+        assert bool(np.load(tmp_path / f"ok_{r}.npy")[0])
+
+
 @pytest.mark.parametrize("world,n_total", [(2, 6), (2, 5), (3, 7)])
 def test_energy_sharding_gather_matches_single_process(tmp_path, world, n_total):
     from oracle import dense
