@@ -11,7 +11,7 @@
 
 using namespace ss;
 
-static int g_default_variant = GV_3M_64x32s4;   // process-wide default GEMM variant (new handles, handle-less building blocks)
+static int g_default_variant = GV_3M;   // process-wide default GEMM variant (new handles, handle-less building blocks)
 
 struct ss_handle_s {
     int nb = 0, bs = 0, n_energy = 0;
@@ -27,19 +27,13 @@ struct ss_handle_s {
     int stream_groups = 4;
     int want_trace = 0;
     std::vector<TraceRec> trace;
-    // CUDA graph of the solve
-    struct SolveKey { const void *sl, *sr, *i1, *i2, *x; int nrhs, groups, variant, nb_lu, want_T, pad; const void *hd, *hu, *sd, *su; };   // no padding bytes: compared with memcmp
-    int use_graph = 0;       // measured slower than direct launches on every config: off by default
-    SolveKey key{};
-    bool direct_done = false;
-    cudaGraphExec_t graph_exec = nullptr;
-    long long graph_launches = 0;
     cudaStream_t main_stream = nullptr;
     cudaEvent_t ev_in = nullptr, ev_out = nullptr;
     // asynchronous upload of H, S from host buffers (ss_set_hamiltonian_host)
     cudaStream_t copy_stream = nullptr;
     std::vector<cudaEvent_t> up_ev;
-    bool upload_pending = false;
+    bool upload_pending = false;     // the next solve must wait for the per-block upload events
+    bool upload_consumed = false;    // a solve that waited for them has been enqueued: cleared once it has completed
     cudaEvent_t ev_sig = nullptr;    // ss_solve_host: Sigma / Inj uploads done (only the post-processing waits for it)
     bool post_wait = false;
     GemmProfile prof;
@@ -99,8 +93,10 @@ static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
     w.slots = (size_t)nE * 2 * (nb + 1) * B2 * C;
     w.aug = (size_t)nE * 2 * bs * pad_ld(2 * bs) * C;
     w.aop = (size_t)nE * 2 * B2 * C;
+    // the sweep and the corner system own disjoint regions: stream groups do not wait for one another between the two
+    // phases, so one group's corner LU may run while another group's sweep still uses its triangular inverses
     int blk_sweep = 2 * nE * (int)cdiv(bs, 128), blk_corner = nE * (int)cdiv(2 * bs, 128);
-    w.tinv_blocks = blk_sweep > blk_corner ? blk_sweep : blk_corner;
+    w.tinv_blocks = blk_sweep + blk_corner;
     w.tinv = (size_t)w.tinv_blocks * 128 * 128 * C;
     size_t W = (size_t)pad_ld(3LL * bs + nrhs), W2 = (size_t)pad_ld(2LL * bs + nrhs);   // with / without the e_2 columns
     if (W2 > W) W = W2;
@@ -189,7 +185,6 @@ extern "C" ss_status_t ss_destroy(ss_handle_t h) {
         if (g.ev_mark) cudaEventDestroy(g.ev_mark);
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
-    if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
     if (h->main_stream) cudaStreamDestroy(h->main_stream);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     for (cudaEvent_t e : h->up_ev) cudaEventDestroy(e);
@@ -206,6 +201,7 @@ extern "C" ss_status_t ss_set_hamiltonian(ss_handle_t h, const ss_cplx* Hd, cons
     h->Hd = (const cplx*)Hd; h->Hu = (const cplx*)Hu; h->Sd = (const cplx*)Sd; h->Su = (const cplx*)Su;
     h->have_h = true; h->solved = false;
     h->upload_pending = false;
+    h->upload_consumed = false;
     return SS_OK;
 }
 
@@ -248,6 +244,7 @@ extern "C" ss_status_t ss_set_hamiltonian_host(ss_handle_t h, const ss_cplx* Hd,
     ss_status_t st = ss_set_hamiltonian(h, (ss_cplx*)h->own_hs[0], (ss_cplx*)h->own_hs[1], (ss_cplx*)h->own_hs[2],
                                         (ss_cplx*)h->own_hs[3]);
     h->upload_pending = true;
+    h->upload_consumed = false;
     return st;
 }
 
@@ -264,7 +261,6 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         h->stream_groups = value; return SS_OK;
     }
     if (!strcmp(name, "trace")) { h->want_trace = value ? 1 : 0; return SS_OK; }
-    if (!strcmp(name, "cuda_graph")) { h->use_graph = value ? 1 : 0; if (!value) { if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; } return SS_OK; }
     if (!strcmp(name, "gemm_variant")) {
         if (value < 0 || value >= GV_COUNT) return SS_ERR_INVALID_ARG;
         h->gemm_variant = value; return SS_OK;
@@ -414,7 +410,8 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
         }
     const int blk_corner = (int)cdiv(2 * bs, 128);
     LuWork w;
-    w.tinv = h->tinv + (long long)e0 * blk_corner * 128 * 128; w.tinv_blocks = nE * blk_corner;
+    const long long blk_sweep_total = 2LL * h->n_energy * cdiv(bs, 128);
+    w.tinv = h->tinv + (blk_sweep_total + (long long)e0 * blk_corner) * 128 * 128; w.tinv_blocks = nE * blk_corner;
     w.ipiv = h->ipiv + (long long)2 * h->n_energy * 2 * bs + (long long)e0 * 2 * bs; w.ipiv_stride = 2 * bs;
     w.info = h->info + 2 * h->n_energy + e0;
     lu_factor(ctx, bp_strided(raug, s_r), ldW, 2 * bs, W, nE, h->nb_lu, w, 0);
@@ -472,14 +469,10 @@ static bool ensure_groups(ss_handle_t h, int n) {
     return true;
 }
 
-// Everything ss_solve puts on the device, enqueued on `stream` (a non-default stream the handle owns).  With
-// `capturing`, `stream` is in stream-capture mode: the group streams join the capture through the fork event, and the
-// three phase-timing events are recorded as external event nodes so that they carry real timestamps at every replay.
+// Everything ss_solve puts on the device, enqueued on `stream` (a non-default stream the handle owns).
 static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx* Sigma_L, const cplx* Sigma_R,
-                                 const cplx* Inj_first, const cplx* Inj_last, int nrhs, cplx* X, bool capturing) {
-    auto mark = [&](cudaEvent_t ev) {
-        return capturing ? cudaEventRecordWithFlags(ev, stream, cudaEventRecordExternal) : cudaEventRecord(ev, stream);
-    };
+                                 const cplx* Inj_first, const cplx* Inj_last, int nrhs, cplx* X) {
+    auto mark = [&](cudaEvent_t ev) { return cudaEventRecord(ev, stream); };
     if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
         cudaMemsetAsync(h->info, 0, sizeof(int) * 3 * (size_t)h->n_energy, stream) != cudaSuccess)
         return cudaErrorUnknown;
@@ -540,21 +533,14 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx*
     return err;
 }
 
-static void drop_graph(ss_handle_t h) {
-    if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
-    h->direct_done = false;
-}
-
 extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L, const ss_cplx* Sigma_R,
                                 const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs, ss_cplx* X,
                                 void* cuda_stream) {
     if (!h || !E_host || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
     if (nrhs > 0 && (!Inj_first || !X)) return SS_ERR_INVALID_ARG;
     if (!h->have_h) return SS_ERR_NOT_READY;
-    const int ws_before = h->ws_nrhs;
     ss_status_t st = ensure_workspace(h, nrhs);
     if (st != SS_OK) return st;
-    if (h->ws_nrhs != ws_before) drop_graph(h);
     const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
     if (nG > 1 && !ensure_groups(h, nG)) { cudaGetLastError(); return SS_ERR_CUDA; }
     if (!h->main_stream) {
@@ -564,54 +550,18 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
     }
     cudaStream_t user = (cudaStream_t)cuda_stream, main = h->main_stream;
     if (h->launched) cudaEventSynchronize(h->ev[2]);      // E_pinned of the previous call is free again
+    if (h->upload_consumed) { h->upload_pending = false; h->upload_consumed = false; }   // that solve saw the whole upload
     memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
     h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
-    // the solve runs on a stream of the handle (a capture cannot start on the legacy default stream), ordered after the
-    // caller's stream and joined back to it
+    // the solve runs on a stream of the handle, ordered after the caller's stream and joined back to it
     cudaEventRecord(h->ev_in, user);
     cudaStreamWaitEvent(main, h->ev_in, 0);
 
-    // CUDA graph: the launch sequence of a solve depends only on the sizes, the options and the buffer addresses.  The
-    // first call with a given set enqueues directly; the second identical call captures the same sequence (all group
-    // streams included) into a graph; later calls replay it -- one graph launch instead of 10^4..10^5 kernel launches.
-    ss_handle_s::SolveKey key{Sigma_L, Sigma_R, Inj_first, Inj_last, X, nrhs, nG, h->gemm_variant, h->nb_lu, h->want_T, 0,
-                              h->Hd, h->Hu, h->Sd, h->Su};
-    const bool can_graph = h->use_graph && !h->profile_gemm && !h->want_trace && !h->upload_pending && !h->post_wait;
-    const bool same = h->direct_done && !memcmp(&key, &h->key, sizeof(key));
-    cudaError_t err = cudaSuccess;
-    bool done = false;
-    if (can_graph && same && h->graph_exec) {
-        err = cudaGraphLaunch(h->graph_exec, main);
-        h->launches = h->graph_launches;
-        done = true;
-    } else if (can_graph && same) {
-        cudaGraph_t graph = nullptr;
-        if (cudaStreamBeginCapture(main, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-            cudaError_t e1 = enqueue_solve(h, main, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first,
-                                           (const cplx*)Inj_last, nrhs, (cplx*)X, true);
-            cudaError_t e2 = cudaStreamEndCapture(main, &graph);
-            if (e1 == cudaSuccess && e2 == cudaSuccess && graph &&
-                cudaGraphInstantiate(&h->graph_exec, graph, 0) == cudaSuccess) {
-                h->graph_launches = h->launches;
-                err = cudaGraphLaunch(h->graph_exec, main);
-                done = true;
-            } else {
-                h->graph_exec = nullptr;
-                h->use_graph = 0;                           // capture is not possible here: stay with direct launches
-            }
-            if (graph) cudaGraphDestroy(graph);
-        }
-        cudaGetLastError();
-    }
-    if (!done) {
-        if (!same) { if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; } }
-        err = enqueue_solve(h, main, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first, (const cplx*)Inj_last,
-                            nrhs, (cplx*)X, false);
-        h->key = key;
-        h->direct_done = true;
-    }
+    cudaError_t err = enqueue_solve(h, main, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first,
+                                    (const cplx*)Inj_last, nrhs, (cplx*)X);
     cudaEventRecord(h->ev_out, main);
     cudaStreamWaitEvent(user, h->ev_out, 0);
+    if (h->upload_pending) h->upload_consumed = true;
     h->last_stream = user;
     h->last_nrhs = nrhs;
     h->solved = true;

@@ -75,6 +75,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
     // are 32-bit shared-space addresses; the per-chunk size (16 or 0 = zero fill for rows / columns beyond M / N) is loop
     // invariant, and only the last, partial k-chunk takes the predicated path.  (The first version recomputed pointers,
     // predicates and selects for every chunk of every stage: ~85 integer instructions per 48 DMMA.)
+    constexpr bool LEAN = (Cfg::PF == 0);
     const cplx* a_p[Cfg::ITER_A]; unsigned a_sd[Cfg::ITER_A]; int a_sz[Cfg::ITER_A];
     const unsigned smem_u32 = (unsigned)__cvta_generic_to_shared(smem);
 #pragma unroll
@@ -136,49 +137,30 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
         }
     };
 
-    // ---- the first version of the staging code: descriptors recomputed per stage.  The software-pipelined main loop
-    // (PF = 1) is measurably faster with it (44.2 vs 43.6 TFLOP/s at 2048^3 x 16), the plain loop with the lean one above
-    // (43.6 vs 42.0); unused state of the other version is dead code per instantiation.
-    const cplx* a_src[Cfg::ITER_A]; int a_dst[Cfg::ITER_A]; int a_kc[Cfg::ITER_A]; bool a_ok[Cfg::ITER_A];
-#pragma unroll
-    for (int q = 0; q < Cfg::ITER_A; q++) {
-        int c = tid + q * NT;
-        int row = c / KC, kc = c % KC;
-        a_kc[q] = (c < Cfg::CH_A) ? kc : (1 << 28);          // beyond the tile: never in range
-        a_ok[q] = (c < Cfg::CH_A) && (m0 + row) < M;
-        a_src[q] = Ag + (long long)(a_ok[q] ? (m0 + row) : 0) * p.lda + kc;
-        a_dst[q] = (c < Cfg::CH_A) ? row * LDA_S + 2 * kc : -1;
-    }
-    const cplx* b_src[Cfg::ITER_B]; int b_dst[Cfg::ITER_B]; int b_kr[Cfg::ITER_B]; bool b_ok[Cfg::ITER_B];
-#pragma unroll
-    for (int q = 0; q < Cfg::ITER_B; q++) {
-        int c = tid + q * NT;
-        int kr = c / BN, col = c % BN;
-        b_kr[q] = (c < Cfg::CH_B) ? kr : (1 << 28);
-        b_ok[q] = (c < Cfg::CH_B) && (n0 + col) < N;
-        b_src[q] = Bg + (long long)kr * p.ldb + (b_ok[q] ? (n0 + col) : 0);
-        b_dst[q] = (c < Cfg::CH_B) ? BM * LDA_S + kr * LDB_S + 2 * col : -1;
-    }
-
+    // ---- staging of the software-pipelined build (PF = 1): descriptors kept per chunk, address and predicate formed per
+    // stage.  Measured, that kernel is faster with this form (44.2 vs 43.6 TFLOP/s at 2048^3 x 16) and the plain loop with
+    // the running pointers above (43.6 vs 42.0); `if constexpr` keeps exactly one of the two in each instantiation.
     auto load_stage_desc = [&](int kt, int stage) {
         double* sbase = smem + stage * STAGE_D;
         const int k0 = kt * KC;
 #pragma unroll
         for (int q = 0; q < Cfg::ITER_A; q++) {
-            if (a_dst[q] < 0) continue;
-            bool ok = a_ok[q] && (k0 + a_kc[q] < K);
-            cp_async16(sbase + a_dst[q], ok ? (const void*)(a_src[q] + k0) : (const void*)Ag, ok ? 16 : 0);
+            if (a_sz[q] < 0) continue;
+            const int kc = (tid + q * NT) % KC;
+            bool ok = a_sz[q] > 0 && (k0 + kc < K);
+            cp_async16(sbase + (a_sd[q] - smem_u32) / 8, ok ? (const void*)(a_p[q] + k0) : (const void*)Ag, ok ? 16 : 0);
         }
 #pragma unroll
         for (int q = 0; q < Cfg::ITER_B; q++) {
-            if (b_dst[q] < 0) continue;
-            bool ok = b_ok[q] && (k0 + b_kr[q] < K);
-            cp_async16(sbase + b_dst[q], ok ? (const void*)(b_src[q] + (long long)k0 * p.ldb) : (const void*)Bg, ok ? 16 : 0);
+            if (b_sz[q] < 0) continue;
+            const int kr = (tid + q * NT) / BN;
+            bool ok = b_sz[q] > 0 && (k0 + kr < K);
+            cp_async16(sbase + (b_sd[q] - smem_u32) / 8, ok ? (const void*)(b_p[q] + (long long)k0 * p.ldb) : (const void*)Bg, ok ? 16 : 0);
         }
     };
 
     auto load_stage = [&](int kt, int stage) {
-        if (Cfg::PF) load_stage_desc(kt, stage); else load_stage_lean(kt, stage);
+        if constexpr (LEAN) load_stage_lean(kt, stage); else load_stage_desc(kt, stage);
     };
 
     // ---- fragment offsets (doubles, within a stage)
@@ -380,23 +362,17 @@ static cudaError_t gemm3m_launch_t(GemmArgs a, int batch, cudaStream_t st) {
 }
 
 // tile configurations.  Measured on B200 at M=N=K=2048 x 16 (profiles/r01_gemm_variants.md): the small tile with
-// several independent CTAs per SM wins (42.0 TFLOP/s LAPACK-convention, 44.2 with the prefetching main loop, vs 34.1
-// for 4M): with one CTA per SM every __syncthreads idles the whole DMMA pipe, and the larger warp tiles do not fit 3
-// accumulator sets in registers.
-using C3_64x32s4 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3>;      // 4 warps of 32x16, 4-stage ring, 3 CTAs/SM   (default)
-using C3_64x32s3 = Gemm3Cfg<64, 32, 2, 2, 8, 3, 3>;      // same, 3-stage ring
-using C3_64x64 = Gemm3Cfg<64, 64, 2, 4, 16, 3, 1>;       // 8 warps of 32x16, 1 CTA/SM
-using C3_64x96 = Gemm3Cfg<64, 96, 2, 4, 16, 3, 1>;       // 8 warps of 32x24
-using C3_128x48 = Gemm3Cfg<128, 48, 4, 2, 16, 3, 1>;     // 8 warps of 32x24
-using C3_64x48 = Gemm3Cfg<64, 48, 2, 2, 8, 4, 2>;        // 4 warps of 32x24, 2 CTAs/SM
-using C3_96x32 = Gemm3Cfg<96, 32, 2, 2, 8, 4, 2>;        // 4 warps of 48x16, 2 CTAs/SM
+// several independent CTAs per SM wins (43.6 TFLOP/s LAPACK-convention, 44.2 with the prefetching main loop, vs 34.1
+// for 4M): with one CTA per SM every __syncthreads idles the whole DMMA pipe, and larger warp tiles do not fit 3
+// accumulator sets in registers.  The other tile shapes tried in round 1 (64x64, 64x96, 128x48, 64x48, 96x32, 3-stage
+// ring) are recorded in that file and are no longer built.
+using C3_64x32s4 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3>;      // 4 warps of 32x16, 4-stage ring, 3 CTAs/SM
 using C3_64x32pf = Gemm3Cfg<64, 32, 2, 2, 8, 4, 2, 1>;   // 4 warps of 32x16, cross-stage fragment prefetch, 220 registers, 2 CTAs/SM
-using C3_Tall = Gemm3Cfg<128, 16, 4, 1, 8, 4, 2>;       // one CTA owns all (<=128) rows of its 16 columns: in-place L^-1 * A12
-                                                         // (2 CTAs/SM; 8 % faster than the first 128x32 / 8 warps / 1 CTA build)
+using C3_Tall = Gemm3Cfg<128, 16, 4, 1, 8, 4, 2>;        // one CTA owns all (<=128) rows of its 16 columns: in-place L^-1 * A12
 
-// GEMM variants: 0 = 4M (zgemm.cuh), 1.. = 3M tile shapes.  GEMM_TALL always maps to the one-CTA-per-column
-// configuration of the same arithmetic.
-enum { GV_4M = 0, GV_3M_64x32s4 = 1, GV_3M_64x32s3 = 2, GV_3M_64x64 = 3, GV_3M_64x96 = 4, GV_3M_128x48 = 5, GV_3M_64x48 = 6, GV_3M_96x32 = 7, GV_3M_64x32s4_FIXED = 8, GV_3M_64x32pf = 9, GV_COUNT = 10 };
+// GEMM variants: 0 = 4M (zgemm.cuh), 1 = 3M, kernel chosen by K (the default), 2 / 3 = the two 3M kernels for every K.
+// GEMM_TALL always maps to the one-CTA-per-column configuration of the same arithmetic.
+enum { GV_4M = 0, GV_3M = 1, GV_3M_LEAN = 2, GV_3M_PF = 3, GV_COUNT = 4 };
 
 template <class Cfg>
 static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_t st) {
@@ -407,21 +383,13 @@ static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_
 static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, cudaStream_t st, int variant) {
     if (variant == GV_4M) return gemm4m_launch(a, batch, cfg, epi, st);
     if (cfg == GEMM_TALL) return gemm3m_launch_t<C3_Tall, EPI_STD>(a, batch, st);
-    // default (GV_3M_64x32s4): the 64x32 tile at 3 CTAs/SM (lean staging code: 43.6 TFLOP/s at 2048^3 x 16, 38.9 at K = 128);
-    // for long K the software-pipelined main loop (fragments of the next k-step prefetched across the stage boundary,
-    // 2 CTAs/SM) is another 1-2 % faster (44.2 / 44.6 at 2048^3 / 4096^3); the crossover measured on isolated launches lies
-    // near K = 1200, inside the solve (4 stream groups) K >= 768 is at least as good (profiles/r01_gemm_variants.md)
-    if (variant == GV_3M_64x32s4 && a.K >= 768) variant = GV_3M_64x32pf;
-    switch (variant) {
-        case GV_3M_64x32s3: return gemm3m_epi<C3_64x32s3>(a, batch, epi, st);
-        case GV_3M_64x64: return gemm3m_epi<C3_64x64>(a, batch, epi, st);
-        case GV_3M_64x96: return gemm3m_epi<C3_64x96>(a, batch, epi, st);
-        case GV_3M_128x48: return gemm3m_epi<C3_128x48>(a, batch, epi, st);
-        case GV_3M_64x48: return gemm3m_epi<C3_64x48>(a, batch, epi, st);
-        case GV_3M_96x32: return gemm3m_epi<C3_96x32>(a, batch, epi, st);
-        case GV_3M_64x32pf: return gemm3m_epi<C3_64x32pf>(a, batch, epi, st);
-        default: return gemm3m_epi<C3_64x32s4>(a, batch, epi, st);
-    }
+    // default: the 64x32 tile at 3 CTAs/SM (lean staging code: 43.6 TFLOP/s at 2048^3 x 16, 38.9 at K = 128); for long K the
+    // software-pipelined main loop (fragments of the next k-step prefetched across the stage boundary, 2 CTAs/SM) is
+    // another 1-2 % faster (44.2 / 44.6 at 2048^3 / 4096^3); the crossover measured on isolated launches lies near
+    // K = 1200, inside the solve (4 stream groups) K >= 768 is at least as good (profiles/r01_gemm_variants.md)
+    if (variant == GV_3M) variant = (a.K >= 768) ? GV_3M_PF : GV_3M_LEAN;
+    if (variant == GV_3M_PF) return gemm3m_epi<C3_64x32pf>(a, batch, epi, st);
+    return gemm3m_epi<C3_64x32s4>(a, batch, epi, st);
 }
 
 }  // namespace ss

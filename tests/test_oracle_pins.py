@@ -334,6 +334,8 @@ def test_golden_impurity_chain_table():
 
 
 def test_golden_config0_is_reproducible():
+    """Regression guard only (the file was written by dense.solve_all itself, so this pins nothing: the pins of dense.py
+    are the brute-force, closed-form and invariant tests above)."""
     tab = _golden("c0_transmission.txt")
     p = inputs.make_problem(inputs.CONFIGS["C0"])
     X, T = dense.solve_all(p)
@@ -399,3 +401,82 @@ def test_bond_current_conservation_closed_form_and_brute_force():
                     acc += np.conj(X[i * bs + a, c]) * (E * Su[i, a, b] - Hu[i, a, b]) * X[(i + 1) * bs + b, c]
         want[i] = 2.0 * acc.imag
     assert np.allclose(observables.bond_current(E, Hu, Su, X), want, rtol=1e-13, atol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------------------
+# the error metrics every parity assert rests on (north_star tolerances; reading c18): hand-computed values
+# ------------------------------------------------------------------------------------------------------
+def test_rel_frobenius_hand_computed():
+    """||X - R||_F / ||R||_F on 2x2 data worked out by hand: X - R = [[3, 0], [0, 4i]] -> 5; ||R||_F = sqrt(1+4+4+16) = 5."""
+    R = np.array([[1.0, 2.0j], [-2.0, 4.0]])
+    X = R + np.array([[3.0, 0.0], [0.0, 4.0j]])
+    assert residual.rel_frobenius(X, R) == pytest.approx(1.0, rel=1e-15)
+    assert residual.rel_frobenius(R, R) == 0.0
+    # not symmetric in its arguments (a swapped-argument mistake changes the value): ||X||_F = sqrt(16+4+4+32) != 5
+    assert residual.rel_frobenius(R, X) == pytest.approx(5.0 / np.sqrt(56.0), rel=1e-15)
+    # reference of norm zero: the absolute error is returned
+    assert residual.rel_frobenius(np.array([[3.0, 4.0]]), np.zeros((1, 2))) == pytest.approx(5.0)
+    # a sign error (X + R instead of X - R) would give 2 here
+    assert residual.rel_frobenius(-R, R) == pytest.approx(2.0, rel=1e-15)
+
+
+def test_rel_T_hand_computed():
+    assert residual.rel_T(64.0 + 6.4e-8, 64.0) == pytest.approx(1e-9, rel=1e-6)
+    assert residual.rel_T(0.5, 2.0) == pytest.approx(0.75)            # relative to the REFERENCE (second argument)
+    assert residual.rel_T(2.0, 0.5) == pytest.approx(3.0)
+    assert residual.rel_T(-1.0, 1.0) == pytest.approx(2.0)            # sign errors are not forgiven
+    assert residual.rel_T(3.0, 3.0) == 0.0
+    assert residual.rel_T(1e-301, 0.0) == pytest.approx(0.1)           # the 1e-300 floor of reading c18
+
+
+def test_inverse_column_residual_sees_a_wrong_Q():
+    """A [Q|P] = [e_1|e_nb].  The exact columns give ~u; a perturbation dQ of relative size eps
+    must show up as ||A dQ||_F / (||A||_F ||[Q|P]||_F), of order eps (computed here independently with the dense A);
+    wrong structure (P and Q exchanged, one block shifted) gives O(1)."""
+    p = tiny(4, 5)
+    E = p.E[0]
+    Q, P = dense.inverse_columns(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    A = dense.assemble_A(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    a = (E, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    assert residual.inverse_column_residual(*a, Q, P) < 1e-14
+    for eps in (1e-3, 1e-8):
+        dQ = eps * inputs.complex_gaussian(1, 98, 0, Q.shape, 1.0)
+        QP = np.concatenate([(Q + dQ).reshape(20, 4), P.reshape(20, 4)], axis=1)
+        rhs = np.zeros((20, 8), dtype=np.complex128)
+        rhs[:4, :4] = np.eye(4)
+        rhs[-4:, 4:] = np.eye(4)
+        want = np.linalg.norm(A @ QP - rhs) / (np.linalg.norm(A) * np.linalg.norm(QP))
+        got = residual.inverse_column_residual(*a, Q + dQ, P)
+        assert got == pytest.approx(want, rel=1e-6) and 0.05 * eps < got < 50 * eps
+    assert residual.inverse_column_residual(*a, P, Q) > 0.01
+    assert residual.inverse_column_residual(*a, np.roll(Q, 1, axis=0), P) > 0.01
+
+
+def test_backward_error_sees_a_wrong_X_at_the_size_of_the_perturbation():
+    """Tier C is the certificate at C3/C4: a relative perturbation eps of X must give a backward error of order eps
+    (value checked against the dense definition in test_residual_matches_dense_residual), a dropped Sigma an O(1) one."""
+    p = tiny(6, 5, inj_last=True)
+    r = dense.solve_energy(*args(p, 0))
+    for eps in (1e-4, 1e-9, 1e-12):
+        X = r["X"] * (1.0 + eps)
+        got = residual.backward_error(*args(p, 0), X)
+        assert 0.01 * eps < got < eps * 1.0001
+    a = list(args(p, 0))
+    a[5] = np.zeros_like(a[5])                                          # forget Sigma_L
+    assert residual.backward_error(*a, r["X"]) > 1e-3
+
+
+def test_banded_column_solve_is_the_banded_solve():
+    """solve_energy_columns / solve_factored (the large-size form used for the C3/C4 fingerprints) against dense.py:
+    selected columns of X, the whole last block column of T^-1, T_LR; chunking and threading change nothing."""
+    p = tiny(9, 6, nrhs=11)
+    for e in range(p.n_energy):
+        rd = dense.solve_energy(*args(p, e))
+        cols = [0, 3, 10]
+        r1 = banded.solve_energy_columns(*args(p, e), x_cols=cols, chunk=0)
+        r2 = banded.solve_energy_columns(*args(p, e), x_cols=cols, chunk=4, threads=3)
+        assert np.array_equal(r1["X_cols"], r2["X_cols"]) and np.array_equal(r1["G_last"], r2["G_last"])
+        assert residual.rel_frobenius(r1["X_cols"], rd["X"][:, cols]) < 1e-11
+        assert residual.rel_T(r1["T_LR"], rd["T_LR"]) < 1e-10
+        T = dense.assemble_T(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e])
+        assert np.allclose(r1["G_last"], np.linalg.inv(T)[:, -9:], rtol=1e-9, atol=1e-12)
