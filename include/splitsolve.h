@@ -148,9 +148,7 @@ ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long*
 
 /* Options: "nb_lu" (outer LU block, 16..128, multiple of 16; default 128), "transmission" (0/1, default 1:
  * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0), "gemm_variant" (see ss_set_default_gemm_variant;
- * default = the process-wide default at ss_create), "cuda_graph" (0/1, default 0: when 1, the second solve with the
- * same buffers, sizes and options captures the whole launch sequence, all group streams included, into a CUDA graph that
- * later identical solves replay; measured 2-4 % slower than direct launches on configs C2 and C3, hence off), "trace" (0/1, default 0: record a CUDA-event
+ * default = the process-wide default at ss_create), "trace" (0/1, default 0: record a CUDA-event
  * timeline of every group's high-/low-priority phases, see ss_trace_write), "stream_groups" (1..16,
  * default 4: the energy points are split
  * over that many groups, each with a high-priority stream for the latency-bound panel kernels and a low-priority
@@ -196,13 +194,12 @@ ss_status_t ss_density(const ss_cplx* X_dev, int n_energy, long long n, int nrhs
  * returned by that solve (nrhs <= its nrhs), J_host out [n_energy][nb-1].  Overwrites handle scratch; synchronises. */
 ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X_dev, int nrhs, double* J_host);
 
-/* Arithmetic / tile shape of the complex GEMM kernel (north_star: "4M or 3M ... whichever reaches the higher fraction
- * of the chip's FP64 peak"):  0 = 4M (four real products per complex product, 64x64 tile);  1..9 = 3M (three real
- * products, P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi); 6 instead of 8 real flops per complex multiply-add; rounding
- * differs, normwise error stays O(u)) with CTA tiles: 1 = 64x32 (3 CTAs/SM for K < 768, software-pipelined main loop at 2 CTAs/SM
- * from K = 768) = the default, 2 = 64x32 (3-stage), 3 = 64x64, 4 = 64x96, 5 = 128x48, 6 = 64x48, 7 = 96x32, 8 / 9 = the two
- * 64x32 kernels of the default for every shape.  The process-wide default
- * (initially 1) applies to handles created afterwards and to the handle-less building blocks above. */
+/* Arithmetic of the complex GEMM kernel (north_star: "4M or 3M ... whichever reaches the higher fraction of the chip's
+ * FP64 peak"):  0 = 4M (four real products per complex product, 64x64 tile);  1 = 3M, the default (three real products,
+ * P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi); 6 instead of 8 real flops per complex multiply-add; rounding differs,
+ * normwise error stays O(u)), 64x32 CTA tile, kernel chosen by K (3 CTAs/SM for K < 768, software-pipelined main loop at
+ * 2 CTAs/SM from K = 768);  2 / 3 = those two 3M kernels for every K.  The process-wide default (initially 1) applies to
+ * handles created afterwards and to the handle-less building blocks above. */
 ss_status_t ss_set_default_gemm_variant(int variant);
 int ss_get_default_gemm_variant(void);
 

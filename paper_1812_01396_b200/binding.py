@@ -271,8 +271,8 @@ def density(X, w=None):
     return rho
 
 
-GEMM_VARIANTS = {0: "4M 64x64", 1: "3M auto (64x32: 3 CTAs/SM for K<768, prefetching 2 CTAs/SM above)", 2: "3M 64x32 s3", 3: "3M 64x64", 4: "3M 64x96",
-                 5: "3M 128x48", 6: "3M 64x48", 7: "3M 96x32", 8: "3M 64x32 s4", 9: "3M 64x32 pf"}
+GEMM_VARIANTS = {0: "4M 64x64", 1: "3M 64x32 (3 CTAs/SM for K<768, software-pipelined 2 CTAs/SM above)",
+                 2: "3M 64x32 lean, every K", 3: "3M 64x32 software-pipelined, every K"}
 
 
 def set_default_gemm_variant(variant: int):
