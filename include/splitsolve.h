@@ -146,7 +146,7 @@ ss_status_t ss_trace_write(ss_handle_t h, const char* path);
  * algorithmic flops (8 M N K per complex GEMM) and their number.  Synchronises. */
 ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long* launches);
 
-/* Options: "nb_lu" (outer LU block, 16..128, multiple of 16; default 128), "transmission" (0/1, default 1:
+/* Options: "transmission" (0/1, default 1:
  * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0), "gemm_variant" (see ss_set_default_gemm_variant;
  * default = the process-wide default at ss_create), "trace" (0/1, default 0: record a CUDA-event
  * timeline of every group's high-/low-priority phases, see ss_trace_write), "stream_groups" (1..16,
@@ -167,18 +167,25 @@ ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const ss_cplx* A
                              const ss_cplx* B_dev, int ldb, long long strideB, double beta, ss_cplx* C_dev, int ldc,
                              long long strideC, int batch, void* cuda_stream);
 
-/* Batched blocked right-looking LU with partial pivoting (ZGETRF) of the leading n x n part of the
- * n x ncols (ncols >= n, ld) row-major matrices AB[z]; the row interchanges and the L-solve are applied to
- * the trailing ncols - n columns too (so that AB[:, n:] becomes L^-1 P B).  ipiv_dev: [batch][n] 0-based
- * row indices (LAPACK semantics: row j was swapped with row ipiv[j]); info_dev: [batch], 0 or 1 + index of
- * the first zero pivot.  n <= 8192. */
+/* Batched blocked LU with partial pivoting (ZGETRF) of the leading n x n part of the n x ncols (ncols >= n, ld)
+ * row-major matrices AB[z]; the row interchanges and the L-solve are applied to the trailing ncols - n columns too (so
+ * that AB[:, n:] becomes L^-1 P B).  Recursive over column ranges down to 128-column panels (leaf panels of 16 columns
+ * factored by a thread-block-cluster kernel: warp-shuffle / redux pivot search, rows in registers), every update a DMMA
+ * GEMM.  ipiv_dev: [batch][n] 0-based row indices (LAPACK semantics: row j was swapped with row ipiv[j]); info_dev:
+ * [batch], 0 or 1 + index of the first zero pivot.  n <= 8192.
+ * work_dev: caller-owned device scratch of at least ss_lu_workspace_bytes(n, batch) bytes (the inverses of the 128 x 128
+ * diagonal blocks of L and U); its contents are needed by nothing after the call's work has completed.
+ * Asynchronous: everything is enqueued on cuda_stream, nothing is allocated, the host does not wait. */
+size_t ss_lu_workspace_bytes(int n, int batch);
 ss_status_t ss_zgetrf_batched(int n, int ncols, ss_cplx* AB_dev, int ld, long long stride, int* ipiv_dev,
-                              int* info_dev, int batch, void* cuda_stream);
+                              int* info_dev, int batch, void* work_dev, size_t work_bytes, void* cuda_stream);
 
 /* Batched solve A X = B (ZGESV): LU as above on AB = [A | B] (n x (n + nrhs), ld), then blocked ZTRSM back
- * substitution with the upper factor; X[z] (n x nrhs, ldx) at X_dev + z*strideX.  AB is overwritten. */
+ * substitution with the upper factor (left-looking over 128-row blocks, explicit block inverses: GEMMs); X[z]
+ * (n x nrhs, ldx) at X_dev + z*strideX.  AB is overwritten.  Workspace and asynchrony as for ss_zgetrf_batched. */
 ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB_dev, int ld, long long stride, ss_cplx* X_dev, int ldx,
-                             long long strideX, int* ipiv_dev, int* info_dev, int batch, void* cuda_stream);
+                             long long strideX, int* ipiv_dev, int* info_dev, int batch, void* work_dev, size_t work_bytes,
+                             void* cuda_stream);
 
 /* Carrier density from the solution ("charge and current densities can be directly
  * derived from ... c(E)"):  rho[i] = sum_e w[e] * sum_c |X[e][i][c]|^2,  i = 0..n-1.

@@ -39,9 +39,11 @@ SIGNATURES = {
     "ss_strerror": (c_char_p, [c_int]),
     "ss_zgemm_batched": (c_int, [c_int, c_int, c_int, c_double, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong,
                                  c_double, c_void_p, c_int, c_longlong, c_int, c_void_p]),
-    "ss_zgetrf_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_void_p, c_int, c_void_p]),
+    "ss_lu_workspace_bytes": (c_size_t, [c_int, c_int]),
+    "ss_zgetrf_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_void_p, c_int, c_void_p, c_size_t,
+                                  c_void_p]),
     "ss_zgesv_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong, c_void_p,
-                                 c_void_p, c_int, c_void_p]),
+                                 c_void_p, c_int, c_void_p, c_size_t, c_void_p]),
     "ss_fp64_peak_tflops": (c_int, [c_double, POINTER(c_double)]),
     "ss_density": (c_int, [c_void_p, c_int, c_longlong, c_int, c_void_p, c_void_p, c_void_p]),
     "ss_bond_current": (c_int, [c_void_p, c_void_p, c_int, c_void_p]),
@@ -234,6 +236,12 @@ def zgemm_batched(A, B, C, alpha=1.0, beta=0.0):
     return C
 
 
+def _lu_work(n, batch, device):
+    """Caller-owned scratch of ss_zgetrf_batched / ss_zgesv_batched (torch keeps it alive until the stream has used it)."""
+    import torch
+    return torch.empty(int(load().ss_lu_workspace_bytes(n, batch)), dtype=torch.uint8, device=device)
+
+
 def zgetrf_batched(AB, n):
     """In-place LU of the leading n x n part of AB [batch, n, ncols]; returns (ipiv, info) int32 CUDA tensors."""
     import torch
@@ -241,8 +249,9 @@ def zgetrf_batched(AB, n):
     assert rows == n
     ipiv = torch.zeros((batch, n), dtype=torch.int32, device=AB.device)
     info = torch.zeros((batch,), dtype=torch.int32, device=AB.device)
+    work = _lu_work(n, batch, AB.device)
     _check(load().ss_zgetrf_batched(n, ncols, _dev(AB, "AB"), ncols, n * ncols, ipiv.data_ptr(), info.data_ptr(), batch,
-                                    _stream()), "ss_zgetrf_batched")
+                                    work.data_ptr(), work.numel(), _stream()), "ss_zgetrf_batched")
     return ipiv, info
 
 
@@ -254,8 +263,10 @@ def zgesv_batched(AB, n):
     X = torch.empty((batch, n, nrhs), dtype=torch.complex128, device=AB.device)
     ipiv = torch.zeros((batch, n), dtype=torch.int32, device=AB.device)
     info = torch.zeros((batch,), dtype=torch.int32, device=AB.device)
+    work = _lu_work(n, batch, AB.device)
     _check(load().ss_zgesv_batched(n, nrhs, _dev(AB, "AB"), ncols, n * ncols, _dev(X, "X"), nrhs, n * nrhs,
-                                   ipiv.data_ptr(), info.data_ptr(), batch, _stream()), "ss_zgesv_batched")
+                                   ipiv.data_ptr(), info.data_ptr(), batch, work.data_ptr(), work.numel(), _stream()),
+           "ss_zgesv_batched")
     return X, ipiv, info
 
 

@@ -20,7 +20,6 @@ struct ss_handle_s {
     bool have_h = false, solved = false;
     bool launched = false;           // some ss_solve has been enqueued: ev[2] is a valid event to wait on
     // options
-    int nb_lu = 128;
     int want_T = 1;
     int profile_gemm = 0;
     int gemm_variant = g_default_variant;
@@ -47,7 +46,6 @@ struct ss_handle_s {
     cplx *gam_l = nullptr, *gam_r = nullptr, *g1n = nullptr, *w1 = nullptr, *w2 = nullptr, *E_dev = nullptr;
     double *tpart = nullptr, *T_dev = nullptr;
     int *ipiv = nullptr, *info = nullptr;
-    int tinv_blocks_total = 0;
     cplx* E_pinned = nullptr;
     // host-path buffers
     cplx *hp_sigl = nullptr, *hp_sigr = nullptr, *hp_inj1 = nullptr, *hp_inj2 = nullptr, *hp_x = nullptr;
@@ -83,7 +81,6 @@ static void free_workspace(ss_handle_t h) {
 
 struct WsSizes {
     size_t slots, aug, aop, tinv, raug, wz, sq, E, tpart, T, ipiv, info;
-    int tinv_blocks;
     size_t total() const { return slots + aug + aop + tinv + raug + wz + 5 * sq + E + tpart + T + ipiv + info; }
 };
 
@@ -95,9 +92,7 @@ static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
     w.aop = (size_t)nE * 2 * B2 * C;
     // the sweep and the corner system own disjoint regions: stream groups do not wait for one another between the two
     // phases, so one group's corner LU may run while another group's sweep still uses its triangular inverses
-    int blk_sweep = 2 * nE * (int)cdiv(bs, 128), blk_corner = nE * (int)cdiv(2 * bs, 128);
-    w.tinv_blocks = blk_sweep + blk_corner;
-    w.tinv = (size_t)w.tinv_blocks * 128 * 128 * C;
+    w.tinv = (lu_tinv_elems(bs, 2 * nE) + lu_tinv_elems(2 * bs, nE)) * C;
     size_t W = (size_t)pad_ld(3LL * bs + nrhs), W2 = (size_t)pad_ld(2LL * bs + nrhs);   // with / without the e_2 columns
     if (W2 > W) W = W2;
     w.raug = (size_t)nE * 2 * bs * W * C;
@@ -123,7 +118,6 @@ static ss_status_t ensure_workspace(ss_handle_t h, int nrhs) {
     A((void**)&h->w2, w.sq); A((void**)&h->E_dev, w.E); A((void**)&h->tpart, w.tpart); A((void**)&h->T_dev, w.T);
     A((void**)&h->ipiv, w.ipiv); A((void**)&h->info, w.info);
     if (!ok) { cudaGetLastError(); free_workspace(h); return SS_ERR_ALLOC; }
-    h->tinv_blocks_total = w.tinv_blocks;
     h->ws_nrhs = nrhs;
     return SS_OK;
 }
@@ -250,10 +244,6 @@ extern "C" ss_status_t ss_set_hamiltonian_host(ss_handle_t h, const ss_cplx* Hd,
 
 extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value) {
     if (!h || !name) return SS_ERR_INVALID_ARG;
-    if (!strcmp(name, "nb_lu")) {
-        if (value < 16 || value > 128 || value % 16) return SS_ERR_INVALID_ARG;
-        h->nb_lu = value; return SS_OK;
-    }
     if (!strcmp(name, "transmission")) { h->want_T = value ? 1 : 0; return SS_OK; }
     if (!strcmp(name, "profile_gemm")) { h->profile_gemm = value ? 1 : 0; return SS_OK; }
     if (!strcmp(name, "stream_groups")) {
@@ -261,6 +251,7 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         h->stream_groups = value; return SS_OK;
     }
     if (!strcmp(name, "trace")) { h->want_trace = value ? 1 : 0; return SS_OK; }
+    if (!strcmp(name, "panel_fused")) { g_panel_fused = value ? 1 : 0; return SS_OK; }      // process-wide (tuning)
     if (!strcmp(name, "gemm_variant")) {
         if (value < 0 || value >= GV_COUNT) return SS_ERR_INVALID_ARG;
         h->gemm_variant = value; return SS_OK;
@@ -316,9 +307,8 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
     const BPtr aug = bp_chain(h->aug + e0 * s_aug_e, h->aug + e0 * s_aug_e + (long long)bs * ldg, s_aug_e);
     const BPtr aop = bp_chain(h->aop + e0 * 2 * B2, h->aop + e0 * 2 * B2 + B2, 2 * B2);
     const cplx* E = h->E_dev + e0;
-    const int blk_chain = (int)cdiv(bs, 128);
     LuWork w;
-    w.tinv = h->tinv + (long long)2 * e0 * blk_chain * 128 * 128; w.tinv_blocks = batch * blk_chain;
+    w.tinv = h->tinv + lu_tinv_elems(bs, 2 * e0);
     w.ipiv = h->ipiv + (long long)2 * e0 * 2 * bs; w.ipiv_stride = 2 * bs; w.info = h->info + 2 * e0;
     const int info_stride = 2 * bs + 2;
 
@@ -350,7 +340,7 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
     g.lds = bs; g.E = E;
     gemm_run(ctx, g, batch, GEMM_BIG, EPI_SCHUR);
     // a2 + the L half of a3
-    lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, h->nb_lu, w, s * info_stride);
+    lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, w, s * info_stride);
     // U half of a3: X_i / Y_i into its slot
     BPtr out = bp_chain(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
     back_substitute(ctx, aug, ldg, bs, bs, out, bs, batch, w);
@@ -408,13 +398,11 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
                                   bp_strided(raug + (long long)br * bs * ldW + (long long)bc * bs, s_r), ldW);
             gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         }
-    const int blk_corner = (int)cdiv(2 * bs, 128);
     LuWork w;
-    const long long blk_sweep_total = 2LL * h->n_energy * cdiv(bs, 128);
-    w.tinv = h->tinv + (blk_sweep_total + (long long)e0 * blk_corner) * 128 * 128; w.tinv_blocks = nE * blk_corner;
+    w.tinv = h->tinv + lu_tinv_elems(bs, 2 * h->n_energy) + lu_tinv_elems(2 * bs, e0);
     w.ipiv = h->ipiv + (long long)2 * h->n_energy * 2 * bs + (long long)e0 * 2 * bs; w.ipiv_stride = 2 * bs;
     w.info = h->info + 2 * h->n_energy + e0;
-    lu_factor(ctx, bp_strided(raug, s_r), ldW, 2 * bs, W, nE, h->nb_lu, w, 0);
+    lu_factor(ctx, bp_strided(raug, s_r), ldW, 2 * bs, W, nE, w, 0);
     back_substitute(ctx, bp_strided(raug, s_r), ldW, 2 * bs, nr, bp_strided(wz, s_w), nr, nE, w);
     // a6: X_i = Q_i w_top + P_i w_bot, batch z = e*nb + (i-1)
     if (m > 0) {
@@ -767,37 +755,38 @@ extern "C" ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const
     return SS_OK;
 }
 
+extern "C" size_t ss_lu_workspace_bytes(int n, int batch) {
+    if (n < 1 || batch < 1) return 0;
+    return lu_tinv_elems(n, batch) * sizeof(cplx);
+}
+
 static ss_status_t lu_common(int n, int nrhs_solve, int ncols, ss_cplx* AB, int ld, long long stride, ss_cplx* X, int ldx,
-                             long long sX, int* ipiv, int* info, int batch, void* stream) {
-    if (n < 1 || n > LEAF_TPB * LEAF_MAXC || ncols < n || ld < ncols || batch < 1 || !AB || !ipiv || !info)
+                             long long sX, int* ipiv, int* info, int batch, void* work, size_t work_bytes, void* stream) {
+    if (n < 1 || n > LEAF_TPB * LEAF_MAXC || ncols < n || ld < ncols || batch < 1 || !AB || !ipiv || !info || !work)
         return SS_ERR_INVALID_ARG;
+    if (work_bytes < ss_lu_workspace_bytes(n, batch)) return SS_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     LuWork w;
-    const int nblk = (int)cdiv(n, 128);
-    if (cudaMalloc((void**)&w.tinv, sizeof(cplx) * 128 * 128 * (size_t)nblk * batch) != cudaSuccess) {
-        cudaGetLastError(); return SS_ERR_ALLOC;
-    }
-    w.tinv_blocks = nblk * batch; w.ipiv = ipiv; w.ipiv_stride = n; w.info = info;
+    w.tinv = (cplx*)work; w.ipiv = ipiv; w.ipiv_stride = n; w.info = info;
     Ctx ctx; ctx.st = st; ctx.variant = g_default_variant;
     cudaMemsetAsync(info, 0, sizeof(int) * (size_t)batch, st);
     BPtr Ab = bp_strided((cplx*)AB, stride);
-    lu_factor(ctx, Ab, ld, n, ncols, batch, 128, w, 0);
+    lu_factor(ctx, Ab, ld, n, ncols, batch, w, 0);
     if (nrhs_solve > 0) back_substitute(ctx, Ab, ld, n, nrhs_solve, bp_strided((cplx*)X, sX), ldx, batch, w);
-    cudaError_t e = cudaStreamSynchronize(st);
-    cudaFree(w.tinv);
-    if (e != cudaSuccess || ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }
 
 extern "C" ss_status_t ss_zgetrf_batched(int n, int ncols, ss_cplx* AB, int ld, long long stride, int* ipiv, int* info,
-                                         int batch, void* stream) {
-    return lu_common(n, 0, ncols, AB, ld, stride, nullptr, 0, 0, ipiv, info, batch, stream);
+                                         int batch, void* work, size_t work_bytes, void* stream) {
+    return lu_common(n, 0, ncols, AB, ld, stride, nullptr, 0, 0, ipiv, info, batch, work, work_bytes, stream);
 }
 
 extern "C" ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB, int ld, long long stride, ss_cplx* X, int ldx,
-                                        long long sX, int* ipiv, int* info, int batch, void* stream) {
+                                        long long sX, int* ipiv, int* info, int batch, void* work, size_t work_bytes,
+                                        void* stream) {
     if (nrhs < 0 || (nrhs > 0 && (!X || ldx < nrhs))) return SS_ERR_INVALID_ARG;
-    return lu_common(n, nrhs, n + nrhs, AB, ld, stride, X, ldx, sX, ipiv, info, batch, stream);
+    return lu_common(n, nrhs, n + nrhs, AB, ld, stride, X, ldx, sX, ipiv, info, batch, work, work_bytes, stream);
 }
 
 extern "C" ss_status_t ss_density(const ss_cplx* X, int n_energy, long long n, int nrhs, const double* w, double* rho,

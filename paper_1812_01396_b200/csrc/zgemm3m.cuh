@@ -139,23 +139,43 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
 
     // ---- staging of the software-pipelined build (PF = 1): descriptors kept per chunk, address and predicate formed per
     // stage.  Measured, that kernel is faster with this form (44.2 vs 43.6 TFLOP/s at 2048^3 x 16) and the plain loop with
-    // the running pointers above (43.6 vs 42.0); `if constexpr` keeps exactly one of the two in each instantiation.
+    // the running pointers above (43.6 vs 42.0); only the state of the form an instantiation uses survives in it.
+    const cplx* a_src[Cfg::ITER_A]; int a_dst[Cfg::ITER_A]; int a_kc[Cfg::ITER_A]; bool a_ok[Cfg::ITER_A];
+    const cplx* b_src[Cfg::ITER_B]; int b_dst[Cfg::ITER_B]; int b_kr[Cfg::ITER_B]; bool b_ok[Cfg::ITER_B];
+    if constexpr (!LEAN) {
+#pragma unroll
+        for (int q = 0; q < Cfg::ITER_A; q++) {
+            int c = tid + q * NT;
+            int row = c / KC, kc = c % KC;
+            a_kc[q] = (c < Cfg::CH_A) ? kc : (1 << 28);          // beyond the tile: never in range
+            a_ok[q] = (c < Cfg::CH_A) && (m0 + row) < M;
+            a_src[q] = Ag + (long long)(a_ok[q] ? (m0 + row) : 0) * p.lda + kc;
+            a_dst[q] = (c < Cfg::CH_A) ? row * LDA_S + 2 * kc : -1;
+        }
+#pragma unroll
+        for (int q = 0; q < Cfg::ITER_B; q++) {
+            int c = tid + q * NT;
+            int kr = c / BN, col = c % BN;
+            b_kr[q] = (c < Cfg::CH_B) ? kr : (1 << 28);
+            b_ok[q] = (c < Cfg::CH_B) && (n0 + col) < N;
+            b_src[q] = Bg + (long long)kr * p.ldb + (b_ok[q] ? (n0 + col) : 0);
+            b_dst[q] = (c < Cfg::CH_B) ? BM * LDA_S + kr * LDB_S + 2 * col : -1;
+        }
+    }
     auto load_stage_desc = [&](int kt, int stage) {
         double* sbase = smem + stage * STAGE_D;
         const int k0 = kt * KC;
 #pragma unroll
         for (int q = 0; q < Cfg::ITER_A; q++) {
-            if (a_sz[q] < 0) continue;
-            const int kc = (tid + q * NT) % KC;
-            bool ok = a_sz[q] > 0 && (k0 + kc < K);
-            cp_async16(sbase + (a_sd[q] - smem_u32) / 8, ok ? (const void*)(a_p[q] + k0) : (const void*)Ag, ok ? 16 : 0);
+            if (a_dst[q] < 0) continue;
+            bool ok = a_ok[q] && (k0 + a_kc[q] < K);
+            cp_async16(sbase + a_dst[q], ok ? (const void*)(a_src[q] + k0) : (const void*)Ag, ok ? 16 : 0);
         }
 #pragma unroll
         for (int q = 0; q < Cfg::ITER_B; q++) {
-            if (b_sz[q] < 0) continue;
-            const int kr = (tid + q * NT) / BN;
-            bool ok = b_sz[q] > 0 && (k0 + kr < K);
-            cp_async16(sbase + (b_sd[q] - smem_u32) / 8, ok ? (const void*)(b_p[q] + (long long)k0 * p.ldb) : (const void*)Bg, ok ? 16 : 0);
+            if (b_dst[q] < 0) continue;
+            bool ok = b_ok[q] && (k0 + b_kr[q] < K);
+            cp_async16(sbase + b_dst[q], ok ? (const void*)(b_src[q] + (long long)k0 * p.ldb) : (const void*)Bg, ok ? 16 : 0);
         }
     };
 

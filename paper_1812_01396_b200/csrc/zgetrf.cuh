@@ -294,17 +294,182 @@ lu_leaf3_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restr
     }
 }
 
-// Apply the row interchanges ipiv[row0 .. row0+jb) to columns [0, skip_lo) U [skip_hi, ncols) of each matrix.
+// ---- the whole 128-column panel in ONE launch (panels of up to 4096 rows): the thread-block cluster stays resident over
+// the 8 inner blocks of 16 columns instead of being re-scheduled for every one of them (4 launches per inner block before:
+// leaf, row swaps, 16-row triangular solve, rank-16 update).  One thread = one matrix row for the whole panel; pivoting is
+// IMPLICIT for the whole panel (no row moves until the end), with the same position bookkeeping as the leaf kernel.
+// Per inner block:  (1) the 16 active columns of the own row -> registers;  (2) 16 pivot steps exactly as in
+// lu_leaf3_kernel (redux arg-max, key exchange through distributed shared memory, one cluster barrier, winner row pulled);
+// every CTA keeps the 16 pivot rows' active entries (L11 \ U11) and their physical row numbers;  (3) the pivot rows'
+// remaining panel columns are read by every CTA, U12 = L11^-1 A12 is solved redundantly in shared memory (one thread per
+// column), the owners write it back;  (4) rank-16 update of the own row's remaining panel columns with the multipliers
+// still in registers.  At the end the rows that moved (at most 2 x 128) are carried to their final positions, 16 columns at
+// a time through registers with a cluster barrier between the reads and the writes of a chunk.
+constexpr int PANEL_W = 128;
+
+__global__ void __launch_bounds__(LEAF2_TPB, 2)
+lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv, int ipiv_stride,
+                int* __restrict__ info, int info_base) {
+    cg::cluster_group cluster = cg::this_cluster();
+    const int csize = (int)cluster.num_blocks();
+    const int crank = (int)cluster.block_rank();
+    const int z = blockIdx.y;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = LEAF2_TPB / 32, JB = LEAF_JB;
+
+    __shared__ __align__(16) LeafCand wcand[2][NW];
+    __shared__ __align__(16) LeafKey keys[2][LEAF2_MAXC];
+    __shared__ __align__(16) cplx prow[JB];
+    __shared__ __align__(16) cplx Lpiv[JB][JB];          // row k: the k-th pivot row's active entries (multipliers | U)
+    __shared__ int piv_phys[JB];                          // its physical row inside the panel
+    __shared__ __align__(16) cplx U12[JB][PANEL_W - JB];
+
+    cplx* A = bptr(Ab, z) + (long long)j0 * ld + j0;      // no __restrict__/const: other CTAs write rows this CTA reads
+    const int r = crank * LEAF2_TPB + tid;                // my (physical) row inside the panel
+    const bool valid = r < m;
+    cplx* Arow = A + (long long)r * ld;
+    int cur_pos = r;
+    bool done = !valid;
+    int final_pos = r;
+
+    for (int c = 0; c < nbw; c += JB) {
+        const int jb = min(JB, nbw - c), wrest = nbw - c - jb;
+        cplx a[JB];
+#pragma unroll
+        for (int k = 0; k < JB; k++) a[k] = (valid && k < jb) ? Arow[c + k] : make_c(0.0, 0.0);
+#pragma unroll
+        for (int j = 0; j < JB; j++) {
+            if (j < jb) {
+                const int q = c + j;                      // pivot step = position inside the panel
+                const int par = j & 1;
+                double wv; int wp;
+                const double myv = done ? -1.0 : (fabs(a[j].re) + fabs(a[j].im));
+                if (warp_argmax(myv, cur_pos, wv, wp)) {
+                    LeafCand* cd = &wcand[par][warp];
+                    cd->val = myv; cd->pos = cur_pos; cd->pad = r;
+#pragma unroll
+                    for (int k = 0; k < JB; k++) cd->row[k] = a[k];
+                }
+                if (lane == 0 && wv < 0.0) { wcand[par][warp].val = -1.0; wcand[par][warp].pos = 0x7fffffff; wcand[par][warp].pad = 0; }
+                __syncthreads();
+                if (warp == 0) {
+                    double v2 = lane < NW ? wcand[par][lane].val : -1.0;
+                    int p2 = lane < NW ? wcand[par][lane].pos : 0x7fffffff;
+                    double cv; int cp;
+                    bool win = warp_argmax(v2, p2, cv, cp);
+                    unsigned bal = __ballot_sync(0xffffffffu, win);
+                    LeafKey k; k.val = cv; k.pos = cp; k.warp = bal ? (__ffs(bal) - 1) : 0;
+                    if (lane < csize) *cluster.map_shared_rank(&keys[par][crank], lane) = k;
+                }
+                cluster.sync();
+                double kv = -1.0; int kp = 0x7fffffff, kw = 0;
+                if (lane < csize) { LeafKey k = keys[par][lane]; kv = k.val; kp = k.pos; kw = k.warp; }
+                double gv; int gp;
+                bool gwin = warp_argmax(kv, kp, gv, gp);
+                unsigned gbal = __ballot_sync(0xffffffffu, gwin);
+                const int wcta = gbal ? (__ffs(gbal) - 1) : 0;
+                const int wslot = __shfl_sync(0xffffffffu, kw, wcta);
+                if (warp == 0 && lane < JB) {
+                    const LeafCand* src = cluster.map_shared_rank(&wcand[par][wslot], wcta);
+                    cplx v = (gv >= 0.0) ? src->row[lane] : make_c(0.0, 0.0);
+                    prow[lane] = v;
+                    Lpiv[j][lane] = v;
+                    if (lane == 0) piv_phys[j] = (gv >= 0.0) ? src->pad : 0;
+                }
+                if (gv < 0.0) { gp = q; }                 // no rows left: nothing to do
+                const bool singular = !(gv > 0.0);
+                if (crank == 0 && tid == 0) {
+                    ipiv[(long long)z * ipiv_stride + j0 + q] = j0 + gp;
+                    if (singular && gv >= 0.0) atomicCAS(&info[z], 0, info_base + j0 + q + 1);
+                }
+                __syncthreads();
+                if (!done) {
+                    if (cur_pos == gp && gv >= 0.0) {
+                        done = true; final_pos = q;       // I am the pivot row: becomes row q of the panel's U
+                    } else {
+                        if (cur_pos == q) cur_pos = gp;   // LAPACK swap bookkeeping
+                        if (!singular) {
+                            cplx rinv = crecip_fast(prow[j]);
+                            cplx l = cmul(a[j], rinv);
+                            a[j] = l;
+#pragma unroll
+                            for (int k = j + 1; k < JB; k++) a[k] = cfnma(a[k], l, prow[k]);
+                        }
+                    }
+                }
+            }
+        }
+        if (valid) {
+#pragma unroll
+            for (int k = 0; k < JB; k++)
+                if (k < jb) Arow[c + k] = a[k];
+        }
+        if (wrest > 0) {
+            const int cr = c + jb;                        // first remaining column
+            // A12: the pivot rows' remaining columns (every CTA reads all of them; .cg: written by their owner CTAs)
+            for (int idx = tid; idx < jb * wrest; idx += LEAF2_TPB) {
+                int k = idx / wrest, cc = idx - k * wrest;
+                const double2 v = __ldcg(reinterpret_cast<const double2*>(A + (long long)piv_phys[k] * ld + cr + cc));
+                U12[k][cc] = make_c(v.x, v.y);
+            }
+            cluster.sync();                               // all CTAs have read A12 before any owner overwrites it
+            if (tid < wrest) {                            // U12 = L11^-1 A12 in place, one thread per column
+                for (int k = 1; k < jb; k++) {
+                    cplx acc = U12[k][tid];
+                    for (int kk = 0; kk < k; kk++) acc = cfnma(acc, Lpiv[k][kk], U12[kk][tid]);
+                    U12[k][tid] = acc;
+                }
+            }
+            __syncthreads();
+            for (int idx = tid; idx < jb * wrest; idx += LEAF2_TPB) {
+                int k = idx / wrest, cc = idx - k * wrest;
+                int pr = piv_phys[k];
+                if (pr / LEAF2_TPB == crank) A[(long long)pr * ld + cr + cc] = U12[k][cc];
+            }
+            if (valid && !done) {                         // A22 -= L21 U12 on my row (multipliers a[0..jb) in registers)
+                for (int cc = 0; cc < wrest; cc++) {
+                    cplx x = Arow[cr + cc];
+#pragma unroll
+                    for (int k = 0; k < JB; k++)
+                        if (k < jb) x = cfnma(x, a[k], U12[k][cc]);
+                    Arow[cr + cc] = x;
+                }
+            }
+            __syncthreads();                              // U12 / Lpiv / piv_phys are rewritten by the next inner block
+        }
+    }
+    // ---- carry the moved rows to their final positions
+    if (!done) final_pos = cur_pos;
+    const bool moved = valid && final_pos != r;
+    cplx* Adst = A + (long long)final_pos * ld;
+    for (int c = 0; c < nbw; c += JB) {
+        cplx a[JB];
+        if (moved) {
+#pragma unroll
+            for (int k = 0; k < JB; k++)
+                if (c + k < nbw) a[k] = Arow[c + k];
+        }
+        cluster.sync();
+        if (moved) {
+#pragma unroll
+            for (int k = 0; k < JB; k++)
+                if (c + k < nbw) Adst[c + k] = a[k];
+        }
+    }
+    cluster.sync();                                       // no CTA may exit while another still reads its shared memory
+}
+
+// Apply the row interchanges ipiv[row0 .. row0+jb) to the columns [c_lo, skip_lo) U [skip_hi, c_hi) of each matrix.
 // One thread per column: consecutive threads touch consecutive elements of a row (coalesced in row-major).
 __global__ void __launch_bounds__(256)
-laswp_kernel(BPtr Ab, int ld, int ncols, int row0, int jb, int skip_lo, int skip_hi,
+laswp_kernel(BPtr Ab, int ld, int c_lo, int c_hi, int row0, int jb, int skip_lo, int skip_hi,
              const int* __restrict__ ipiv, int ipiv_stride) {
     const int z = blockIdx.y;
     int c = blockIdx.x * blockDim.x + threadIdx.x;
-    const int nleft = skip_lo;
-    const int total = nleft + (ncols - skip_hi);
+    const int nleft = skip_lo - c_lo;
+    const int total = nleft + (c_hi - skip_hi);
     if (c >= total) return;
-    if (c >= nleft) c = skip_hi + (c - nleft);
+    c = (c >= nleft) ? skip_hi + (c - nleft) : c_lo + c;
     cplx* __restrict__ A = bptr(Ab, z);
     const int* piv = ipiv + (long long)z * ipiv_stride + row0;
     for (int j = 0; j < jb; j++) {
@@ -551,12 +716,13 @@ static void gemm_run(Ctx& ctx, const GemmArgs& g, int batch, int cfg, int epi) {
 }
 
 struct LuWork {
-    cplx* tinv = nullptr;       // [batch][tinv_blocks][128*128] triangular-inverse scratch
-    int tinv_blocks = 0;
+    cplx* tinv = nullptr;       // [batch][2 * nblk(n)][128*128]: inverses of the 128 x 128 diagonal blocks of L, then of U
     int* ipiv = nullptr;        // [batch][ipiv_stride]
     int ipiv_stride = 0;
     int* info = nullptr;        // [batch]
 };
+static inline int lu_nblk(int n) { return (n + 127) / 128; }
+static inline size_t lu_tinv_elems(int n, int batch) { return (size_t)2 * lu_nblk(n) * 128 * 128 * (size_t)batch; }
 
 static inline GemmArgs gemm_std(int M, int N, int K, double alpha, BPtr A, int lda, BPtr B, int ldb, double beta,
                                 BPtr C, int ldc) {
@@ -599,56 +765,140 @@ static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, in
         ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
 }
 
-// LU with partial pivoting of the leading n x n part of the n x ncols matrices; interchanges and L-solve applied
-// to all ncols columns.  nb_lu: outer block (multiple of 16, <= 128).  n <= LEAF_TPB * LEAF_MAXC.
-static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, int nb_lu, const LuWork& w,
-                      int info_base) {
-    for (int j0 = 0; j0 < n; j0 += nb_lu) {
-        const int nbw = min(nb_lu, n - j0);
-        ctx.use(CLS_HI);
+// ---------------------------------------------------------------------------------------------------------
+// LU with partial pivoting of the leading n x n part of the n x ncols matrices (row-major, ld); the interchanges and the
+// L-solve are applied to the trailing ncols - n columns too.  n <= LEAF_TPB * LEAF_MAXC.
+//
+// Recursive over column ranges (Toledo's recursive LU down to 128-column panels), so that the O(n^3) work runs in GEMMs
+// with long K instead of rank-128 trailing updates:
+//     rlu([c0, c1)):  rlu(left half) -> swaps on the right half -> A12 = L11^-1 A12 -> A22 -= A21 A12 (K = width of the
+//     left half) -> rlu(right half) -> swaps on the left half.
+// Triangular solves are left-looking over 128-row blocks with explicit inverses of the 128 x 128 diagonal blocks
+// (trtri_kernel, one per panel), so they are GEMMs with K growing from 128 to the size of the triangle:
+//     X_k = L_kk^-1 (A_k - L_{k,<k} X_{<k}).
+// The right-hand-side columns [n, ncols) get all n interchanges at the end, then one left-looking L-solve.
+// ---------------------------------------------------------------------------------------------------------
+struct LuCall {
+    Ctx& ctx; BPtr Ab; int ld, n, ncols, batch; const LuWork& w; int info_base;
+    int nblk() const { return lu_nblk(n); }
+    BPtr tinvL(int blk) const { return bp_strided(w.tinv + (long long)blk * 128 * 128, 2LL * nblk() * 128 * 128); }
+    BPtr tinvU(int blk) const { return bp_strided(w.tinv + (long long)(nblk() + blk) * 128 * 128, 2LL * nblk() * 128 * 128); }
+};
+
+static void lu_swaps(const LuCall& L, int piv_lo, int piv_hi, int c_lo, int c_hi, int skip_lo, int skip_hi) {
+    const int total = (skip_lo - c_lo) + (c_hi - skip_hi);
+    if (total <= 0 || piv_hi <= piv_lo) return;
+    dim3 grid((unsigned)((total + 255) / 256), (unsigned)L.batch);
+    laswp_kernel<<<grid, 256, 0, L.ctx.st>>>(L.Ab, L.ld, c_lo, c_hi, piv_lo, piv_hi - piv_lo, skip_lo, skip_hi, L.w.ipiv, L.w.ipiv_stride);
+    L.ctx.note(cudaGetLastError());
+}
+
+static int g_panel_fused = 1;        // 1: lu_panel_kernel for panels of up to 4096 rows; 0: always the per-16-column launches
+
+static void launch_panel_fused(Ctx& ctx, BPtr Ab, int ld, int j0, int m, int nbw, const LuWork& w, int info_base, int batch) {
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(lu_panel_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        configured = true;
+    }
+    int need = (m + LEAF2_TPB - 1) / LEAF2_TPB, csize = 1;
+    while (csize < need) csize <<= 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)csize, (unsigned)batch, 1);
+    cfg.blockDim = dim3((unsigned)LEAF2_TPB, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = ctx.st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)csize;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ctx.note(cudaLaunchKernelEx(&cfg, lu_panel_kernel, Ab, ld, j0, m, nbw, w.ipiv, w.ipiv_stride, w.info, info_base));
+}
+
+// Panel of nbw <= 128 columns at (j0, j0), rows j0 .. n-1, swaps applied inside the panel only; then the inverse of its
+// unit-lower 128 x 128 block for the solves that follow.  Up to 4096 rows: one fused launch (lu_panel_kernel); above
+// (the 2bs corner system at bs > 2048): inner blocks of 16 columns by separate launches (leaf kernel, row swaps,
+// 16-row triangular solve, rank-16 GEMM).
+static void lu_panel(const LuCall& L, int j0, int nbw) {
+    Ctx& ctx = L.ctx;
+    ctx.use(CLS_HI);
+    if (g_panel_fused && L.n - j0 <= LEAF2_TPB * LEAF2_MAXC) {
+        launch_panel_fused(ctx, L.Ab, L.ld, j0, L.n - j0, nbw, L.w, L.info_base, L.batch);
+    } else {
         for (int c = j0; c < j0 + nbw; c += LEAF_JB) {
             const int jb = min(LEAF_JB, j0 + nbw - c);
-            const int m = n - c;
-            launch_leaf(ctx, Ab, ld, c, c, m, jb, w, info_base, batch);
-            {
-                int total = c + (ncols - (c + jb));
-                if (total > 0) {
-                    dim3 grid((unsigned)((total + 255) / 256), (unsigned)batch);
-                    laswp_kernel<<<grid, 256, 0, ctx.st>>>(Ab, ld, ncols, c, jb, c, c + jb, w.ipiv, w.ipiv_stride);
-                    ctx.note(cudaGetLastError());
-                }
-            }
+            const int m = L.n - c;
+            launch_leaf(ctx, L.Ab, L.ld, c, c, m, jb, L.w, L.info_base, L.batch);
+            lu_swaps(L, c, c + jb, j0, j0 + nbw, c, c + jb);
             const int wcols = j0 + nbw - (c + jb);
             if (wcols > 0) {
-                dim3 grid((unsigned)((wcols + 127) / 128), (unsigned)batch);
-                trsm_leaf_kernel<<<grid, 128, 0, ctx.st>>>(Ab, ld, c, jb, c + jb, wcols);
+                dim3 grid((unsigned)((wcols + 127) / 128), (unsigned)L.batch);
+                trsm_leaf_kernel<<<grid, 128, 0, ctx.st>>>(L.Ab, L.ld, c, jb, c + jb, wcols);
                 ctx.note(cudaGetLastError());
                 if (m - jb > 0) {
-                    GemmArgs g = gemm_std(m - jb, wcols, jb, -1.0, bp_offset(Ab, (long long)(c + jb) * ld + c), ld,
-                                          bp_offset(Ab, (long long)c * ld + c + jb), ld, 1.0,
-                                          bp_offset(Ab, (long long)(c + jb) * ld + c + jb), ld);
-                    gemm_run(ctx, g, batch, GEMM_BIG, EPI_STD);
+                    GemmArgs g = gemm_std(m - jb, wcols, jb, -1.0, bp_offset(L.Ab, (long long)(c + jb) * L.ld + c), L.ld,
+                                          bp_offset(L.Ab, (long long)c * L.ld + c + jb), L.ld, 1.0,
+                                          bp_offset(L.Ab, (long long)(c + jb) * L.ld + c + jb), L.ld);
+                    gemm_run(ctx, g, L.batch, GEMM_BIG, EPI_STD);
                 }
             }
         }
-        const int rest = ncols - (j0 + nbw);
-        if (rest > 0) {
-            TrtriArgs t{};
-            t.T = bp_offset(Ab, (long long)j0 * ld + j0); t.ld = ld; t.t_step = 0; t.n_total = nbw;
-            t.out = w.tinv; t.nblocks = 1; t.upper = 0; t.unit = 1;
-            launch_trtri(ctx.st, t, 1, batch);
-            ctx.note(cudaGetLastError());
-            ctx.use(CLS_LO);
-            BPtr A12 = bp_offset(Ab, (long long)j0 * ld + j0 + nbw);
-            GemmArgs g = gemm_std(nbw, rest, nbw, 1.0, bp_strided(w.tinv, 128 * 128), 128, A12, ld, 0.0, A12, ld);
-            gemm_run(ctx, g, batch, GEMM_TALL, EPI_STD);
-            const int mrest = n - (j0 + nbw);
-            if (mrest > 0) {
-                GemmArgs u = gemm_std(mrest, rest, nbw, -1.0, bp_offset(Ab, (long long)(j0 + nbw) * ld + j0), ld, A12, ld,
-                                      1.0, bp_offset(Ab, (long long)(j0 + nbw) * ld + j0 + nbw), ld);
-                gemm_run(ctx, u, batch, GEMM_BIG, EPI_STD);
-            }
+    }
+    TrtriArgs t{};
+    t.T = bp_offset(L.Ab, (long long)j0 * L.ld + j0); t.ld = L.ld; t.t_step = 0; t.n_total = nbw;
+    t.out = L.w.tinv + (long long)(j0 / 128) * 128 * 128; t.nblocks = 2 * L.nblk(); t.upper = 0; t.unit = 1;
+    launch_trtri(ctx.st, t, 1, L.batch);
+    ctx.note(cudaGetLastError());
+}
+
+// A[r0:r1, ca:cb] <- L[r0:r1, r0:r1]^-1 A[r0:r1, ca:cb], L = unit lower factor in place; r0 a multiple of 128.
+static void lu_trsm_lower(const LuCall& L, int r0, int r1, int ca, int cb) {
+    if (cb <= ca) return;
+    Ctx& ctx = L.ctx;
+    ctx.use(CLS_LO);
+    for (int k = r0; k < r1; k += 128) {
+        const int nk = min(128, r1 - k);
+        BPtr Ak = bp_offset(L.Ab, (long long)k * L.ld + ca);
+        if (k > r0) {
+            GemmArgs g = gemm_std(nk, cb - ca, k - r0, -1.0, bp_offset(L.Ab, (long long)k * L.ld + r0), L.ld,
+                                  bp_offset(L.Ab, (long long)r0 * L.ld + ca), L.ld, 1.0, Ak, L.ld);
+            gemm_run(ctx, g, L.batch, GEMM_BIG, EPI_STD);
         }
+        GemmArgs g2 = gemm_std(nk, cb - ca, nk, 1.0, L.tinvL(k / 128), 128, Ak, L.ld, 0.0, Ak, L.ld);
+        gemm_run(ctx, g2, L.batch, GEMM_TALL, EPI_STD);
+    }
+}
+
+static void lu_recursive(const LuCall& L, int c0, int c1) {
+    const int wd = c1 - c0;
+    if (wd <= 128) { lu_panel(L, c0, wd); return; }
+    const int mid = c0 + ((wd / 2 + 127) / 128) * 128;
+    lu_recursive(L, c0, mid);
+    L.ctx.use(CLS_HI);
+    lu_swaps(L, c0, mid, mid, c1, mid, mid);
+    lu_trsm_lower(L, c0, mid, mid, c1);
+    if (L.n > mid) {
+        GemmArgs u = gemm_std(L.n - mid, c1 - mid, mid - c0, -1.0, bp_offset(L.Ab, (long long)mid * L.ld + c0), L.ld,
+                              bp_offset(L.Ab, (long long)c0 * L.ld + mid), L.ld, 1.0,
+                              bp_offset(L.Ab, (long long)mid * L.ld + mid), L.ld);
+        L.ctx.use(CLS_LO);
+        gemm_run(L.ctx, u, L.batch, GEMM_BIG, EPI_STD);
+    }
+    lu_recursive(L, mid, c1);
+    L.ctx.use(CLS_HI);
+    lu_swaps(L, mid, c1, c0, mid, mid, mid);
+}
+
+static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, const LuWork& w, int info_base) {
+    LuCall L{ctx, Ab, ld, n, ncols, batch, w, info_base};
+    lu_recursive(L, 0, n);
+    if (ncols > n) {
+        ctx.use(CLS_HI);
+        lu_swaps(L, 0, n, n, ncols, ncols, ncols);
+        lu_trsm_lower(L, 0, n, n, ncols);
     }
 }
 
@@ -656,9 +906,10 @@ static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, in
 static void back_substitute(Ctx& ctx, BPtr Ab, int ld, int n, int nrhs, BPtr X, int ldx, int batch, const LuWork& w) {
     if (nrhs <= 0 || n <= 0) return;
     const int P = 128;
-    const int nblk = (n + P - 1) / P;
+    LuCall L{ctx, Ab, ld, n, n + nrhs, batch, w, 0};
+    const int nblk = L.nblk();
     TrtriArgs t{};
-    t.T = Ab; t.ld = ld; t.t_step = (long long)P * ld + P; t.n_total = n; t.out = w.tinv; t.nblocks = nblk;
+    t.T = Ab; t.ld = ld; t.t_step = (long long)P * ld + P; t.n_total = n; t.out = w.tinv + (long long)nblk * P * P; t.nblocks = 2 * nblk;
     t.upper = 1; t.unit = 0;
     ctx.use(CLS_HI);
     launch_trtri(ctx.st, t, nblk, batch);
@@ -672,8 +923,7 @@ static void back_substitute(Ctx& ctx, BPtr Ab, int ld, int n, int nrhs, BPtr X, 
                                   bp_offset(X, (long long)(j + nbj) * ldx), ldx, 1.0, Yj, ld);
             gemm_run(ctx, g, batch, GEMM_BIG, EPI_STD);
         }
-        GemmArgs g2 = gemm_std(nbj, nrhs, nbj, 1.0, bp_strided(w.tinv + (long long)jb * P * P, (long long)nblk * P * P), P,
-                               Yj, ld, 0.0, bp_offset(X, (long long)j * ldx), ldx);
+        GemmArgs g2 = gemm_std(nbj, nrhs, nbj, 1.0, L.tinvU(jb), P, Yj, ld, 0.0, bp_offset(X, (long long)j * ldx), ldx);
         gemm_run(ctx, g2, batch, GEMM_BIG, EPI_STD);
     }
 }

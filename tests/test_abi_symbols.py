@@ -54,7 +54,7 @@ def test_pure_host_queries(libpath):
     assert lib.ss_create(4, 5000, 1, ctypes.byref(h)) == binding.SS_ERR_INVALID_ARG
     assert lib.ss_create(4, 16, 0, ctypes.byref(h)) == binding.SS_ERR_INVALID_ARG
     assert lib.ss_destroy(None) == binding.SS_OK
-    assert lib.ss_set_option(None, b"nb_lu", 64) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_set_option(None, b"stream_groups", 2) == binding.SS_ERR_INVALID_ARG
 
 
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):
@@ -92,7 +92,7 @@ def test_host_side_argument_logic_without_a_device(libpath):
     assert lib.ss_destroy(None) == binding.SS_OK
     assert lib.ss_solve(None, None, None, None, None, None, 0, None, None) == binding.SS_ERR_INVALID_ARG
     assert lib.ss_transmission(None, None) == binding.SS_ERR_INVALID_ARG
-    assert lib.ss_set_option(None, b"nb_lu", 64) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_set_option(None, b"stream_groups", 2) == binding.SS_ERR_INVALID_ARG
     assert lib.ss_strerror(binding.SS_OK) == b"ok" and lib.ss_strerror(binding.SS_ERR_SINGULAR) == b"exactly zero pivot"
     assert lib.ss_workspace_bytes(1, 8, 1, 1) == 0 and lib.ss_workspace_bytes(2, 8, 1, -1) == 0
     # workspace grows with every size argument and is dominated by the 2 (nb+1) bs^2 slots per energy
@@ -107,7 +107,8 @@ def test_host_side_argument_logic_without_a_device(libpath):
     assert lib.ss_set_default_gemm_variant(len(binding.GEMM_VARIANTS)) == binding.SS_ERR_INVALID_ARG
     assert binding.get_default_gemm_variant() == d
     assert lib.ss_zgemm_batched(-1, 1, 1, 1.0, None, 1, 0, None, 1, 0, 0.0, None, 1, 0, 1, None) == binding.SS_ERR_INVALID_ARG
-    assert lib.ss_zgetrf_batched(0, 0, None, 0, 0, None, None, 1, None) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_zgetrf_batched(0, 0, None, 0, 0, None, None, 1, None, 0, None) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_lu_workspace_bytes(0, 1) == 0 and lib.ss_lu_workspace_bytes(300, 2) == 2 * 2 * 3 * 128 * 128 * 16
 
 
 def test_closed_form_flop_counts_match_survey_table():
