@@ -69,6 +69,7 @@ def parse():
                     "default: the library default (3M)")
     ap.add_argument("--stream-groups", type=int, default=None, help="stream groups the energies are split over "
                     "(library default 4; 1 = single stream)")
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=INT", help="extra ss_set_option calls (tuning)")
     ap.add_argument("--trace", default=None, help="write the phase timeline of the last timed step to this CSV")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -266,6 +267,9 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     ss = binding.SplitSolve(nb, bs, nE)
     groups = 4 if args.stream_groups is None else args.stream_groups
     ss.set_option("stream_groups", groups)
+    for kv in args.option:
+        k, v = kv.split("=")
+        ss.set_option(k, int(v))
     if args.trace:
         ss.set_option("trace", 1)
     ss.set_hamiltonian(devt["H_diag"], devt["H_upper"], devt["S_diag"], devt["S_upper"])

@@ -16,20 +16,22 @@ from . import dense
 
 def assemble_T_band(E, H_diag, H_upper, S_diag, S_upper, Sigma_L, Sigma_R):
     """T = E*S - H - Sigma^RB (Eq. 5; Sigma blocks per L148) in zgbsv layout:
-    ab[kl + ku + i - j, j] = T[i, j], shape (2*kl + ku + 1, n), kl = ku = 2*bs - 1."""
-    H_diag = np.asarray(H_diag, dtype=np.complex128)
-    nb, bs, _ = H_diag.shape
+    ab[kl + ku + i - j, j] = T[i, j], shape (2*kl + ku + 1, n), kl = ku = 2*bs - 1.
+    The block stacks are only indexed block by block (H_diag[i], ...), so lazy sequences that generate a block on
+    access work too (BASELINE.json config 4: H and S are 25 GB, the band 39 GB).  Column-major, as LAPACK wants it."""
+    nb = len(H_diag)
+    bs = np.asarray(H_diag[0]).shape[0]
     n = nb * bs
     kl = ku = 2 * bs - 1
     E = complex(E)
-    ab = np.zeros((2 * kl + ku + 1, n), dtype=np.complex128)
+    ab = np.zeros((2 * kl + ku + 1, n), dtype=np.complex128, order="F")
     ii, jj = np.meshgrid(np.arange(bs), np.arange(bs), indexing="ij")
 
     def put(block, r0, c0):
         ab[kl + ku + (r0 - c0) + ii - jj, c0 + jj] = block
 
     for i in range(nb):
-        blk = E * np.asarray(S_diag[i], dtype=np.complex128) - H_diag[i]
+        blk = E * np.asarray(S_diag[i], dtype=np.complex128) - np.asarray(H_diag[i], dtype=np.complex128)
         if i == 0:
             blk = blk - np.asarray(Sigma_L, dtype=np.complex128)
         if i == nb - 1:
@@ -46,8 +48,8 @@ def assemble_T_band(E, H_diag, H_upper, S_diag, S_upper, Sigma_L, Sigma_R):
 def solve_energy(E, H_diag, H_upper, S_diag, S_upper, Sigma_L, Sigma_R, Inj_first, Inj_last=None,
                  want_G=True):
     """Same contract as dense.solve_energy (X, G_1N, G_N1, T_LR, T_RL), via banded LU (zgbsv)."""
-    H_diag = np.asarray(H_diag)
-    nb, bs, _ = H_diag.shape
+    nb = len(H_diag)
+    bs = np.asarray(H_diag[0]).shape[0]
     n = nb * bs
     ab, kl, ku = assemble_T_band(E, H_diag, H_upper, S_diag, S_upper, Sigma_L, Sigma_R)
     b = dense.pad_injection(Inj_first, Inj_last, nb)
@@ -131,8 +133,8 @@ def solve_energy_columns(E, H_diag, H_upper, S_diag, S_upper, Sigma_L, Sigma_R, 
     """Large-size form of `solve_energy`: one banded LU of T, then X only for the columns `x_cols` of Inj (every
     column of X = T^-1 Inj is its own solve, Eq. 5) and the whole last block column of T^-1 (Eq. 4), whose top block
     is G_1N.  Returns dict(X_cols [n, len(x_cols)], x_cols, G_last [n, bs], G_1N, T_LR, T_LR_complex)."""
-    H_diag = np.asarray(H_diag)
-    nb, bs, _ = H_diag.shape
+    nb = len(H_diag)
+    bs = np.asarray(H_diag[0]).shape[0]
     n = nb * bs
     b = dense.pad_injection(Inj_first, Inj_last, nb)
     x_cols = list(range(b.shape[1])) if x_cols is None else [int(c) for c in x_cols]

@@ -47,6 +47,21 @@ def algorithm1_first_column(E, H_diag, H_upper, S_diag, S_upper):
     return np.stack(Q[1:]), X[1:nb + 1]
 
 
+def schur_complements_first_column(E, H_diag, H_upper, S_diag, S_upper):
+    """The matrices D_i = A_ii - A_{i,i+1} X_{i+1} that Algorithm 1's "Solve" step (L164) factors, i = 1..nb
+    (D[i-1] = D_i).  PAPER.md L154: "A is usually real symmetric in 3-D structures and complex Hermitian in 1-D and
+    2-D" -- at real E every D_i is then Hermitian, which is what L266's zhesv_nopiv_gpu exploits (SURVEY.md 8(f1))."""
+    Ad, Au, Al = _blocks(E, H_diag, H_upper, S_diag, S_upper)
+    nb = len(Ad)
+    D = [None] * (nb + 1)
+    Xn = None
+    for i in range(nb, 0, -1):
+        D[i] = Ad[i - 1] - (Au[i - 1] @ Xn if i < nb else 0.0)
+        if i > 1:
+            Xn = np.linalg.solve(D[i], Al[i - 2])
+    return D[1:]
+
+
 def algorithm1_last_column(E, H_diag, H_upper, S_diag, S_upper):
     """Mirror of Algorithm 1 for the last block column (L167 "derived similarly"; reading c2).
     Returns P [nb,bs,bs], P[i-1] = (A^-1)_{i,nb}, and the list of Y_i."""

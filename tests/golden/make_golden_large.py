@@ -42,6 +42,21 @@ def sample_plan(cfg):
     return x_cols, rows, r, gpos
 
 
+class LazyBlocks:
+    """A block stack that generates block i on access (input plumbing only: config 4's H and S are 25 GB)."""
+
+    def __init__(self, fn, count):
+        self.fn, self.count = fn, count
+
+    def __len__(self):
+        return self.count
+
+    def __getitem__(self, i):
+        if not 0 <= i < self.count:
+            raise IndexError(i)
+        return self.fn(i)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("config", choices=["C3", "C4", "C2"])
@@ -52,13 +67,16 @@ def main():
     cfg = inputs.CONFIGS[a.config]
     e = DEFAULT_ENERGY.get(a.config, 0) if a.energy is None else a.energy
     t0 = time.perf_counter()
-    hs = inputs.random_problem(cfg.bs, cfg.nb, 1, 1, seed=cfg.seed, threads=os.cpu_count() or 1)      # H, S only
+    Hd = LazyBlocks(lambda i: inputs.h_diag_block(cfg.seed, i, cfg.bs), cfg.nb)
+    Hu = LazyBlocks(lambda i: inputs.h_upper_block(cfg.seed, i, cfg.bs), cfg.nb - 1)
+    Sd = LazyBlocks(lambda i: inputs.s_diag_block(cfg.seed, i, cfg.bs), cfg.nb)
+    Su = LazyBlocks(lambda i: inputs.s_upper_block(cfg.seed, i, cfg.bs), cfg.nb - 1)
     E = inputs.energy_grid(cfg.n_energy, cfg.e_lo, cfg.e_hi, cfg.eta)[e]
     sl, sr = inputs.sigma_block(cfg.seed, e, cfg.bs, "L"), inputs.sigma_block(cfg.seed, e, cfg.bs, "R")
     inj = inputs.inj_block(cfg.seed, e, cfg.bs, cfg.nrhs)
     x_cols, rows, r, gpos = sample_plan(cfg)
     print(f"inputs {time.perf_counter() - t0:.1f} s", flush=True)
-    res = banded.solve_energy_columns(E, hs.H_diag, hs.H_upper, hs.S_diag, hs.S_upper, sl, sr, inj, None,
+    res = banded.solve_energy_columns(E, Hd, Hu, Sd, Su, sl, sr, inj, None,
                                       x_cols=x_cols, chunk=16, threads=a.threads)
     dt = time.perf_counter() - t0
     print(f"banded solve done {dt:.1f} s, T_LR = {res['T_LR']!r}", flush=True)
@@ -68,19 +86,19 @@ def main():
         f.write(f"# Tier B fingerprint of BASELINE.json config {a.config} (bs={cfg.bs} nb={cfg.nb} nrhs={cfg.nrhs} seed {cfg.seed}), "
                 f"energy index {e}; oracle/banded.py solve_energy_columns (zgbtrf/zgbtrs on the full matrix T, Eq. 5 PAPER.md L82);\n"
                 f"# written by tests/golden/make_golden_large.py in {dt:.0f} s on {os.cpu_count()} host cores\n")
-        f.write(f"config {a.config}\nenergy_index {e}\nE {E.real!r} {E.imag!r}\n")
-        f.write(f"T_LR {res['T_LR']!r}\nT_LR_imag {res['T_LR_complex'].imag!r}\n")
+        f.write(f"config {a.config}\nenergy_index {e}\nE {float(E.real)!r} {float(E.imag)!r}\n")
+        f.write(f"T_LR {float(res['T_LR'])!r}\nT_LR_imag {float(res['T_LR_complex'].imag)!r}\n")
         f.write(f"G1N_fro {float(np.linalg.norm(G))!r}\n")
         for j, c in enumerate(x_cols):
             pr = np.vdot(r, X[:, j])
-            f.write(f"xcol {int(c)} {float(np.linalg.norm(X[:, j]))!r} {pr.real!r} {pr.imag!r}\n")
+            f.write(f"xcol {int(c)} {float(np.linalg.norm(X[:, j]))!r} {float(pr.real)!r} {float(pr.imag)!r}\n")
         for j, c in enumerate(x_cols):
             for i in rows:
                 v = X[i, j]
-                f.write(f"x {int(i)} {int(c)} {v.real!r} {v.imag!r}\n")
+                f.write(f"x {int(i)} {int(c)} {float(v.real)!r} {float(v.imag)!r}\n")
         for (i, j) in gpos:
             v = G[i, j]
-            f.write(f"g {int(i)} {int(j)} {v.real!r} {v.imag!r}\n")
+            f.write(f"g {int(i)} {int(j)} {float(v.real)!r} {float(v.imag)!r}\n")
     print("wrote", out, flush=True)
 
 

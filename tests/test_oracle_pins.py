@@ -480,3 +480,25 @@ def test_banded_column_solve_is_the_banded_solve():
         assert residual.rel_T(r1["T_LR"], rd["T_LR"]) < 1e-10
         T = dense.assemble_T(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e])
         assert np.allclose(r1["G_last"], np.linalg.inv(T)[:, -9:], rtol=1e-9, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------------
+# structure at real energies
+# ------------------------------------------------------------------------------------------------------
+def test_schur_complements_are_hermitian_at_real_energy_and_match_the_dense_definition():
+    """D_i of Algorithm 1 is the Schur complement of the trailing blocks: D_i^-1 = [(A_{i:,i:})^-1]_11 (checked against
+    a dense inverse of the trailing sub-matrix, not against the recursion).  A = A^H at Im E = 0 (L154) => D_i = D_i^H;
+    at Im E != 0 it is not (reading c8: E is never conjugated), so a Hermitian factorisation may be used at real E only."""
+    p = tiny(5, 4, eta=0.0)
+    E = p.E[0].real
+    D = stepwise.schur_complements_first_column(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    A = dense.assemble_A(E, p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+    assert np.allclose(A, A.conj().T, atol=1e-15)
+    for i in range(4):
+        sub = A[i * 5:, i * 5:]
+        want = np.linalg.inv(np.linalg.inv(sub)[:5, :5])
+        assert np.allclose(D[i], want, rtol=1e-9, atol=1e-11)
+        assert np.abs(D[i] - D[i].conj().T).max() <= 1e-12 * np.abs(D[i]).max()
+    p2 = tiny(5, 4, eta=1e-3)
+    D2 = stepwise.schur_complements_first_column(p2.E[0], p2.H_diag, p2.H_upper, p2.S_diag, p2.S_upper)
+    assert np.abs(D2[0] - D2[0].conj().T).max() >= 1e-4
