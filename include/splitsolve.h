@@ -123,9 +123,16 @@ ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cplx* Q_first_
 ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int* column);
 
 /* Closed-form flop count of steps a1-a7 per energy point (LAPACK convention: complex multiply-add = 8 flops;
- * ZGEMM 8MNK, ZGETRF (8/3)n^3, ZTRSM 4n^2 nrhs).  ss_flops_sweep counts a1-a4 only: (160/3 nb - 32) bs^3. */
+ * ZGEMM 8MNK, ZGETRF (8/3)n^3, ZTRSM 4n^2 nrhs) of the path the LAST ss_solve took (before any solve: the general
+ * path).  ss_flops_sweep counts a1-a4 only: general path (160/3 nb - 32) bs^3; with the Hermitian Schur update
+ * (modes 1, 2 of option "hermitian") a1 counts 4 bs^3 per block instead of 8, with L Delta L^H a2 counts 4/3 bs^3 instead of 8/3. */
 double ss_flops(ss_handle_t h, int nrhs);
 double ss_flops_sweep(ss_handle_t h);
+
+/* Which path the last ss_solve took: *mode = 0 general, 1 Hermitian Schur update, 2 + no-pivot L Delta L^H;
+  * *retried = 1 if a mode-2 solve exceeded its growth limit and was redone on the general path (then *mode = 0).
+ * Meaningful after ss_synchronize / ss_transmission. */
+ss_status_t ss_last_mode(ss_handle_t h, int* mode, int* retried);
 
 /* Device bytes the handle allocates for (nb, bs, n_energy, nrhs), excluding caller-owned inputs/outputs. */
 size_t ss_workspace_bytes(int nb, int bs, int n_energy, int nrhs);
@@ -146,7 +153,22 @@ ss_status_t ss_trace_write(ss_handle_t h, const char* path);
  * algorithmic flops (8 M N K per complex GEMM) and their number.  Synchronises. */
 ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long* launches);
 
-/* Options: "transmission" (0/1, default 1:
+/* Options: "hermitian" (0/1/2, default 0): what to exploit when EVERY energy of a
+ * solve has Im E == 0, where A = E S - H and all Schur complements D_i are Hermitian in exact arithmetic.
+ *   0: nothing (the general path: full Schur update, LU with partial pivoting).
+ *   1: the Schur update D_i = A_ii - A_{i,i+1} X_{i+1} computes the lower triangle only (half the a1 flops) and mirrors it.
+ *   2: additionally D_i is factored WITHOUT pivoting as L Delta L^H (the paper's zhesv_nopiv: half the a2 flops, no pivot
+ *      search, no row interchanges); the largest multiplier met is monitored, and if it exceeds "hermitian_growth_limit"
+ *      (default 64) -- or a pivot is exactly zero -- the results are discarded at the next ss_synchronize / ss_transmission /
+ *      ss_solve_host and the whole solve is redone on the general path with the same arguments (which must therefore still
+ *      be valid then).
+ * NUMERICAL CAVEAT (measured): both modes replace the computed product A_{i,i+1} X_{i+1} by its
+ * Hermitian part.  The discarded anti-Hermitian part is the forward error of X_{i+1} (~ kappa(D_{i+1}) u), and the general
+ * path owes its small backward error to keeping it: at real energies INSIDE the band, where A itself is nearly singular,
+ * modes 1 and 2 lose digits in proportion to kappa(A) (backward errors 1e-11 .. 1e-4 on the random test devices against
+ * 1e-15 .. 1e-12 for mode 0).  They are exact on the perfect chain (config 1) and meet the tolerances when A is
+ * definite (energies outside the spectrum).  Hence off by default.
+ * "transmission" (0/1, default 1:
  * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0), "gemm_variant" (see ss_set_default_gemm_variant;
  * default = the process-wide default at ss_create), "trace" (0/1, default 0: record a CUDA-event
  * timeline of every group's high-/low-priority phases, see ss_trace_write), "stream_groups" (1..16,

@@ -28,6 +28,7 @@ SIGNATURES = {
     "ss_inverse_columns": (c_int, [c_void_p, c_int, POINTER(c_void_p), POINTER(c_void_p)]),
     "ss_copy_inverse_columns": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
     "ss_last_info": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int), POINTER(c_int)]),
+    "ss_last_mode": (c_int, [c_void_p, POINTER(c_int), POINTER(c_int)]),
     "ss_flops": (c_double, [c_void_p, c_int]),
     "ss_flops_sweep": (c_double, [c_void_p]),
     "ss_workspace_bytes": (c_size_t, [c_int, c_int, c_int, c_int]),
@@ -176,6 +177,12 @@ class SplitSolve:
         e, b, c = c_int(), c_int(), c_int()
         _check(load().ss_last_info(self._h, byref(e), byref(b), byref(c)), "ss_last_info")
         return e.value, b.value, c.value
+
+    def last_mode(self):
+        """(mode, retried) of the last solve: 0 general, 1 Hermitian Schur update, 2 + no-pivot L Delta L^H."""
+        m, r = c_int(), c_int()
+        _check(load().ss_last_mode(self._h, byref(m), byref(r)), "ss_last_mode")
+        return m.value, r.value
 
     def flops(self, nrhs: int) -> float:
         return float(load().ss_flops(self._h, nrhs))

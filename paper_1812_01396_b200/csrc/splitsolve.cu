@@ -21,6 +21,12 @@ struct ss_handle_s {
     bool launched = false;           // some ss_solve has been enqueued: ev[2] is a valid event to wait on
     // options
     int want_T = 1;
+    int hermitian = 0;               // SURVEY 8(f1) at real energies: 0 off, 1 Hermitian Schur update, 2 + no-pivot L Delta L^H
+    int growth_limit = 64;           // mode 2: largest multiplier tolerated before the solve is redone with the pivoted LU
+    int mode = 0;                    // what the last ss_solve used
+    bool force_general = false;      // set while a solve is being redone
+    int retried = 0;                 // that solve was redone on the pivoted path (growth limit exceeded)
+    struct { const ss_cplx *sl, *sr, *i1, *i2; ss_cplx* x; int nrhs; void* stream; } last_args{};
     int profile_gemm = 0;
     int gemm_variant = g_default_variant;
     int stream_groups = 4;
@@ -45,7 +51,7 @@ struct ss_handle_s {
     cplx *slots = nullptr, *aug = nullptr, *aop = nullptr, *tinv = nullptr, *raug = nullptr, *wz = nullptr;
     cplx *gam_l = nullptr, *gam_r = nullptr, *g1n = nullptr, *w1 = nullptr, *w2 = nullptr, *E_dev = nullptr;
     double *tpart = nullptr, *T_dev = nullptr;
-    int *ipiv = nullptr, *info = nullptr;
+    int *ipiv = nullptr, *info = nullptr, *perm = nullptr;
     cplx* E_pinned = nullptr;
     // host-path buffers
     cplx *hp_sigl = nullptr, *hp_sigr = nullptr, *hp_inj1 = nullptr, *hp_inj2 = nullptr, *hp_x = nullptr;
@@ -72,17 +78,21 @@ static void free_dev(void* p) { if (p) cudaFree(p); }
 static void free_workspace(ss_handle_t h) {
     free_dev(h->slots); free_dev(h->aug); free_dev(h->aop); free_dev(h->tinv); free_dev(h->raug); free_dev(h->wz);
     free_dev(h->gam_l); free_dev(h->gam_r); free_dev(h->g1n); free_dev(h->w1); free_dev(h->w2); free_dev(h->E_dev);
-    free_dev(h->tpart); free_dev(h->T_dev); free_dev(h->ipiv); free_dev(h->info);
+    free_dev(h->tpart); free_dev(h->T_dev); free_dev(h->ipiv); free_dev(h->info); free_dev(h->perm);
     h->slots = h->aug = h->aop = h->tinv = h->raug = h->wz = nullptr;
     h->gam_l = h->gam_r = h->g1n = h->w1 = h->w2 = h->E_dev = nullptr;
-    h->tpart = h->T_dev = nullptr; h->ipiv = h->info = nullptr;
+    h->tpart = h->T_dev = nullptr; h->ipiv = h->info = h->perm = nullptr;
     h->ws_nrhs = -1;
 }
 
 struct WsSizes {
-    size_t slots, aug, aop, tinv, raug, wz, sq, E, tpart, T, ipiv, info;
-    size_t total() const { return slots + aug + aop + tinv + raug + wz + 5 * sq + E + tpart + T + ipiv + info; }
+    size_t slots, aug, aop, tinv, raug, wz, sq, E, tpart, T, ipiv, info, perm;
+    size_t total() const { return slots + aug + aop + tinv + raug + wz + 5 * sq + E + tpart + T + ipiv + info + perm; }
 };
+
+// ints of row-permutation scratch per energy: enough for its two chains' sweeps (n = bs) and, afterwards, its corner
+// system (n = 2bs); every stream group owns the slice of its energies
+static inline size_t perm_ints_per_energy(int bs) { return ((size_t)2 * (3 * (size_t)bs + 1) + 7) / 4 * 4 + 4; }
 
 static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
     WsSizes w;
@@ -102,7 +112,8 @@ static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
     w.tpart = (size_t)nE * TRACE_PARTS * sizeof(double);
     w.T = (size_t)nE * sizeof(double);
     w.ipiv = (size_t)3 * nE * 2 * bs * sizeof(int);
-    w.info = (size_t)3 * nE * sizeof(int);
+    w.info = (size_t)5 * nE * sizeof(int);                     // 3 nE zero-pivot records, 2 nE growth monitors
+    w.perm = (size_t)nE * perm_ints_per_energy(bs) * sizeof(int);
     return w;
 }
 
@@ -116,7 +127,7 @@ static ss_status_t ensure_workspace(ss_handle_t h, int nrhs) {
     A((void**)&h->raug, w.raug); A((void**)&h->wz, w.wz);
     A((void**)&h->gam_l, w.sq); A((void**)&h->gam_r, w.sq); A((void**)&h->g1n, w.sq); A((void**)&h->w1, w.sq);
     A((void**)&h->w2, w.sq); A((void**)&h->E_dev, w.E); A((void**)&h->tpart, w.tpart); A((void**)&h->T_dev, w.T);
-    A((void**)&h->ipiv, w.ipiv); A((void**)&h->info, w.info);
+    A((void**)&h->ipiv, w.ipiv); A((void**)&h->info, w.info); A((void**)&h->perm, w.perm);
     if (!ok) { cudaGetLastError(); free_workspace(h); return SS_ERR_ALLOC; }
     h->ws_nrhs = nrhs;
     return SS_OK;
@@ -251,6 +262,14 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         h->stream_groups = value; return SS_OK;
     }
     if (!strcmp(name, "trace")) { h->want_trace = value ? 1 : 0; return SS_OK; }
+    if (!strcmp(name, "hermitian")) {
+        if (value < 0 || value > 2) return SS_ERR_INVALID_ARG;
+        h->hermitian = value; return SS_OK;
+    }
+    if (!strcmp(name, "hermitian_growth_limit")) {
+        if (value < 1) return SS_ERR_INVALID_ARG;
+        h->growth_limit = value; return SS_OK;
+    }
     if (!strcmp(name, "panel_fused")) { g_panel_fused = value ? 1 : 0; return SS_OK; }      // process-wide (tuning)
     if (!strcmp(name, "gemm_variant")) {
         if (value < 0 || value >= GV_COUNT) return SS_ERR_INVALID_ARG;
@@ -259,23 +278,38 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
     return SS_ERR_INVALID_ARG;
 }
 
+// Closed-form flop counts (LAPACK convention) of the path the LAST ss_solve took (before any solve: the general path).
+// Per block and chain: a1 8 bs^3 (Hermitian Schur update, modes 1 and 2: 4 bs^3), a2 8/3 bs^3 (mode 2, L Delta L^H: 4/3 bs^3),
+// a3 8 bs^3, a4 8 bs^3; the first block of a chain has no a1, the last no a4.
+static double sweep_flops(const ss_handle_s* h) {
+    const double bs3 = (double)h->bs * h->bs * h->bs, nb = h->nb;
+    const double a1 = (h->mode >= 1 ? 4.0 : 8.0), a2 = (h->mode == 2 ? 4.0 / 3.0 : 8.0 / 3.0);
+    return 2.0 * ((nb - 1) * a1 + nb * a2 + nb * 8.0 + (nb - 1) * 8.0) * bs3;
+}
+
 extern "C" double ss_flops_sweep(ss_handle_t h) {
     if (!h) return 0.0;
-    double bs3 = (double)h->bs * h->bs * h->bs;
-    return (160.0 / 3.0 * h->nb - 32.0) * bs3;
+    return sweep_flops(h);
 }
 
 extern "C" double ss_flops(ss_handle_t h, int nrhs) {
     if (!h || nrhs < 0) return 0.0;
     const double bs = h->bs, nb = h->nb, m = nrhs;
     const double bs3 = bs * bs * bs;
-    double sweep = (160.0 / 3.0 * nb - 32.0) * bs3;
+    double sweep = sweep_flops(h);
     // a5: 4 GEMM (32 bs^3) + ZGETRF(2bs) (64/3 bs^3) + 2 ZTRSM with m rhs (2 * 4 (2bs)^2 m = 32 bs^2 m)
     double a5 = 32.0 * bs3 + 64.0 / 3.0 * bs3 + 32.0 * bs * bs * m;
     double a6 = 16.0 * nb * bs * bs * m;
     // a7: R^-1[:, bs:] (2 ZTRSM with bs rhs: 32 bs^3) + G (16 bs^3) + two Gamma products (16 bs^3) + trace (8 bs^2)
     double a7 = h->want_T ? (64.0 * bs3 + 8.0 * bs * bs) : 0.0;
     return sweep + a5 + a6 + a7;
+}
+
+extern "C" ss_status_t ss_last_mode(ss_handle_t h, int* mode, int* retried) {
+    if (!h || !mode || !retried) return SS_ERR_INVALID_ARG;
+    if (!h->solved) return SS_ERR_NOT_READY;
+    *mode = h->mode; *retried = h->retried;
+    return SS_OK;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -310,17 +344,25 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
     LuWork w;
     w.tinv = h->tinv + lu_tinv_elems(bs, 2 * e0);
     w.ipiv = h->ipiv + (long long)2 * e0 * 2 * bs; w.ipiv_stride = 2 * bs; w.info = h->info + 2 * e0;
+    w.growth = h->info + 3 * h->n_energy + 2 * e0;
+    const int mode = h->mode;                                  // 0 general, 1 Hermitian Schur update, 2 + L Delta L^H (real energies)
     const int info_stride = 2 * bs + 2;
+
+    w.perm = h->perm + (long long)e0 * perm_ints_per_energy(bs);
+    w.tmp = h->aop + e0 * 2 * B2; w.tmp_elems = B2;            // the formed operand is consumed before the LU starts
 
     const int i_f = nb - s, i_m = s + 1;                       // 1-based block index of each chain
     ctx.use(CLS_HI);
     if (h->upload_pending) cudaStreamWaitEvent(ctx.st, h->up_ev[s], 0);   // H, S blocks of this step (ss_set_hamiltonian_host)
-    // right-hand sides: A_{i,i-1} (column 0) / A_{i,i+1} (column 1); identity at the ends (L164, reading c1)
+    // right-hand sides: A_{i,i-1} (column 0) / A_{i,i+1} (column 1); identity at the ends (L164, reading c1).  Formed into
+    // the slot X_i / Y_i will occupy; the LU copies them into [D | B] with the row interchanges already applied.
     FormSide r0 = (i_f > 1) ? FormSide{h->Su + (long long)(i_f - 2) * B2, h->Hu + (long long)(i_f - 2) * B2, FORM_CONJT}
                             : FormSide{nullptr, nullptr, FORM_IDENT};
     FormSide r1 = (i_m < nb) ? FormSide{h->Su + (long long)(i_m - 1) * B2, h->Hu + (long long)(i_m - 1) * B2, FORM_PLAIN}
                              : FormSide{nullptr, nullptr, FORM_IDENT};
-    launch_form(ctx, r0, r1, E, bp_offset(aug, bs), ldg, bs, batch);
+    const BPtr out = bp_chain(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
+    if (mode == 2) launch_form(ctx, r0, r1, E, bp_offset(aug, bs), ldg, bs, batch);    // no interchanges: straight into [D | B]
+    else launch_form(ctx, r0, r1, E, out, bs, bs, batch);
     GemmArgs g{};
     g.M = bs; g.N = bs; g.K = 0;
     g.A = aop; g.lda = bs; g.B = aop; g.ldb = bs;
@@ -338,11 +380,16 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
     g.S = bp_chain(h->Sd + (long long)(i_f - 1) * B2, h->Sd + (long long)(i_m - 1) * B2, 0);
     g.H = bp_chain(h->Hd + (long long)(i_f - 1) * B2, h->Hd + (long long)(i_m - 1) * B2, 0);
     g.lds = bs; g.E = E;
+    if (mode >= 1) g.tri = 1;                                  // D_i is Hermitian at real E (L154): lower triangle only
     gemm_run(ctx, g, batch, GEMM_BIG, EPI_SCHUR);
     // a2 + the L half of a3
-    lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, w, s * info_stride);
+    if (mode == 2) {
+        lu_factor_herm(ctx, aug, ldg, bs, 2 * bs, batch, w, s * info_stride);
+    } else {
+        if (mode == 1) { ctx.use(CLS_HI); launch_mirror(ctx, aug, ldg, 0, 0, bs, bs, 0, 1, batch); }
+        lu_factor(ctx, aug, ldg, bs, 2 * bs, batch, w, s * info_stride, &out, bs);
+    }
     // U half of a3: X_i / Y_i into its slot
-    BPtr out = bp_chain(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
     back_substitute(ctx, aug, ldg, bs, bs, out, bs, batch, w);
 }
 
@@ -402,6 +449,8 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     w.tinv = h->tinv + lu_tinv_elems(bs, 2 * h->n_energy) + lu_tinv_elems(2 * bs, e0);
     w.ipiv = h->ipiv + (long long)2 * h->n_energy * 2 * bs + (long long)e0 * 2 * bs; w.ipiv_stride = 2 * bs;
     w.info = h->info + 2 * h->n_energy + e0;
+    w.perm = h->perm + (long long)e0 * perm_ints_per_energy(bs);
+    w.tmp = h->aop + e0 * 2 * B2; w.tmp_elems = 2 * B2;
     lu_factor(ctx, bp_strided(raug, s_r), ldW, 2 * bs, W, nE, w, 0);
     back_substitute(ctx, bp_strided(raug, s_r), ldW, 2 * bs, nr, bp_strided(wz, s_w), nr, nE, w);
     // a6: X_i = Q_i w_top + P_i w_bot, batch z = e*nb + (i-1)
@@ -462,7 +511,7 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx*
                                  const cplx* Inj_first, const cplx* Inj_last, int nrhs, cplx* X) {
     auto mark = [&](cudaEvent_t ev) { return cudaEventRecord(ev, stream); };
     if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-        cudaMemsetAsync(h->info, 0, sizeof(int) * 3 * (size_t)h->n_energy, stream) != cudaSuccess)
+        cudaMemsetAsync(h->info, 0, sizeof(int) * 5 * (size_t)h->n_energy, stream) != cudaSuccess)
         return cudaErrorUnknown;
     // Energy points are independent: split them over stream groups.  Group g owns the energies
     // [e0, e0 + nE); the host interleaves the groups' launches step by step so that every group's streams stay fed.
@@ -539,7 +588,17 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
     cudaStream_t user = (cudaStream_t)cuda_stream, main = h->main_stream;
     if (h->launched) cudaEventSynchronize(h->ev[2]);      // E_pinned of the previous call is free again
     if (h->upload_consumed) { h->upload_pending = false; h->upload_consumed = false; }   // that solve saw the whole upload
-    memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
+    if ((const void*)E_host != (const void*)h->E_pinned) memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
+    {   // A = E S - H is Hermitian when every energy is real
+        bool all_real = true;
+        for (int e = 0; e < h->n_energy; e++) all_real = all_real && (E_host[e].im == 0.0);
+        int mode = all_real ? h->hermitian : 0;
+        if (mode == 2 && h->bs > LEAF2_TPB * LEAF2_MAXC) mode = 1;
+        if (h->force_general) mode = 0;
+        h->mode = mode;
+        if (!h->force_general) h->retried = 0;
+    }
+    h->last_args = {Sigma_L, Sigma_R, Inj_first, Inj_last, X, nrhs, cuda_stream};
     h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
     // the solve runs on a stream of the handle, ordered after the caller's stream and joined back to it
     cudaEventRecord(h->ev_in, user);
@@ -559,14 +618,36 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
 }
 
 static ss_status_t check_info(ss_handle_t h) {
-    const int n = 3 * h->n_energy;
+    const int nE = h->n_energy, n = 5 * nE;
     int* host = (int*)malloc(sizeof(int) * (size_t)n);
     if (!host) return SS_ERR_ALLOC;
     cudaError_t e = cudaMemcpy(host, h->info, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost);
     ss_status_t st = SS_OK;
+    bool grown = false;
     if (e != cudaSuccess) { cudaGetLastError(); st = SS_ERR_CUDA; }
-    else for (int i = 0; i < n; i++) if (host[i] != 0) { st = SS_ERR_SINGULAR; break; }
+    else {
+        for (int i = 0; i < 3 * nE; i++) if (host[i] != 0) { st = SS_ERR_SINGULAR; break; }
+        if (h->mode == 2) {
+            const float lim = (float)h->growth_limit;
+            for (int i = 3 * nE; i < n; i++) {
+                float g; memcpy(&g, &host[i], sizeof(float));
+                if (!(g <= lim)) grown = true;
+            }
+        }
+    }
     free(host);
+    if (st != SS_ERR_CUDA && h->mode == 2 && (grown || st == SS_ERR_SINGULAR) && !h->force_general) {
+        // the no-pivot L Delta L^H met a multiplier above the limit (or a zero pivot): its results are discarded and the
+        // whole solve is redone on the general path (mode 0), same arguments, same stream
+        h->force_general = true;
+        h->retried = 1;
+        ss_status_t s2 = ss_solve(h, (const ss_cplx*)h->E_pinned, h->last_args.sl, h->last_args.sr, h->last_args.i1,
+                                  h->last_args.i2, h->last_args.nrhs, h->last_args.x, h->last_args.stream);
+        h->force_general = false;
+        if (s2 != SS_OK) return s2;
+        if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+        return check_info(h);
+    }
     return st;
 }
 
@@ -581,10 +662,12 @@ extern "C" ss_status_t ss_transmission(ss_handle_t h, double* T_host) {
     if (!h || !T_host) return SS_ERR_INVALID_ARG;
     if (!h->solved || !h->want_T) return SS_ERR_NOT_READY;
     if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    ss_status_t st = check_info(h);                       // may redo the solve (hermitian mode 2 above its growth limit)
+    if (st == SS_ERR_CUDA || st == SS_ERR_ALLOC) return st;
     if (cudaMemcpy(T_host, h->T_dev, sizeof(double) * (size_t)h->n_energy, cudaMemcpyDeviceToHost) != cudaSuccess) {
         cudaGetLastError(); return SS_ERR_CUDA;
     }
-    return check_info(h);
+    return st;
 }
 
 extern "C" ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int* column) {
@@ -730,6 +813,11 @@ extern "C" ss_status_t ss_solve_host(ss_handle_t h, const ss_cplx* E_host, const
                              (nrhs && Inj2) ? (ss_cplx*)h->hp_inj2 : nullptr, nrhs, nrhs ? (ss_cplx*)h->hp_x : nullptr, st);
     h->post_wait = false;
     if (s != SS_OK) return s;
+    if (h->mode == 2) {                                   // the no-pivot path may be redone: decide before downloading
+        if (cudaStreamSynchronize(st) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+        ss_status_t c = check_info(h);
+        if (c == SS_ERR_CUDA || c == SS_ERR_ALLOC) return c;
+    }
     if (X_host && nrhs > 0 && cudaMemcpyAsync(X_host, h->hp_x, x_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) {
         cudaGetLastError(); return SS_ERR_CUDA;
     }
@@ -757,7 +845,7 @@ extern "C" ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const
 
 extern "C" size_t ss_lu_workspace_bytes(int n, int batch) {
     if (n < 1 || batch < 1) return 0;
-    return lu_tinv_elems(n, batch) * sizeof(cplx);
+    return (lu_tinv_elems(n, batch) + (size_t)lu_tmp_elems_default(n) * batch) * sizeof(cplx) + lu_perm_ints(n, batch) * sizeof(int);
 }
 
 static ss_status_t lu_common(int n, int nrhs_solve, int ncols, ss_cplx* AB, int ld, long long stride, ss_cplx* X, int ldx,
@@ -768,6 +856,8 @@ static ss_status_t lu_common(int n, int nrhs_solve, int ncols, ss_cplx* AB, int 
     cudaStream_t st = (cudaStream_t)stream;
     LuWork w;
     w.tinv = (cplx*)work; w.ipiv = ipiv; w.ipiv_stride = n; w.info = info;
+    w.tmp = w.tinv + lu_tinv_elems(n, batch); w.tmp_elems = lu_tmp_elems_default(n);
+    w.perm = (int*)(w.tmp + (size_t)w.tmp_elems * batch);
     Ctx ctx; ctx.st = st; ctx.variant = g_default_variant;
     cudaMemsetAsync(info, 0, sizeof(int) * (size_t)batch, st);
     BPtr Ab = bp_strided((cplx*)AB, stride);
@@ -865,3 +955,12 @@ extern "C" ss_status_t ss_fp64_peak_tflops(double ms, double* tflops) {
     *tflops = best;
     return SS_OK;
 }
+
+#ifdef SS_PANEL_TIMING
+extern "C" int ss_debug_panel_clocks(long long* out16, int reset) {
+    cudaDeviceSynchronize();
+    if (out16 && cudaMemcpyFromSymbol(out16, ss_panel_clk, sizeof(long long) * 16) != cudaSuccess) return 1;
+    if (reset) { long long z[16] = {0}; cudaMemcpyToSymbol(ss_panel_clk, z, sizeof(z)); }
+    return 0;
+}
+#endif

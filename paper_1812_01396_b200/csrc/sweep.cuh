@@ -67,6 +67,33 @@ form_kernel(FormSide s0, FormSide s1, const cplx* __restrict__ E, BPtr dst, int 
     }
 }
 
+// SURVEY.md 8(f1) (A Hermitian at real E): mirror of a block across the diagonal of a batch matrix.
+// Source S = A[rs .. rs+nr) x [cs .. cs+nc) (below or on the diagonal), destination its mirror image:
+//     A[cs + k][rs + r] = f_k * conj(A[rs + r][cs + k]),   f_k = A[cs+k][cs+k] if scaled (U12 = Delta * L21^H of an LDL^H), else 1;
+// strict: only r > k is written (source and destination are the same diagonal block).  Tiles through shared memory so that
+// both the reads and the writes are coalesced.
+__global__ void __launch_bounds__(256)
+herm_mirror_kernel(BPtr Ab, int ld, int rs, int cs, int nr, int nc, int scaled, int strict) {
+    __shared__ cplx tile[32][33];
+    cplx* __restrict__ A = bptr(Ab, blockIdx.z);
+    const int r0 = blockIdx.y * 32, k0 = blockIdx.x * 32;        // tile of the SOURCE block: rows r0.., columns k0..
+    if (strict && k0 > r0 + 31) return;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;      // 32 x 8
+    for (int rr = ty; rr < 32; rr += 8) {
+        int r = r0 + rr, k = k0 + tx;
+        tile[rr][tx] = (r < nr && k < nc) ? A[(long long)(rs + r) * ld + cs + k] : make_c(0.0, 0.0);
+    }
+    __syncthreads();
+    for (int kk = ty; kk < 32; kk += 8) {
+        int k = k0 + kk, r = r0 + tx;
+        if (k < nc && r < nr && (!strict || r > k)) {
+            cplx v = cconj(tile[tx][kk]);
+            if (scaled) v = cmul(A[(long long)(cs + k) * ld + cs + k], v);
+            A[(long long)(cs + k) * ld + rs + r] = v;
+        }
+    }
+}
+
 // Raug[e] : 2bs x W row-major (leading dimension ld >= W), W = 2bs + m + bs:  [ 1_{2bs} | Inj_first ; Inj_last | 0 ; 1_bs ]
 __global__ void __launch_bounds__(256)
 corner_init_kernel(cplx* __restrict__ Raug, long long stride, int W, int ld, int bs, int m, const cplx* __restrict__ inj_first,

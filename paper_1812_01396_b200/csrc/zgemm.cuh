@@ -31,6 +31,9 @@ struct GemmArgs {
     BPtr S; BPtr H; int lds;   // EPI_SCHUR: C = (E[z>>1]*S - H) - acc   (a0 fused into a1's epilogue)
     const cplx* E;
     int tiles_m, tiles_n;
+    // tri != 0: only the tiles that touch the lower triangle are computed (Hermitian updates): element
+    // (i, j) of C is at global position (tri_row0 + i, tri_col0 + j); a tile whose every column lies right of its last row is skipped
+    int tri, tri_row0, tri_col0;
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
@@ -88,6 +91,7 @@ __global__ void __launch_bounds__(Cfg::NT, MINB) zgemm_kernel(const GemmArgs p) 
     }
     const int m0 = tile_m * BM, n0 = tile_n * BN;
     const int M = p.M, N = p.N, K = p.K;
+    if (p.tri && (n0 + p.tri_col0) > (m0 + BM - 1 + p.tri_row0)) return;
 
     const cplx* __restrict__ Ag = bptr(p.A, z);
     const cplx* __restrict__ Bg = bptr(p.B, z);

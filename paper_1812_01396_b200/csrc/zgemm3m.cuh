@@ -66,6 +66,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
     }
     const int m0 = tile_m * BM, n0 = tile_n * BN;
     const int M = p.M, N = p.N, K = p.K;
+    if (p.tri && (n0 + p.tri_col0) > (m0 + BM - 1 + p.tri_row0)) return;
 
     const cplx* __restrict__ Ag = bptr(p.A, z);
     const cplx* __restrict__ Bg = bptr(p.B, z);

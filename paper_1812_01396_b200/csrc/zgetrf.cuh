@@ -20,8 +20,10 @@
 //   Back substitution (left-looking, block rows of NB): T_j = Y_j - U_{j,>j} X_{>j} (GEMM), X_j = U_jj^-1 T_j (GEMM).
 #pragma once
 #include <cooperative_groups.h>
+#include <cstddef>
 #include <vector>
 #include "zgemm3m.cuh"
+#include "sweep.cuh"
 
 namespace ss {
 namespace cg = cooperative_groups;
@@ -163,10 +165,15 @@ lu_leaf_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restri
 constexpr int LEAF2_TPB = 256;
 constexpr int LEAF2_MAXC = 16;
 
+// 1 / a.  |a|^2 in the normal range: hardware reciprocal approximation (rcp.approx.ftz.f64, ~2^-23) + two Newton steps
+// (relative error ~1 ulp: ample for a pivot reciprocal), no IEEE division on the critical path of a pivot step
 __device__ __forceinline__ cplx crecip_fast(cplx a) {
     double n = fma(a.re, a.re, a.im * a.im);
     if (n > 1e-280 && n < 1e280) {
-        double r = 1.0 / n;
+        double r;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(n));
+        r = fma(r, fma(-n, r, 1.0), r);
+        r = fma(r, fma(-n, r, 1.0), r);
         return make_c(a.re * r, -a.im * r);
     }
     return crecip(a);
@@ -294,35 +301,92 @@ lu_leaf3_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restr
     }
 }
 
+// ---- cluster-scope mbarrier / distributed-shared-memory primitives of the fused panel kernel
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned mapa_cluster(unsigned local, int cta) {
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(cta));
+    return r;
+}
+__device__ __forceinline__ void mbar_init(unsigned bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// 16 bytes into another CTA's shared memory; the store itself completes 16 transaction bytes on that CTA's mbarrier
+// (no fence, no barrier: the receiver's mbarrier wait is the only synchronisation)
+__device__ __forceinline__ void st_async_16(unsigned remote_addr, unsigned long long a, unsigned long long b, unsigned remote_bar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];"
+                 ::"r"(remote_addr), "l"(a), "l"(b), "r"(remote_bar) : "memory");
+}
+
 // ---- the whole 128-column panel in ONE launch (panels of up to 4096 rows): the thread-block cluster stays resident over
 // the 8 inner blocks of 16 columns instead of being re-scheduled for every one of them (4 launches per inner block before:
 // leaf, row swaps, 16-row triangular solve, rank-16 update).  One thread = one matrix row for the whole panel; pivoting is
-// IMPLICIT for the whole panel (no row moves until the end), with the same position bookkeeping as the leaf kernel.
-// Per inner block:  (1) the 16 active columns of the own row -> registers;  (2) 16 pivot steps exactly as in
-// lu_leaf3_kernel (redux arg-max, key exchange through distributed shared memory, one cluster barrier, winner row pulled);
-// every CTA keeps the 16 pivot rows' active entries (L11 \ U11) and their physical row numbers;  (3) the pivot rows'
-// remaining panel columns are read by every CTA, U12 = L11^-1 A12 is solved redundantly in shared memory (one thread per
-// column), the owners write it back;  (4) rank-16 update of the own row's remaining panel columns with the multipliers
-// still in registers.  At the end the rows that moved (at most 2 x 128) are carried to their final positions, 16 columns at
-// a time through registers with a cluster barrier between the reads and the writes of a chunk.
+// IMPLICIT for the whole panel (no row moves until the end), with the position bookkeeping of LAPACK's sequential swaps.
+// Per inner block:
+//  (1) the 16 active columns of the own row -> registers;
+//  (2) 16 pivot steps WITHOUT any CTA or cluster barrier: every warp finds its candidate (three redux.sync on the bit
+//      pattern of |re|+|im| and the position), leaves the candidate row in its CTA's shared memory, and lane c pushes the
+//      16-byte key into CTA c's shared memory (st.shared::cluster) followed by an mbarrier arrive with release semantics
+//      at cluster scope; every thread waits on its own CTA's mbarrier (8 warps x csize arrivals per step, acquire at
+//      cluster scope), every warp reduces the keys, pulls the winning row out of the winner CTA's shared memory
+//      (ld.shared::cluster) and applies the rank-1 update to the rows in its registers.  Candidate rows and keys are
+//      double-buffered by step parity: a warp can be at most one step ahead of the slowest warp of the cluster, because
+//      the barrier of step j+1 cannot complete without that warp's arrival.
+//  (3) the pivot rows' remaining panel columns are read by every CTA, U12 = L11^-1 A12 is solved redundantly in shared
+//      memory (one thread per column), the owners write it back;
+//  (4) rank-16 update of the own row's remaining panel columns with the multipliers still in registers (four columns
+//      per trip, the next four prefetched).
+// At the end the rows that moved (at most 2 x 128) are carried to their final positions, 16 columns at a time through
+// registers with a cluster barrier between the reads and the writes of a chunk.
 constexpr int PANEL_W = 128;
+constexpr int PANEL_DYN_SMEM = (LEAF2_TPB / 32) * LEAF_JB * 32 * (int)sizeof(cplx);   // Lsm: 64 KB
+
+#ifdef SS_PANEL_TIMING
+__device__ long long ss_panel_clk[16];                    // tuning aid: accumulated clock64 deltas of CTA 0, thread 0, matrix 0
+#define PCLK_BEGIN long long pclk_t = clock64(); long long pclk_acc[11] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+#define PCLK(i) { long long t1 = clock64(); pclk_acc[i] += t1 - pclk_t; pclk_t = t1; }
+#define PCLK_END if (tid == 0 && crank == 0 && z == 0) { for (int i = 0; i < 11; i++) ss_panel_clk[i] += pclk_acc[i]; }
+#else
+#define PCLK_BEGIN
+#define PCLK(i)
+#define PCLK_END
+#endif
 
 __global__ void __launch_bounds__(LEAF2_TPB, 2)
 lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv, int ipiv_stride,
-                int* __restrict__ info, int info_base) {
+                int* __restrict__ info, int info_base, int nopiv, int* __restrict__ growth) {
     cg::cluster_group cluster = cg::this_cluster();
     const int csize = (int)cluster.num_blocks();
     const int crank = (int)cluster.block_rank();
     const int z = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = LEAF2_TPB / 32, JB = LEAF_JB;
+    double lmax = 0.0;                                    // nopiv: largest multiplier met (growth monitor)
 
-    __shared__ __align__(16) LeafCand wcand[2][NW];
-    __shared__ __align__(16) LeafKey keys[2][LEAF2_MAXC];
-    __shared__ __align__(16) cplx prow[JB];
-    __shared__ __align__(16) cplx Lpiv[JB][JB];          // row k: the k-th pivot row's active entries (multipliers | U)
-    __shared__ int piv_phys[JB];                          // its physical row inside the panel
+    constexpr int MSG = JB + 2;                                        // pivot-row message: 16 entries, 1/pivot, {physical row}
+    __shared__ __align__(16) ulonglong2 keys[2][NW * LEAF2_MAXC];      // [src CTA * NW + src warp]: {value bits, position}
+    __shared__ __align__(16) cplx rowmsg[2][MSG];                      // the winner's row, pushed by its warp
+    __shared__ __align__(16) cplx wstage[NW][MSG];                     // every warp's candidate, staged for that push
+    __shared__ __align__(16) cplx Lpiv[JB][JB];                        // row k: the k-th pivot row's active entries (multipliers | U)
+    __shared__ int piv_phys[JB];                                       // its physical row inside the panel
     __shared__ __align__(16) cplx U12[JB][PANEL_W - JB];
+    __shared__ __align__(8) unsigned long long bars[4];                // [0..1] keys of even / odd steps, [2..3] row messages
+    extern __shared__ __align__(16) unsigned char panel_dyn[];
+    cplx* Lsm = reinterpret_cast<cplx*>(panel_dyn);                    // [NW][JB][32] multipliers of the warp's rows
 
     cplx* A = bptr(Ab, z) + (long long)j0 * ld + j0;      // no __restrict__/const: other CTAs write rows this CTA reads
     const int r = crank * LEAF2_TPB + tid;                // my (physical) row inside the panel
@@ -332,80 +396,142 @@ lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv,
     bool done = !valid;
     int final_pos = r;
 
+    const unsigned bars_a = smem_addr(bars);
+    if (tid == 0) {
+        for (int i = 0; i < 4; i++) mbar_init(bars_a + 8u * i, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cluster.sync();
+    const int nkeys = NW * csize;
+    const int dest = lane & (LEAF2_MAXC - 1), half = lane >> 4;        // lane -> (destination CTA, half of a message)
+    const unsigned r_bars = mapa_cluster(bars_a, dest < csize ? dest : 0);
+    const unsigned r_keys = mapa_cluster(smem_addr(&keys[0][crank * NW + warp]), dest < csize ? dest : 0);
+    const unsigned r_rowmsg = mapa_cluster(smem_addr(&rowmsg[0][0]), dest < csize ? dest : 0);
+
+    PCLK_BEGIN
     for (int c = 0; c < nbw; c += JB) {
         const int jb = min(JB, nbw - c), wrest = nbw - c - jb;
         cplx a[JB];
 #pragma unroll
         for (int k = 0; k < JB; k++) a[k] = (valid && k < jb) ? Arow[c + k] : make_c(0.0, 0.0);
+        PCLK(0)
+        // Pivot steps, software-pipelined: after the pivot row of step j has arrived, only column j+1 of the own row is
+        // updated before the arg-max of step j+1 starts; the rest of step j's rank-1 update (columns j+2 ..) and the staging
+        // of the candidate row run while the keys of step j+1 are in flight.
+        bool pend = false; cplx lp = make_c(0.0, 0.0);    // deferred part of the previous step's update: a[k] -= lp * pp[k]
+        const cplx* pp = rowmsg[0];
 #pragma unroll
         for (int j = 0; j < JB; j++) {
             if (j < jb) {
                 const int q = c + j;                      // pivot step = position inside the panel
                 const int par = j & 1;
+                const unsigned ph = (unsigned)(q >> 1) & 1u;
+                if (tid == 0) {                           // this step's transaction bytes: csize * NW keys, one row message
+                    mbar_expect_tx(bars_a + 8u * par, 16u * (unsigned)nkeys);
+                    mbar_expect_tx(bars_a + 8u * (2 + par), 16u * MSG);
+                }
                 double wv; int wp;
-                const double myv = done ? -1.0 : (fabs(a[j].re) + fabs(a[j].im));
-                if (warp_argmax(myv, cur_pos, wv, wp)) {
-                    LeafCand* cd = &wcand[par][warp];
-                    cd->val = myv; cd->pos = cur_pos; cd->pad = r;
+                const double myv = done ? -1.0 : (nopiv ? (cur_pos == q ? (fabs(a[j].re) + fabs(a[j].im)) : -1.0)
+                                                        : (fabs(a[j].re) + fabs(a[j].im)));
+                const bool iwin = warp_argmax(myv, cur_pos, wv, wp);
+                if (lane < csize) {
+                    const unsigned long long kb = (wv >= 0.0) ? (unsigned long long)__double_as_longlong(wv) + 1ull : 0ull;
+                    st_async_16(r_keys + (unsigned)(par * sizeof(ulonglong2) * NW * LEAF2_MAXC), kb, (unsigned long long)(unsigned)wp,
+                                r_bars + 8u * par);
+                }
+                if (pend) {                               // the previous step's update, columns j+1 .. (column j went ahead)
 #pragma unroll
-                    for (int k = 0; k < JB; k++) cd->row[k] = a[k];
+                    for (int k = j + 1; k < JB; k++) a[k] = cfnma(a[k], lp, pp[k]);
                 }
-                if (lane == 0 && wv < 0.0) { wcand[par][warp].val = -1.0; wcand[par][warp].pos = 0x7fffffff; wcand[par][warp].pad = 0; }
-                __syncthreads();
+                if (iwin) {                               // stage my row, the pivot's reciprocal and my row number
+                    cplx* st = wstage[warp];
+#pragma unroll
+                    for (int k = 0; k < JB; k++) st[k] = a[k];
+                    st[JB] = crecip_fast(a[j]);
+                    st[JB + 1] = make_c(__longlong_as_double((long long)r), 0.0);
+                }
+                PCLK(1)
+                mbar_wait(bars_a + 8u * par, ph);
+                PCLK(2)
+                // ---- winner among the NW * csize keys: per lane over its keys, then one redux pass
+                unsigned long long bk = 0ull; unsigned bp = 0xffffffffu; int bi = 0;
+                for (int i = lane; i < nkeys; i += 32) {
+                    const ulonglong2 kk = keys[par][i];
+                    const unsigned kp = (unsigned)kk.y;
+                    if (kk.x > bk || (kk.x == bk && kk.x != 0ull && kp < bp)) { bk = kk.x; bp = kp; bi = i; }
+                }
+                const unsigned hi = (unsigned)(bk >> 32), lo = (unsigned)bk;
+                const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+                const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
+                const bool cand = (hi == mh) && (lo == ml);
+                const unsigned mp = __reduce_min_sync(0xffffffffu, cand ? bp : 0xffffffffu);
+                const unsigned long long gk = ((unsigned long long)mh << 32) | ml;
+                const bool have = gk != 0ull;                 // some row is left
+                const bool zero_piv = (gk == 1ull);           // best |value| is exactly 0
+                const unsigned wl = __ballot_sync(0xffffffffu, cand && bp == mp);
+                const int widx = __shfl_sync(0xffffffffu, bi, wl ? (__ffs(wl) - 1) : 0);
+                const int gp = have ? (int)mp : q;
+                // ---- the warp that holds the winner pushes its staged row to every CTA (with no row left: CTA 0's warp 0
+                // pushes zeros, so that the row barrier of the step completes everywhere)
+                const bool pusher = have ? (widx == crank * NW + warp) : (crank == 0 && warp == 0);
+                if (pusher) {
+                    __syncwarp();
+                    if (dest < csize) {
+                        const cplx* st = wstage[warp];
+#pragma unroll
+                        for (int i = 0; i < MSG / 2; i++) {
+                            const int e = half * (MSG / 2) + i;
+                            cplx v = have ? st[e] : make_c(0.0, 0.0);
+                            st_async_16(r_rowmsg + (unsigned)((par * MSG + e) * sizeof(cplx)), (unsigned long long)__double_as_longlong(v.re),
+                                        (unsigned long long)__double_as_longlong(v.im), r_bars + 8u * (2 + par));
+                        }
+                    }
+                }
+                PCLK(3)
+                mbar_wait(bars_a + 8u * (2 + par), ph);
+                PCLK(4)
+                const cplx* prow = rowmsg[par];
                 if (warp == 0) {
-                    double v2 = lane < NW ? wcand[par][lane].val : -1.0;
-                    int p2 = lane < NW ? wcand[par][lane].pos : 0x7fffffff;
-                    double cv; int cp;
-                    bool win = warp_argmax(v2, p2, cv, cp);
-                    unsigned bal = __ballot_sync(0xffffffffu, win);
-                    LeafKey k; k.val = cv; k.pos = cp; k.warp = bal ? (__ffs(bal) - 1) : 0;
-                    if (lane < csize) *cluster.map_shared_rank(&keys[par][crank], lane) = k;
+                    if (lane < JB) Lpiv[j][lane] = prow[lane];
+                    else if (lane == JB) piv_phys[j] = have ? (int)__double_as_longlong(prow[JB + 1].re) : 0;
                 }
-                cluster.sync();
-                double kv = -1.0; int kp = 0x7fffffff, kw = 0;
-                if (lane < csize) { LeafKey k = keys[par][lane]; kv = k.val; kp = k.pos; kw = k.warp; }
-                double gv; int gp;
-                bool gwin = warp_argmax(kv, kp, gv, gp);
-                unsigned gbal = __ballot_sync(0xffffffffu, gwin);
-                const int wcta = gbal ? (__ffs(gbal) - 1) : 0;
-                const int wslot = __shfl_sync(0xffffffffu, kw, wcta);
-                if (warp == 0 && lane < JB) {
-                    const LeafCand* src = cluster.map_shared_rank(&wcand[par][wslot], wcta);
-                    cplx v = (gv >= 0.0) ? src->row[lane] : make_c(0.0, 0.0);
-                    prow[lane] = v;
-                    Lpiv[j][lane] = v;
-                    if (lane == 0) piv_phys[j] = (gv >= 0.0) ? src->pad : 0;
-                }
-                if (gv < 0.0) { gp = q; }                 // no rows left: nothing to do
-                const bool singular = !(gv > 0.0);
+                const bool singular = !have || zero_piv;
                 if (crank == 0 && tid == 0) {
                     ipiv[(long long)z * ipiv_stride + j0 + q] = j0 + gp;
-                    if (singular && gv >= 0.0) atomicCAS(&info[z], 0, info_base + j0 + q + 1);
+                    if (zero_piv) atomicCAS(&info[z], 0, info_base + j0 + q + 1);
                 }
-                __syncthreads();
+                pend = false;
                 if (!done) {
-                    if (cur_pos == gp && gv >= 0.0) {
+                    if (cur_pos == gp && have) {
                         done = true; final_pos = q;       // I am the pivot row: becomes row q of the panel's U
                     } else {
                         if (cur_pos == q) cur_pos = gp;   // LAPACK swap bookkeeping
                         if (!singular) {
-                            cplx rinv = crecip_fast(prow[j]);
-                            cplx l = cmul(a[j], rinv);
+                            cplx l = cmul(a[j], prow[JB]);
                             a[j] = l;
-#pragma unroll
-                            for (int k = j + 1; k < JB; k++) a[k] = cfnma(a[k], l, prow[k]);
+                            if (nopiv) lmax = fmax(lmax, fabs(l.re) + fabs(l.im));
+                            if (j + 1 < JB) a[j + 1] = cfnma(a[j + 1], l, prow[j + 1]);
+                            pend = true; lp = l; pp = prow;
                         }
                     }
                 }
+                PCLK(5)
             }
+        }
+        if (pend) {                                       // jb < 16 only: nothing is left to update when jb == 16
+#pragma unroll
+            for (int k = 0; k < JB; k++)
+                if (k > jb) a[k] = cfnma(a[k], lp, pp[k]);
         }
         if (valid) {
 #pragma unroll
             for (int k = 0; k < JB; k++)
                 if (k < jb) Arow[c + k] = a[k];
         }
+        PCLK(6)
         if (wrest > 0) {
             const int cr = c + jb;                        // first remaining column
+            __syncthreads();                              // Lpiv, piv_phys (written by warp 0) complete
             // A12: the pivot rows' remaining columns (every CTA reads all of them; .cg: written by their owner CTAs)
             for (int idx = tid; idx < jb * wrest; idx += LEAF2_TPB) {
                 int k = idx / wrest, cc = idx - k * wrest;
@@ -413,6 +539,7 @@ lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv,
                 U12[k][cc] = make_c(v.x, v.y);
             }
             cluster.sync();                               // all CTAs have read A12 before any owner overwrites it
+            PCLK(7)
             if (tid < wrest) {                            // U12 = L11^-1 A12 in place, one thread per column
                 for (int k = 1; k < jb; k++) {
                     cplx acc = U12[k][tid];
@@ -426,17 +553,67 @@ lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv,
                 int pr = piv_phys[k];
                 if (pr / LEAF2_TPB == crank) A[(long long)pr * ld + cr + cc] = U12[k][cc];
             }
-            if (valid && !done) {                         // A22 -= L21 U12 on my row (multipliers a[0..jb) in registers)
-                for (int cc = 0; cc < wrest; cc++) {
-                    cplx x = Arow[cr + cc];
+            PCLK(8)
+            // ---- A22 -= L21 U12 on the rows of this warp.  A thread walking along its own row touches 32 different cache
+            // lines per warp instruction (measured: half of the whole panel time went here), so the warp works row-wise
+            // instead: the multipliers go through a per-warp shared-memory tile Lsm[k][lane], then 4 rows at a time, lane
+            // l owns columns l, l+32, l+64, l+96 of each (512-byte coalesced accesses), 4 + 4 shared loads per 16 complex
+            // multiply-adds.
+            {
+                cplx* Lw = Lsm + (size_t)warp * (JB * 32);
 #pragma unroll
-                    for (int k = 0; k < JB; k++)
-                        if (k < jb) x = cfnma(x, a[k], U12[k][cc]);
-                    Arow[cr + cc] = x;
+                for (int k = 0; k < JB; k++) Lw[k * 32 + lane] = a[k];
+                unsigned act = __ballot_sync(0xffffffffu, valid && !done);
+                __syncwarp();
+                cplx* Awarp = A + (long long)(crank * LEAF2_TPB + warp * 32) * ld + cr;
+                while (act) {
+                    int rho[4]; bool on[4];
+#pragma unroll
+                    for (int i = 0; i < 4; i++) {
+                        on[i] = act != 0u;
+                        rho[i] = on[i] ? (__ffs(act) - 1) : 0;
+                        if (on[i]) act &= act - 1u;
+                    }
+                    cplx x[4][4];
+#pragma unroll
+                    for (int i = 0; i < 4; i++)
+#pragma unroll
+                        for (int t = 0; t < 4; t++) {
+                            const int col = lane + 32 * t;
+                            x[i][t] = (on[i] && col < wrest) ? Awarp[(long long)rho[i] * ld + col] : make_c(0.0, 0.0);
+                        }
+#pragma unroll 4
+                    for (int k = 0; k < JB; k++) {
+                        if (k < jb) {
+                            cplx l[4], u[4];
+#pragma unroll
+                            for (int i = 0; i < 4; i++) l[i] = Lw[k * 32 + rho[i]];
+#pragma unroll
+                            for (int t = 0; t < 4; t++) u[t] = U12[k][min(lane + 32 * t, PANEL_W - JB - 1)];
+#pragma unroll
+                            for (int i = 0; i < 4; i++)
+#pragma unroll
+                                for (int t = 0; t < 4; t++) x[i][t] = cfnma(x[i][t], l[i], u[t]);
+                        }
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; i++)
+#pragma unroll
+                        for (int t = 0; t < 4; t++) {
+                            const int col = lane + 32 * t;
+                            if (on[i] && col < wrest) Awarp[(long long)rho[i] * ld + col] = x[i][t];
+                        }
                 }
+                __syncwarp();
             }
             __syncthreads();                              // U12 / Lpiv / piv_phys are rewritten by the next inner block
+            PCLK(9)
         }
+    }
+    if (nopiv && growth) {                                // largest |l| (as |re|+|im|) of the panel -> growth[z] (float bits order like ints)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) lmax = fmax(lmax, __shfl_xor_sync(0xffffffffu, lmax, o));
+        if (lane == 0 && lmax > 0.0) atomicMax(&growth[z], __float_as_int(__double2float_ru(lmax)));
     }
     // ---- carry the moved rows to their final positions
     if (!done) final_pos = cur_pos;
@@ -457,6 +634,8 @@ lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv,
         }
     }
     cluster.sync();                                       // no CTA may exit while another still reads its shared memory
+    PCLK(10)
+    PCLK_END
 }
 
 // Apply the row interchanges ipiv[row0 .. row0+jb) to the columns [c_lo, skip_lo) U [skip_hi, c_hi) of each matrix.
@@ -481,6 +660,66 @@ laswp_kernel(BPtr Ab, int ld, int c_lo, int c_hi, int row0, int jb, int skip_lo,
             *x = ty; *y = tx;
         }
     }
+}
+
+// ---- row interchanges as a permutation.  A pivot list of p entries applied swap by swap costs p dependent
+// read-modify-write trips per column thread (latency-bound: the recursive LU applies up to n/2 pivots to a sibling half at
+// once).  Instead: one small kernel turns ipiv[piv_lo .. piv_lo+npiv) into the permutation it amounts to (rowsrc[r] = the
+// row whose content ends up in row r, plus the compact list of rows that move), then the moved rows are copied through a
+// scratch buffer by two fully parallel, coalesced kernels (gather, scatter).
+__global__ void __launch_bounds__(256)
+perm_build_kernel(const int* __restrict__ ipiv, int ipiv_stride, int piv_lo, int npiv, int n,
+                  int* __restrict__ rowsrc, int* __restrict__ moves, int* __restrict__ count) {
+    extern __shared__ int perm_sh[];                  // idx[n - piv_lo], piv[npiv], counter
+    const int z = blockIdx.x, nrows = n - piv_lo;
+    int* idx = perm_sh;
+    int* piv = perm_sh + nrows;
+    int* cnt = piv + npiv;
+    for (int i = threadIdx.x; i < nrows; i += blockDim.x) idx[i] = i;
+    for (int j = threadIdx.x; j < npiv; j += blockDim.x) piv[j] = ipiv[(long long)z * ipiv_stride + piv_lo + j] - piv_lo;
+    if (threadIdx.x == 0) *cnt = 0;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int j = 0; j < npiv; j++) {
+            const int p = piv[j];
+            if (p != j) { int t = idx[j]; idx[j] = idx[p]; idx[p] = t; }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < nrows; i += blockDim.x) {
+        rowsrc[(long long)z * n + piv_lo + i] = piv_lo + idx[i];
+        if (idx[i] != i) {
+            int k = atomicAdd(cnt, 1);
+            moves[((long long)z * n + k) * 2] = piv_lo + i;             // destination row
+            moves[((long long)z * n + k) * 2 + 1] = piv_lo + idx[i];    // source row
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) count[z] = *cnt;
+}
+
+// dir 0: tmp[a][c] = A[src(a)][c_lo + c];  dir 1: A[dst(a)][c_lo + c] = tmp[a][c];  a = blockIdx.y-th moved row
+__global__ void __launch_bounds__(256)
+row_move_kernel(BPtr Ab, int ld, int c_lo, int ncols, int n, const int* __restrict__ moves, const int* __restrict__ count,
+                cplx* __restrict__ tmp, long long tmp_stride, int dir) {
+    const int z = blockIdx.z, a = blockIdx.y;
+    if (a >= count[z]) return;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncols) return;
+    const int row = moves[((long long)z * n + a) * 2 + (dir ? 0 : 1)];
+    cplx* A = bptr(Ab, z) + (long long)row * ld + c_lo + c;
+    cplx* t = tmp + (long long)z * tmp_stride + (long long)a * ncols + c;
+    if (dir) *A = *t; else *t = *A;
+}
+
+// dst[r][c] = src[rowsrc[r]][c] for all n rows (out of place): the right-hand-side block formed elsewhere, permuted on the way in
+__global__ void __launch_bounds__(256)
+row_gather_ext_kernel(BPtr Dst, int ldd, BPtr Src, int lds, int ncols, int n, const int* __restrict__ rowsrc) {
+    const int z = blockIdx.z, r = blockIdx.y;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncols) return;
+    const int sr = rowsrc[(long long)z * n + r];
+    bptr(Dst, z)[(long long)r * ldd + c] = bptr(Src, z)[(long long)sr * lds + c];
 }
 
 // A12 <- L11^-1 A12 for the jb x w block right of a leaf (L11 = unit lower jb x jb at (row0, row0), jb <= 16).
@@ -708,7 +947,15 @@ static void gemm_run(Ctx& ctx, const GemmArgs& g, int batch, int cfg, int epi) {
         ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st, ctx.variant));
         cudaEventRecord(pr->ev[pr->used + 1], ctx.st);
         pr->used += 2;
-        pr->flops += 8.0 * g.M * g.N * g.K * batch;
+        double area = (double)g.M * g.N;
+        if (g.tri) {                                      // only the tiles that touch the lower triangle are computed
+            const int BM = 64, BN = (ctx.variant == GV_4M) ? 64 : 32;
+            area = 0.0;
+            for (int m0 = 0; m0 < g.M; m0 += BM)
+                for (int n0 = 0; n0 < g.N; n0 += BN)
+                    if (n0 + g.tri_col0 <= m0 + BM - 1 + g.tri_row0) area += (double)min(BM, g.M - m0) * min(BN, g.N - n0);
+        }
+        pr->flops += 8.0 * area * g.K * batch;
         pr->launches++;
     } else {
         ctx.note(gemm_launch(g, batch, cfg, epi, ctx.st, ctx.variant));
@@ -720,9 +967,15 @@ struct LuWork {
     int* ipiv = nullptr;        // [batch][ipiv_stride]
     int ipiv_stride = 0;
     int* info = nullptr;        // [batch]
+    int* growth = nullptr;      // [batch] no-pivot factorisation: float bits of the largest multiplier (|re|+|im|) met
+    int* perm = nullptr;        // [batch][3 n + 4] ints: rowsrc [batch][n], moves [batch][2n], count [batch]
+    cplx* tmp = nullptr;        // [batch][tmp_elems] scratch of the row moves
+    long long tmp_elems = 0;    // per matrix
 };
 static inline int lu_nblk(int n) { return (n + 127) / 128; }
 static inline size_t lu_tinv_elems(int n, int batch) { return (size_t)2 * lu_nblk(n) * 128 * 128 * (size_t)batch; }
+static inline size_t lu_perm_ints(int n, int batch) { return ((size_t)batch * (3 * (size_t)n + 1) + 3) / 4 * 4; }
+static inline long long lu_tmp_elems_default(int n) { return (long long)n * (((n + 1) / 2 + 127) / 128 * 128); }
 
 static inline GemmArgs gemm_std(int M, int N, int K, double alpha, BPtr A, int lda, BPtr B, int ldb, double beta,
                                 BPtr C, int ldc) {
@@ -785,20 +1038,61 @@ struct LuCall {
     BPtr tinvU(int blk) const { return bp_strided(w.tinv + (long long)(nblk() + blk) * 128 * 128, 2LL * nblk() * 128 * 128); }
 };
 
+static void lu_perm_build(const LuCall& L, int piv_lo, int piv_hi) {
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(perm_build_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        configured = true;
+    }
+    const int n = L.n, npiv = piv_hi - piv_lo;
+    int* rowsrc = L.w.perm;
+    int* moves = rowsrc + (long long)L.batch * n;
+    int* count = moves + 2LL * L.batch * n;
+    const size_t sh = sizeof(int) * ((size_t)(n - piv_lo) + npiv + 1);
+    perm_build_kernel<<<L.batch, 256, sh, L.ctx.st>>>(L.w.ipiv, L.w.ipiv_stride, piv_lo, npiv, n, rowsrc, moves, count);
+    L.ctx.note(cudaGetLastError());
+}
+
+// Apply the interchanges ipiv[piv_lo .. piv_hi) to the columns [c_lo, skip_lo) U [skip_hi, c_hi).
 static void lu_swaps(const LuCall& L, int piv_lo, int piv_hi, int c_lo, int c_hi, int skip_lo, int skip_hi) {
     const int total = (skip_lo - c_lo) + (c_hi - skip_hi);
-    if (total <= 0 || piv_hi <= piv_lo) return;
-    dim3 grid((unsigned)((total + 255) / 256), (unsigned)L.batch);
-    laswp_kernel<<<grid, 256, 0, L.ctx.st>>>(L.Ab, L.ld, c_lo, c_hi, piv_lo, piv_hi - piv_lo, skip_lo, skip_hi, L.w.ipiv, L.w.ipiv_stride);
-    L.ctx.note(cudaGetLastError());
+    const int npiv = piv_hi - piv_lo;
+    if (total <= 0 || npiv <= 0) return;
+    if (npiv <= 32 || !L.w.perm || !L.w.tmp) {                 // short list: swap by swap
+        dim3 grid((unsigned)((total + 255) / 256), (unsigned)L.batch);
+        laswp_kernel<<<grid, 256, 0, L.ctx.st>>>(L.Ab, L.ld, c_lo, c_hi, piv_lo, npiv, skip_lo, skip_hi, L.w.ipiv, L.w.ipiv_stride);
+        L.ctx.note(cudaGetLastError());
+        return;
+    }
+    lu_perm_build(L, piv_lo, piv_hi);
+    const int n = L.n;
+    const int* moves = L.w.perm + (long long)L.batch * n;
+    const int* count = moves + 2LL * L.batch * n;
+    const int cap = min(2 * npiv, n - piv_lo);                 // rows that can move
+    const int ranges[2][2] = {{c_lo, skip_lo}, {skip_hi, c_hi}};
+    for (int q = 0; q < 2; q++) {
+        long long chunk = L.w.tmp_elems / cap;
+        if (chunk >= 32) chunk = chunk / 32 * 32;
+        if (chunk < 1) chunk = 1;
+        for (int c0 = ranges[q][0]; c0 < ranges[q][1]; c0 += (int)chunk) {
+            const int nc = (int)min((long long)(ranges[q][1] - c0), chunk);
+            dim3 grid((unsigned)((nc + 255) / 256), (unsigned)cap, (unsigned)L.batch);
+            for (int dir = 0; dir < 2; dir++) {
+                row_move_kernel<<<grid, 256, 0, L.ctx.st>>>(L.Ab, L.ld, c0, nc, n, moves, count, L.w.tmp, L.w.tmp_elems, dir);
+                L.ctx.note(cudaGetLastError());
+            }
+        }
+    }
 }
 
 static int g_panel_fused = 1;        // 1: lu_panel_kernel for panels of up to 4096 rows; 0: always the per-16-column launches
 
-static void launch_panel_fused(Ctx& ctx, BPtr Ab, int ld, int j0, int m, int nbw, const LuWork& w, int info_base, int batch) {
+static void launch_panel_fused(Ctx& ctx, BPtr Ab, int ld, int j0, int m, int nbw, const LuWork& w, int info_base, int batch,
+                               int nopiv = 0) {
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(lu_panel_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        cudaFuncSetAttribute(lu_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, PANEL_DYN_SMEM);
         configured = true;
     }
     int need = (m + LEAF2_TPB - 1) / LEAF2_TPB, csize = 1;
@@ -806,7 +1100,7 @@ static void launch_panel_fused(Ctx& ctx, BPtr Ab, int ld, int j0, int m, int nbw
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)csize, (unsigned)batch, 1);
     cfg.blockDim = dim3((unsigned)LEAF2_TPB, 1, 1);
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = PANEL_DYN_SMEM;
     cfg.stream = ctx.st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -815,7 +1109,7 @@ static void launch_panel_fused(Ctx& ctx, BPtr Ab, int ld, int j0, int m, int nbw
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    ctx.note(cudaLaunchKernelEx(&cfg, lu_panel_kernel, Ab, ld, j0, m, nbw, w.ipiv, w.ipiv_stride, w.info, info_base));
+    ctx.note(cudaLaunchKernelEx(&cfg, lu_panel_kernel, Ab, ld, j0, m, nbw, w.ipiv, w.ipiv_stride, w.info, info_base, nopiv, w.growth));
 }
 
 // Panel of nbw <= 128 columns at (j0, j0), rows j0 .. n-1, swaps applied inside the panel only; then the inverse of its
@@ -892,14 +1186,77 @@ static void lu_recursive(const LuCall& L, int c0, int c1) {
     lu_swaps(L, mid, c1, c0, mid, mid, mid);
 }
 
-static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, const LuWork& w, int info_base) {
+// Bext (optional): the right-hand-side block lives elsewhere ((n x (ncols - n)), leading dimension ldb) and is copied into
+// columns [n, ncols) with the rows already permuted, instead of being swapped in place.
+static void lu_factor(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, const LuWork& w, int info_base,
+                      const BPtr* Bext = nullptr, int ldb = 0) {
     LuCall L{ctx, Ab, ld, n, ncols, batch, w, info_base};
     lu_recursive(L, 0, n);
     if (ncols > n) {
         ctx.use(CLS_HI);
-        lu_swaps(L, 0, n, n, ncols, ncols, ncols);
+        if (Bext && w.perm) {
+            lu_perm_build(L, 0, n);
+            dim3 grid((unsigned)((ncols - n + 255) / 256), (unsigned)n, (unsigned)batch);
+            row_gather_ext_kernel<<<grid, 256, 0, ctx.st>>>(bp_offset(Ab, n), ld, *Bext, ldb, ncols - n, n, w.perm);
+            ctx.note(cudaGetLastError());
+        } else {
+            lu_swaps(L, 0, n, n, ncols, ncols, ncols);
+        }
         lu_trsm_lower(L, 0, n, n, ncols);
     }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Hermitian D (A = E S - H at real E) factored WITHOUT pivoting as L Delta L^H -- the paper's
+// zhesv_nopiv_gpu (L266: 241 -> 228 TFLOP per energy point) -- at half the flops of the LU: only the lower triangle of D
+// is read and updated (lower-triangle-only GEMMs), U = Delta L^H is written into the upper triangle panel by panel, so the
+// result has the same [L \ U] layout as lu_factor (ipiv = identity) and the solves that follow are shared.
+//     rec([c0, c1)):  rec(left half) -> lower(A22) -= L21 U12 (K = width of the left half) -> rec(right half)
+//     panel (<= 128 columns): upper triangle of the diagonal block filled from the lower one; lu_panel_kernel with the
+//     pivot search switched off (the diagonal row is the only candidate), which also records the largest multiplier met
+//     (growth monitor); L11^-1; U12 = Delta L21^H (scaled conjugate transpose of the panel's sub-diagonal part).
+// Panels of more than 4096 rows are not supported here (the caller uses the pivoted LU there).
+// ---------------------------------------------------------------------------------------------------------
+static void launch_mirror(Ctx& ctx, BPtr Ab, int ld, int rs, int cs, int nr, int nc, int scaled, int strict, int batch) {
+    if (nr <= 0 || nc <= 0) return;
+    dim3 grid((unsigned)((nc + 31) / 32), (unsigned)((nr + 31) / 32), (unsigned)batch);
+    herm_mirror_kernel<<<grid, 256, 0, ctx.st>>>(Ab, ld, rs, cs, nr, nc, scaled, strict);
+    ctx.note(cudaGetLastError());
+}
+
+static void herm_recursive(const LuCall& L, int c0, int c1) {
+    Ctx& ctx = L.ctx;
+    const int wd = c1 - c0;
+    if (wd <= 128) {
+        ctx.use(CLS_HI);
+        launch_mirror(ctx, L.Ab, L.ld, c0, c0, wd, wd, 0, 1, L.batch);
+        launch_panel_fused(ctx, L.Ab, L.ld, c0, L.n - c0, wd, L.w, L.info_base, L.batch, 1);
+        TrtriArgs t{};
+        t.T = bp_offset(L.Ab, (long long)c0 * L.ld + c0); t.ld = L.ld; t.t_step = 0; t.n_total = wd;
+        t.out = L.w.tinv + (long long)(c0 / 128) * 128 * 128; t.nblocks = 2 * L.nblk(); t.upper = 0; t.unit = 1;
+        launch_trtri(ctx.st, t, 1, L.batch);
+        ctx.note(cudaGetLastError());
+        launch_mirror(ctx, L.Ab, L.ld, c0 + wd, c0, L.n - c0 - wd, wd, 1, 0, L.batch);
+        return;
+    }
+    const int mid = c0 + ((wd / 2 + 127) / 128) * 128;
+    herm_recursive(L, c0, mid);
+    if (L.n > mid) {
+        GemmArgs u = gemm_std(L.n - mid, c1 - mid, mid - c0, -1.0, bp_offset(L.Ab, (long long)mid * L.ld + c0), L.ld,
+                              bp_offset(L.Ab, (long long)c0 * L.ld + mid), L.ld, 1.0,
+                              bp_offset(L.Ab, (long long)mid * L.ld + mid), L.ld);
+        u.tri = 1; u.tri_row0 = mid; u.tri_col0 = mid;
+        ctx.use(CLS_LO);
+        gemm_run(ctx, u, L.batch, GEMM_BIG, EPI_STD);
+    }
+    herm_recursive(L, mid, c1);
+}
+
+// Same contract as lu_factor for Hermitian leading n x n parts given by their LOWER triangle (n <= 4096); no interchanges.
+static void lu_factor_herm(Ctx& ctx, BPtr Ab, int ld, int n, int ncols, int batch, const LuWork& w, int info_base) {
+    LuCall L{ctx, Ab, ld, n, ncols, batch, w, info_base};
+    herm_recursive(L, 0, n);
+    if (ncols > n) lu_trsm_lower(L, 0, n, n, ncols);
 }
 
 // X = U^-1 Y with U = upper factor in AB[:, 0:n], Y = AB[:, n:n+nrhs] (overwritten).  Left-looking over block rows.

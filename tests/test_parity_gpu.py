@@ -188,11 +188,15 @@ def test_perfect_chain_small_closed_form(lib):
         assert abs(out["T"][e] - 8.0) <= 8.0 * TOL_T
 
 
-def test_config1_perfect_chain_full_size(lib):
-    """BASELINE.json config 1: T(E) = 64 exactly, X_j = e^{ikj} 1; all 64 energies (closed form), 3 vs Tier B."""
+@pytest.mark.parametrize("hermitian", [0, 1, 2])
+def test_config1_perfect_chain_full_size(lib, hermitian):
+    """BASELINE.json config 1: T(E) = 64 exactly, X_j = e^{ikj} 1; all 64 energies (closed form), 3 vs Tier B.  Real
+    energies: run on the general path, with the Hermitian Schur update (the default) and with the no-pivot L Delta L^H
+    (SURVEY.md 8(f1)); the chain's Schur complements are multiples of the identity, so mode 2 must not need its fallback."""
     cfg = inputs.CONFIGS["C1"]
     p = inputs.make_problem(cfg)
-    out = run_gpu(lib, p)
+    out = run_gpu(lib, p, options={"hermitian": hermitian})
+    assert out["ss"].last_mode() == (hermitian, 0)
     k = inputs.chain_wavevector(p.E, -1.0)
     j = np.arange(1, cfg.nb + 1)
     for e in range(cfg.n_energy):
@@ -558,3 +562,70 @@ def test_seeded_sweep_of_sizes_and_options(lib):
                 assert residual.rel_frobenius(Xe, r["X"]) <= TOL_X * f, tag
                 assert residual.backward_error(*a, Xe) <= TOL_BWD * f, tag
         ss.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# structure at real energies
+# ------------------------------------------------------------------------------------------------------
+def _sweep_flops(nb, bs, mode):
+    a1, a2 = (4.0 if mode >= 1 else 8.0), (4.0 / 3.0 if mode == 2 else 8.0 / 3.0)
+    return 2.0 * ((nb - 1) * a1 + nb * a2 + nb * 8.0 + (nb - 1) * 8.0) * bs ** 3
+
+
+@pytest.mark.parametrize("bs,nb,n_e,nrhs", [(16, 8, 4, 4), (150, 4, 3, 20), (300, 3, 2, 33)])
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_hermitian_modes_definite_device(lib, bs, nb, n_e, nrhs, mode):
+    """Real energies ABOVE the spectrum (E in [3.5, 4.5]): A = E S - H is Hermitian positive definite, every Schur
+    complement too, so the no-pivot L Delta L^H (mode 2) is stable and must run without its fallback; all modes meet the
+    north_star tolerances against the dense oracle; the flop count follows the mode."""
+    p = inputs.random_problem(bs, nb, n_e, nrhs, seed=31, e_lo=3.5, e_hi=4.5, eta=0.0, inj_last=True)
+    out = run_gpu(lib, p, options={"hermitian": mode}, want_inverse=True)
+    assert out["ss"].last_mode() == (mode, 0)
+    check_against_oracle(p, out)
+    for e in range(n_e):
+        Q, P = dense.inverse_columns(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+        assert residual.rel_frobenius(out["QP"][e][0], Q) <= TOL_X and residual.rel_frobenius(out["QP"][e][1], P) <= TOL_X
+    assert out["ss"].flops_sweep() == pytest.approx(_sweep_flops(nb, bs, mode), rel=1e-12)
+
+
+@pytest.mark.parametrize("bs,nb", [(16, 8), (130, 4)])
+def test_hermitian_modes_indefinite_device_and_fallback(lib, bs, nb):
+    """Real-energy variant of config 0 (energies inside the band: A indefinite and nearly singular).  The general path
+    (the default) agrees with the oracle at the tolerance real energies allow (the Woodbury split itself loses digits
+    there: 1000x looser).  Modes 1 and 2 symmetrise the Schur complements and lose digits in proportion
+    to kappa(A) there (include/splitsolve.h, option "hermitian"): only their plumbing is checked on this device -- mode 2
+    with a growth limit of 1 must detect the growth, redo the solve on the general path and return exactly its results;
+    with a complex energy in the batch the option is ignored."""
+    p = inputs.random_problem(bs, nb, 4, 5, seed=32, eta=0.0)
+    ref = run_gpu(lib, p)
+    assert ref["ss"].last_mode() == (0, 0)
+    for e in range(4):
+        r = dense.solve_energy(*oracle_args(p, e))
+        assert residual.rel_frobenius(ref["X"][e], r["X"]) <= TOL_X * 1e3
+        assert residual.rel_T(ref["T"][e], r["T_LR"]) <= TOL_T * 1e3
+        assert residual.backward_error(*oracle_args(p, e), ref["X"][e]) <= TOL_BWD * 1e3
+    o1 = run_gpu(lib, p, options={"hermitian": 1})
+    assert o1["ss"].last_mode() == (1, 0) and np.all(np.isfinite(o1["X"]))
+    o2 = run_gpu(lib, p, options={"hermitian": 2, "hermitian_growth_limit": 1})
+    assert o2["ss"].last_mode() == (0, 1)
+    assert np.array_equal(o2["X"], ref["X"]) and np.array_equal(o2["T"], ref["T"])
+    p.E = p.E + 1e-3j * (np.arange(4) == 2)
+    o3 = run_gpu(lib, p, options={"hermitian": 2})
+    assert o3["ss"].last_mode() == (0, 0)
+    check_against_oracle(p, o3, energies=[2])
+
+
+def test_config2_definite_real_energy_variant(lib):
+    """Real-energy variant of BASELINE.json config 2 (bs = 512, same generator, Im E = 0, energies above the spectrum so
+    that A is definite), shortened to 8 blocks and 4 energies: general path, Hermitian Schur update and no-pivot
+    L Delta L^H (four panels per block, two recursion levels) against the residual on every energy and against Tier B on one."""
+    cfg = inputs.CONFIGS["C2"]
+    p = inputs.random_problem(cfg.bs, 8, 4, cfg.nrhs, seed=0, e_lo=3.5, e_hi=4.5, eta=0.0, threads=8)
+    rb = banded.solve_energy(*oracle_args(p, 1))
+    for mode in (0, 1, 2):
+        out = run_gpu(lib, p, options={"hermitian": mode})
+        assert out["ss"].last_mode() == (mode, 0)
+        for e in range(4):
+            assert residual.backward_error(*oracle_args(p, e), out["X"][e]) <= TOL_BWD, (mode, e)
+        assert residual.rel_frobenius(out["X"][1], rb["X"]) <= TOL_X
+        assert residual.rel_T(out["T"][1], rb["T_LR"]) <= TOL_T
