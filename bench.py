@@ -71,6 +71,9 @@ def parse():
                     "(library default 4; 1 = single stream)")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=INT", help="extra ss_set_option calls (tuning)")
     ap.add_argument("--trace", default=None, help="write the phase timeline of the last timed step to this CSV")
+    ap.add_argument("--split", default="energy", choices=["energy", "column"], help="N > 1: 'energy' = every rank its own "
+                    "energies (default, SURVEY 8(e)); 'column' = pairs of ranks share their energies, first block column of "
+                    "A^-1 on the even rank, last on the odd one (SURVEY 8(f2), PAPER.md L167)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the second block (C3) of the default C4 line")
@@ -228,10 +231,21 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     from paper_1812_01396_b200 import binding, sharding
 
     nE, bs, nb, m = cfg.n_energy, cfg.bs, cfg.nb, cfg.nrhs
+    column_split = args.split == "column" and world > 1
+    if column_split:
+        # ranks (2j, 2j+1) share the energies of shard j; every rank creates every pair's group
+        if world % 2:
+            raise SystemExit("--split column needs an even number of GPUs")
+        pair_groups = [dist.new_group([2 * j, 2 * j + 1]) for j in range(world // 2)]
+        pair_group = pair_groups[rank // 2]
+        e_world, e_rank = world // 2, rank // 2
+    else:
+        pair_group = None
+        e_world, e_rank = world, rank
     # inputs: same generator as the parity tests; energies sharded round-robin over ranks (weak scaling)
     if cfg.kind == "chain":
-        p = inputs.perfect_chain_problem(bs, nb, nE * world)
-        idx = sharding.energy_indices(nE * world, rank, world)
+        p = inputs.perfect_chain_problem(bs, nb, nE * e_world)
+        idx = sharding.energy_indices(nE * e_world, e_rank, e_world)
         p.E, p.Sigma_L, p.Sigma_R, p.Inj_first = p.E[idx], p.Sigma_L[idx], p.Sigma_R[idx], p.Inj_first[idx]
     else:
         if world > 1 and rank != 0:
@@ -240,8 +254,8 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
                                None, None, None, None)
         else:
             p = inputs.random_problem(bs, nb, 1, 1, seed=cfg.seed, threads=os.cpu_count() or 1)      # H, S only
-        grid = inputs.energy_grid(nE * world, cfg.e_lo, cfg.e_hi, cfg.eta)
-        idx = sharding.energy_indices(nE * world, rank, world)
+        grid = inputs.energy_grid(nE * e_world, cfg.e_lo, cfg.e_hi, cfg.eta)
+        idx = sharding.energy_indices(nE * e_world, e_rank, e_world)
         p.E = grid[idx].copy()
         p.Sigma_L = np.stack([inputs.sigma_block(cfg.seed, int(e), bs, "L") for e in idx])
         p.Sigma_R = np.stack([inputs.sigma_block(cfg.seed, int(e), bs, "R") for e in idx])
@@ -275,8 +289,15 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     ss.set_hamiltonian(devt["H_diag"], devt["H_upper"], devt["S_diag"], devt["S_upper"])
     X = torch.empty((nE, nb * bs, m), dtype=torch.complex128, device="cuda")
 
-    def step():
-        ss.solve(p.E, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None, X)
+    col_T = [None]
+    if column_split:
+        engine = sharding.LibraryColumnEngine(ss, p.E, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None)
+
+        def step():
+            _, col_T[0] = sharding.column_split_solve(engine, rank, group=pair_group)
+    else:
+        def step():
+            ss.solve(p.E, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None, X)
 
     def barrier():
         if world > 1:
@@ -287,7 +308,7 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
         step()
     T_last = ss.transmission()
     sweep_ms, gemm_ms, gemm_fl, gemm_n = [], 0.0, 0.0, 0
-    serial = min(groups, nE) <= 1
+    serial = min(groups, nE) <= 1 or column_split          # column split: no separate per-launch GEMM timing step
     # CUDA events around every GEMM launch.  On a single stream they are taken inside the timed region; with stream
     # groups kernels of different groups overlap, so a launch's event-to-event time is not the kernel's own duration:
     # then the per-launch GEMM timing comes from one extra step with stream_groups = 1, right after the timed region.
@@ -300,8 +321,9 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
         for _ in range(steps):
             step()
             T_last = ss.transmission()               # the step's result: synchronises, 8 B per energy
-            sweep_ms.append(ss.phase_ms(0))
-            if serial:
+            if not column_split:
+                sweep_ms.append(ss.phase_ms(0))
+            if serial and not column_split:
                 a, b, c = ss.gemm_profile()
                 gemm_ms += a; gemm_fl += b; gemm_n += c
         ev1.record()
@@ -323,18 +345,21 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
         ss.set_option("stream_groups", groups)
     ss.set_option("profile_gemm", 0)
     ms_total = sharding.max_over_ranks(ms_total, world, device="cuda")
-    T_all = sharding.gather_transmission(T_last, nE * world, rank, world, device="cuda")   # 8 B per energy
+    if column_split:
+        T_all = T_last                                    # every pair holds its own energies' T(E); no global gather here
+    else:
+        T_all = sharding.gather_transmission(T_last, nE * world, rank, world, device="cuda")   # 8 B per energy
     ms_step = ms_total / steps
-    value = nE * world / (ms_step * 1e-3)
+    value = nE * e_world / (ms_step * 1e-3)
 
     flops_step = ss.flops(m) * nE
     sweep_flops = ss.flops_sweep() * nE
-    sweep_tf = sweep_flops / (np.mean(sweep_ms) * 1e-3) / 1e12
+    sweep_tf = sweep_flops / (np.mean(sweep_ms) * 1e-3) / 1e12 if sweep_ms else 0.0     # column split: not timed separately
     gemm_tf = gemm_fl / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
 
     # ---- e2e: host buffers through the C ABI, H2D of every input and D2H of X and T inside the timed region
     e2e = None
-    if want_e2e:
+    if want_e2e and not column_split:
         Xh = torch.empty((nE, nb * bs, m), dtype=torch.complex128).pin_memory()
         Th = torch.empty(nE, dtype=torch.float64).pin_memory()
 
@@ -364,7 +389,7 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     kern = ("zgemm3m_kernel" if is3m else "zgemm_kernel") + f" [{binding.GEMM_VARIANTS[variant]}] (DMMA.8x8x4, mma.sync f64)"
     out = {
         "value": value, "ms_per_step": ms_step, "steps": steps, "warmup": warmup,
-        "config": config_dict(cfg, world), "launch": {"stream_groups": groups},
+        "config": config_dict(cfg, world), "launch": {"stream_groups": groups, "split": "column pairs" if column_split else "energy"},
         "tflops": {"whole_solve": flops_step / (ms_step * 1e-3) / 1e12, "sweep_a1_a4": sweep_tf,
                    "sweep_executed": sweep_tf * ratio, "sweep_executed_frac_of_fp64_peak": sweep_tf * ratio / FP64_PEAK_NOMINAL_TFLOPS,
                    "flops_per_step": flops_step,

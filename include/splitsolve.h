@@ -50,7 +50,8 @@ typedef enum {
     SS_ERR_NOT_READY = 2,     /* ss_solve before ss_set_hamiltonian, ss_transmission before ss_solve */
     SS_ERR_ALLOC = 3,         /* device or host allocation failed */
     SS_ERR_SINGULAR = 4,      /* an exactly zero pivot was met; see ss_last_info */
-    SS_ERR_CUDA = 5           /* a CUDA runtime call or kernel launch failed */
+    SS_ERR_CUDA = 5,          /* a CUDA runtime call or kernel launch failed */
+    SS_ERR_UNSTABLE = 6       /* split-phase calls with option "hermitian" = 2: the growth limit was exceeded (redo with 0) */
 } ss_status_t;
 
 /* ---- life cycle -------------------------------------------------------------------------------------- */
@@ -101,6 +102,26 @@ ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_
 ss_status_t ss_solve_host(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L_host,
                           const ss_cplx* Sigma_R_host, const ss_cplx* Inj_first_host, const ss_cplx* Inj_last_host,
                           int nrhs, ss_cplx* X_host, double* T_host);
+
+/* ---- one energy batch on two GPUs (computing the first and the last block column of
+ * A^-1 "naturally scale[s] to two accelerators"; L175: z is distributed to all accelerators) --------------------------
+ * GPU 0 runs the first-column sweep, GPU 1 the last-column sweep, each on its own handle with the full H and S:
+ *     ss_sweep_column(h, E, column)                 a0-a4 for that block column only (Q_i resp. P_i, i = 1..nb)
+ *     ss_get_corner_blocks(h, column, out)          out[e][0] = block 1, out[e][1] = block nb of that column
+ *     -- the two GPUs exchange their corner blocks (2 * n_energy * 2 blocks of bs x bs; NCCL / peer copy, caller's job) --
+ *     ss_post_column(h, column, peer_corner, ...)   a5 and a7 redundantly on both GPUs (R needs all four corner blocks and is
+ *                                                   only 2bs x 2bs), a6 for the own column only:
+ *                                                   X_part = Q_i w_top (column 0) resp. P_i w_bot (column 1)
+ *     -- X = X_part(GPU 0) + X_part(GPU 1): one sum-reduction of [n_energy][nb*bs][nrhs] (caller's job) --
+ * ss_transmission / ss_synchronize work as after ss_solve (T(E) is complete on both GPUs).
+ *   column          : 0 = first block column (Q), 1 = last block column (P)
+ *   out_dev / peer_corner_dev : [n_energy][2][bs][bs], caller-owned device memory
+ * Errors as for ss_solve; SS_ERR_NOT_READY if the calls come out of order or for another column than the one swept. */
+ss_status_t ss_sweep_column(ss_handle_t h, const ss_cplx* E_host, int column, void* cuda_stream);
+ss_status_t ss_get_corner_blocks(ss_handle_t h, int column, ss_cplx* out_dev, void* cuda_stream);
+ss_status_t ss_post_column(ss_handle_t h, int column, const ss_cplx* peer_corner_dev, const ss_cplx* Sigma_L_dev,
+                           const ss_cplx* Sigma_R_dev, const ss_cplx* Inj_first_dev, const ss_cplx* Inj_last_dev, int nrhs,
+                           ss_cplx* X_part_dev, void* cuda_stream);
 
 /* Waits for the last ss_solve; returns SS_ERR_SINGULAR if any pivot was exactly zero. */
 ss_status_t ss_synchronize(ss_handle_t h);

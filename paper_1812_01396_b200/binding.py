@@ -13,7 +13,7 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_float, c_int, c_longlon
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(PKG_DIR, "libsplitsolve.so")
 
-SS_OK, SS_ERR_INVALID_ARG, SS_ERR_NOT_READY, SS_ERR_ALLOC, SS_ERR_SINGULAR, SS_ERR_CUDA = range(6)
+SS_OK, SS_ERR_INVALID_ARG, SS_ERR_NOT_READY, SS_ERR_ALLOC, SS_ERR_SINGULAR, SS_ERR_CUDA, SS_ERR_UNSTABLE = range(7)
 
 # every symbol include/splitsolve.h declares: name -> (restype, argtypes)
 SIGNATURES = {
@@ -23,6 +23,9 @@ SIGNATURES = {
     "ss_set_hamiltonian_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "ss_solve": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]),
     "ss_solve_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]),
+    "ss_sweep_column": (c_int, [c_void_p, c_void_p, c_int, c_void_p]),
+    "ss_get_corner_blocks": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
+    "ss_post_column": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]),
     "ss_synchronize": (c_int, [c_void_p]),
     "ss_transmission": (c_int, [c_void_p, c_void_p]),
     "ss_inverse_columns": (c_int, [c_void_p, c_int, POINTER(c_void_p), POINTER(c_void_p)]),
@@ -154,6 +157,31 @@ class SplitSolve:
         nrhs = 0 if Inj_first is None else int(Inj_first.shape[-1])
         _check(load().ss_solve_host(self._h, E.ctypes.data, _host(Sigma_L), _host(Sigma_R), _host(Inj_first),
                                     _host(Inj_last), nrhs, _host(X_out), _host(T_out)), "ss_solve_host")
+
+    # ---- one block column of A^-1 per GPU ----
+    def sweep_column(self, E, column: int):
+        import numpy as np
+        E = np.ascontiguousarray(np.asarray(E, dtype=np.complex128))
+        assert E.shape == (self.n_energy,)
+        _check(load().ss_sweep_column(self._h, E.ctypes.data, int(column), _stream()), "ss_sweep_column")
+
+    def corner_blocks(self, column: int):
+        """Blocks 1 and nb of that block column for every energy: CUDA tensor [n_energy, 2, bs, bs] (enqueued)."""
+        import torch
+        out = torch.empty((self.n_energy, 2, self.bs, self.bs), dtype=torch.complex128, device="cuda")
+        _check(load().ss_get_corner_blocks(self._h, int(column), out.data_ptr(), _stream()), "ss_get_corner_blocks")
+        return out
+
+    def post_column(self, column: int, peer_corner, Sigma_L, Sigma_R, Inj_first, Inj_last=None, X_part=None):
+        import torch
+        nrhs = 0 if Inj_first is None else int(Inj_first.shape[-1])
+        if X_part is None and nrhs > 0:
+            X_part = torch.empty((self.n_energy, self.nb * self.bs, nrhs), dtype=torch.complex128, device=Sigma_L.device)
+        self._keep_solve = [peer_corner, Sigma_L, Sigma_R, Inj_first, Inj_last, X_part]
+        _check(load().ss_post_column(self._h, int(column), _dev(peer_corner, "peer_corner"), _dev(Sigma_L, "Sigma_L"),
+                                     _dev(Sigma_R, "Sigma_R"), _dev(Inj_first, "Inj_first"), _dev(Inj_last, "Inj_last"), nrhs,
+                                     _dev(X_part, "X_part"), _stream()), "ss_post_column")
+        return X_part
 
     def synchronize(self):
         _check(load().ss_synchronize(self._h), "ss_synchronize")
@@ -290,7 +318,9 @@ def density(X, w=None):
 
 
 GEMM_VARIANTS = {0: "4M 64x64", 1: "3M 64x32 (3 CTAs/SM for K<768, software-pipelined 2 CTAs/SM above)",
-                 2: "3M 64x32 lean, every K", 3: "3M 64x32 software-pipelined, every K"}
+                 2: "3M 64x32 lean, every K", 3: "3M 64x32 software-pipelined, every K",
+                 4: "3M 64x32 software-pipelined, TMA-staged operands, 2 CTAs/SM (experiment; uniformly strided batches only)",
+                 5: "3M 64x32 software-pipelined, TMA-staged operands, 3 CTAs/SM (experiment)"}
 
 
 def set_default_gemm_variant(variant: int):

@@ -24,6 +24,8 @@ struct ss_handle_s {
     int hermitian = 0;               // SURVEY 8(f1) at real energies: 0 off, 1 Hermitian Schur update, 2 + no-pivot L Delta L^H
     int growth_limit = 64;           // mode 2: largest multiplier tolerated before the solve is redone with the pivoted LU
     int mode = 0;                    // what the last ss_solve used
+    int swept_cols = 0;              // block columns the last sweep computed (3 = both; 1 / 2: ss_sweep_column)
+    bool whole_solve = true;         // the last post-processing belonged to an ss_solve (so a redo is possible)
     bool force_general = false;      // set while a solve is being redone
     int retried = 0;                 // that solve was redone on the pivoted path (growth limit exceeded)
     struct { const ss_cplx *sl, *sr, *i1, *i2; ss_cplx* x; int nrhs; void* stream; } last_args{};
@@ -112,24 +114,31 @@ static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
     w.tpart = (size_t)nE * TRACE_PARTS * sizeof(double);
     w.T = (size_t)nE * sizeof(double);
     w.ipiv = (size_t)3 * nE * 2 * bs * sizeof(int);
-    w.info = (size_t)5 * nE * sizeof(int);                     // 3 nE zero-pivot records, 2 nE growth monitors
+    w.info = (size_t)6 * nE * sizeof(int);                     // 3 nE zero-pivot records, 2 nE growth monitors, nE single-column sweeps
     w.perm = (size_t)nE * perm_ints_per_energy(bs) * sizeof(int);
     return w;
 }
 
+// The sizes of everything but the corner system [R | b' | e_2] and its solution do not depend on nrhs: that part is
+// allocated once and survives a later call with more right-hand sides (ss_sweep_column knows no nrhs yet, and the sweep's
+// results must outlive the allocation ss_post_column makes).
 static ss_status_t ensure_workspace(ss_handle_t h, int nrhs) {
-    if (h->ws_nrhs >= nrhs) return SS_OK;
-    free_workspace(h);
     WsSizes w = ws_sizes(h->nb, h->bs, h->n_energy, nrhs);
     bool ok = true;
     auto A = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 16) != cudaSuccess) ok = false; };
-    A((void**)&h->slots, w.slots); A((void**)&h->aug, w.aug); A((void**)&h->aop, w.aop); A((void**)&h->tinv, w.tinv);
-    A((void**)&h->raug, w.raug); A((void**)&h->wz, w.wz);
-    A((void**)&h->gam_l, w.sq); A((void**)&h->gam_r, w.sq); A((void**)&h->g1n, w.sq); A((void**)&h->w1, w.sq);
-    A((void**)&h->w2, w.sq); A((void**)&h->E_dev, w.E); A((void**)&h->tpart, w.tpart); A((void**)&h->T_dev, w.T);
-    A((void**)&h->ipiv, w.ipiv); A((void**)&h->info, w.info); A((void**)&h->perm, w.perm);
-    if (!ok) { cudaGetLastError(); free_workspace(h); return SS_ERR_ALLOC; }
-    h->ws_nrhs = nrhs;
+    if (!h->slots) {
+        A((void**)&h->slots, w.slots); A((void**)&h->aug, w.aug); A((void**)&h->aop, w.aop); A((void**)&h->tinv, w.tinv);
+        A((void**)&h->gam_l, w.sq); A((void**)&h->gam_r, w.sq); A((void**)&h->g1n, w.sq); A((void**)&h->w1, w.sq);
+        A((void**)&h->w2, w.sq); A((void**)&h->E_dev, w.E); A((void**)&h->tpart, w.tpart); A((void**)&h->T_dev, w.T);
+        A((void**)&h->ipiv, w.ipiv); A((void**)&h->info, w.info); A((void**)&h->perm, w.perm);
+        if (!ok) { cudaGetLastError(); free_workspace(h); return SS_ERR_ALLOC; }
+    }
+    if (h->ws_nrhs < nrhs) {
+        free_dev(h->raug); free_dev(h->wz); h->raug = h->wz = nullptr;
+        A((void**)&h->raug, w.raug); A((void**)&h->wz, w.wz);
+        if (!ok) { cudaGetLastError(); free_workspace(h); return SS_ERR_ALLOC; }
+        h->ws_nrhs = nrhs;
+    }
     return SS_OK;
 }
 
@@ -146,6 +155,7 @@ extern "C" const char* ss_strerror(ss_status_t s) {
         case SS_ERR_ALLOC: return "allocation failed";
         case SS_ERR_SINGULAR: return "exactly zero pivot";
         case SS_ERR_CUDA: return "CUDA error";
+        case SS_ERR_UNSTABLE: return "no-pivot factorisation exceeded its growth limit";
     }
     return "unknown status";
 }
@@ -315,9 +325,9 @@ extern "C" ss_status_t ss_last_mode(ss_handle_t h, int* mode, int* retried) {
 // ---------------------------------------------------------------------------------------------------------
 // the hot path
 // ---------------------------------------------------------------------------------------------------------
-static void launch_form(Ctx& ctx, FormSide s0, FormSide s1, const cplx* E, BPtr dst, int ld, int bs, int batch) {
+static void launch_form(Ctx& ctx, FormSide s0, FormSide s1, const cplx* E, BPtr dst, int ld, int bs, int batch, int eshift = 1) {
     dim3 grid((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)batch);
-    form_kernel<<<grid, 256, 0, ctx.st>>>(s0, s1, E, dst, ld, bs);
+    form_kernel<<<grid, 256, 0, ctx.st>>>(s0, s1, E, dst, ld, bs, eshift);
     ctx.note(cudaGetLastError());
 }
 
@@ -325,25 +335,35 @@ static void launch_form(Ctx& ctx, FormSide s0, FormSide s1, const cplx* E, BPtr 
 // columns in lockstep.  Chain z = 2*e + col.  Slot layout per chain (nb+1 slots of bs x bs): column 0 keeps X_i in slot i
 // (X_1 in slot 0) and ends with Q_i in slot i-1; column 1 keeps Y_i in slot i-1 (Y_nb in slot nb) and ends with P_i in
 // slot i.  sweep_step(s) is block step s of both sweeps (a0-a3), recursion_step(r) one product of a4.
+// cols: 3 = both sweeps in lockstep (chain z = 2*e + col), 1 / 2 = only the first- / last-column sweep (chain z = e;
+// "naturally scale to two accelerators", one block column per GPU).
 struct Group {
     int e0 = 0, nE = 0;
+    int cols = 3;
     Ctx ctx;
+    bool dual() const { return cols == 3; }
+    int batch() const { return dual() ? 2 * nE : nE; }
+    // pointer of chain z: both columns (p0 first, p1 last) or the one of this group
+    BPtr ch(const cplx* p0, const cplx* p1, long long s_energy) const {
+        return dual() ? bp_chain(p0, p1, s_energy) : bp_strided(cols == 1 ? p0 : p1, s_energy);
+    }
 };
 
 static void sweep_step(ss_handle_t h, Group& G, int s) {
     Ctx& ctx = G.ctx;
-    const int nb = h->nb, bs = h->bs, e0 = G.e0, batch = 2 * G.nE;
+    const int nb = h->nb, bs = h->bs, e0 = G.e0, batch = G.batch(), eshift = G.dual() ? 1 : 0;
     const long long B2 = (long long)bs * bs;
     const long long s_slot_e = 2LL * (nb + 1) * B2;
     auto slot = [&](int col, int idx) { return h->slots + (long long)e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
     const int ldg = pad_ld(2 * bs);
     const long long s_aug_e = 2LL * bs * ldg;
-    const BPtr aug = bp_chain(h->aug + e0 * s_aug_e, h->aug + e0 * s_aug_e + (long long)bs * ldg, s_aug_e);
-    const BPtr aop = bp_chain(h->aop + e0 * 2 * B2, h->aop + e0 * 2 * B2 + B2, 2 * B2);
+    const BPtr aug = G.ch(h->aug + e0 * s_aug_e, h->aug + e0 * s_aug_e + (long long)bs * ldg, s_aug_e);
+    const BPtr aop = G.ch(h->aop + e0 * 2 * B2, h->aop + e0 * 2 * B2 + B2, 2 * B2);
     const cplx* E = h->E_dev + e0;
     LuWork w;
     w.tinv = h->tinv + lu_tinv_elems(bs, 2 * e0);
-    w.ipiv = h->ipiv + (long long)2 * e0 * 2 * bs; w.ipiv_stride = 2 * bs; w.info = h->info + 2 * e0;
+    w.ipiv = h->ipiv + (long long)2 * e0 * 2 * bs; w.ipiv_stride = 2 * bs;
+    w.info = G.dual() ? h->info + 2 * e0 : h->info + 5 * h->n_energy + e0;
     w.growth = h->info + 3 * h->n_energy + 2 * e0;
     const int mode = h->mode;                                  // 0 general, 1 Hermitian Schur update, 2 + L Delta L^H (real energies)
     const int info_stride = 2 * bs + 2;
@@ -360,9 +380,10 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
                             : FormSide{nullptr, nullptr, FORM_IDENT};
     FormSide r1 = (i_m < nb) ? FormSide{h->Su + (long long)(i_m - 1) * B2, h->Hu + (long long)(i_m - 1) * B2, FORM_PLAIN}
                              : FormSide{nullptr, nullptr, FORM_IDENT};
-    const BPtr out = bp_chain(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
-    if (mode == 2) launch_form(ctx, r0, r1, E, bp_offset(aug, bs), ldg, bs, batch);    // no interchanges: straight into [D | B]
-    else launch_form(ctx, r0, r1, E, out, bs, bs, batch);
+    if (G.cols == 2) r0 = r1;                                  // one sweep only: its side goes first
+    const BPtr out = G.ch(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
+    if (mode == 2) launch_form(ctx, r0, r1, E, bp_offset(aug, bs), ldg, bs, batch, eshift);    // no interchanges: straight into [D | B]
+    else launch_form(ctx, r0, r1, E, out, bs, bs, batch, eshift);
     GemmArgs g{};
     g.M = bs; g.N = bs; g.K = 0;
     g.A = aop; g.lda = bs; g.B = aop; g.ldb = bs;
@@ -370,16 +391,17 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
         // left operands: A_{i,i+1} (column 0) / A_{i,i-1} (column 1)
         FormSide a0{h->Su + (long long)(i_f - 1) * B2, h->Hu + (long long)(i_f - 1) * B2, FORM_PLAIN};
         FormSide a1{h->Su + (long long)(i_m - 2) * B2, h->Hu + (long long)(i_m - 2) * B2, FORM_CONJT};
-        launch_form(ctx, a0, a1, E, aop, bs, bs, batch);
+        if (G.cols == 2) a0 = a1;
+        launch_form(ctx, a0, a1, E, aop, bs, bs, batch, eshift);
         g.K = bs;
-        g.B = bp_chain(slot(0, i_f + 1), slot(1, i_m - 2), s_slot_e);   // X_{i+1} / Y_{i-1}
+        g.B = G.ch(slot(0, i_f + 1), slot(1, i_m - 2), s_slot_e);   // X_{i+1} / Y_{i-1}
     }
     // a1 (+ a0 for the diagonal block, fused in the epilogue): D = E S_ii - H_ii - A_op * X_prev
     ctx.use(CLS_LO);
     g.C = aug; g.ldc = ldg; g.Cin = aug; g.ldcin = ldg; g.alpha = 1.0; g.beta = 0.0;
-    g.S = bp_chain(h->Sd + (long long)(i_f - 1) * B2, h->Sd + (long long)(i_m - 1) * B2, 0);
-    g.H = bp_chain(h->Hd + (long long)(i_f - 1) * B2, h->Hd + (long long)(i_m - 1) * B2, 0);
-    g.lds = bs; g.E = E;
+    g.S = G.ch(h->Sd + (long long)(i_f - 1) * B2, h->Sd + (long long)(i_m - 1) * B2, 0);
+    g.H = G.ch(h->Hd + (long long)(i_f - 1) * B2, h->Hd + (long long)(i_m - 1) * B2, 0);
+    g.lds = bs; g.E = E; g.eshift = eshift;
     if (mode >= 1) g.tri = 1;                                  // D_i is Hermitian at real E (L154): lower triangle only
     gemm_run(ctx, g, batch, GEMM_BIG, EPI_SCHUR);
     // a2 + the L half of a3
@@ -395,26 +417,36 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
 
 // a4: Q_i = -X_i Q_{i-1} (i = 2..nb), P_i = -Y_i P_{i+1} (i = nb-1..1); r = 1..nb-1
 static void recursion_step(ss_handle_t h, Group& G, int r) {
-    const int nb = h->nb, bs = h->bs, batch = 2 * G.nE;
+    const int nb = h->nb, bs = h->bs, batch = G.batch();
     const long long B2 = (long long)bs * bs;
     const long long s_slot_e = 2LL * (nb + 1) * B2;
     auto slot = [&](int col, int idx) { return h->slots + (long long)G.e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
     const int i0 = r + 1, i1 = nb - r;
     G.ctx.use(CLS_LO);
-    GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_chain(slot(0, i0), slot(1, i1 - 1), s_slot_e), bs,
-                          bp_chain(slot(0, i0 - 2), slot(1, i1 + 1), s_slot_e), bs, 0.0,
-                          bp_chain(slot(0, i0 - 1), slot(1, i1), s_slot_e), bs);
+    GemmArgs g = gemm_std(bs, bs, bs, -1.0, G.ch(slot(0, i0), slot(1, i1 - 1), s_slot_e), bs,
+                          G.ch(slot(0, i0 - 2), slot(1, i1 + 1), s_slot_e), bs, 0.0,
+                          G.ch(slot(0, i0 - 1), slot(1, i1), s_slot_e), bs);
     gemm_run(G.ctx, g, batch, GEMM_BIG, EPI_STD);
 }
 
 // a5-a7: corner system, solution, transmission (north_star for T).
+// G.cols == 3: both block columns are in this handle's slots.  G.cols == 1 / 2: only the first / last one
+// is; blocks 1 and nb of the other column come from `peer` ([n_energy][2][bs][bs], written there by the caller after the
+// exchange with the GPU that owns that column), and X receives only this column's share Q_i w_top resp. P_i w_bot.
 static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR, const cplx* inj1, const cplx* inj2,
-                     int m, cplx* X) {
+                     int m, cplx* X, const cplx* peer) {
     Ctx& ctx = G.ctx;
     const int nb = h->nb, bs = h->bs, nE = G.nE, e0 = G.e0;
     const long long B2 = (long long)bs * bs;
     const long long s_slot_e = 2LL * (nb + 1) * B2;
     auto slot = [&](int col, int idx) { return h->slots + (long long)e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
+    // corner blocks [column][first / last block] with their energy strides
+    const cplx* cor[2][2] = {{slot(0, 0), slot(0, nb - 1)}, {slot(1, 1), slot(1, nb)}};
+    long long cor_s[2] = {s_slot_e, s_slot_e};
+    if (G.cols != 3) {
+        const int other = (G.cols == 1) ? 1 : 0;
+        cor[other][0] = peer + (long long)e0 * 2 * B2; cor[other][1] = cor[other][0] + B2; cor_s[other] = 2 * B2;
+    }
     const int zc = h->want_T ? bs : 0;                // columns of e_2 (for (R^-1)_{12}, (R^-1)_{22})
     const int W = 2 * bs + m + zc;
     const int nr = m + zc;
@@ -440,8 +472,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     const cplx* sig[2] = {SigL, SigR};
     for (int br = 0; br < 2; br++)
         for (int bc = 0; bc < 2; bc++) {
-            const cplx* Bsrc = (bc == 0) ? slot(0, br == 0 ? 0 : nb - 1) : slot(1, br == 0 ? 1 : nb);
-            GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(Bsrc, s_slot_e), bs, 1.0,
+            GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(cor[bc][br], cor_s[bc]), bs, 1.0,
                                   bp_strided(raug + (long long)br * bs * ldW + (long long)bc * bs, s_r), ldW);
             gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         }
@@ -455,21 +486,25 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     back_substitute(ctx, bp_strided(raug, s_r), ldW, 2 * bs, nr, bp_strided(wz, s_w), nr, nE, w);
     // a6: X_i = Q_i w_top + P_i w_bot, batch z = e*nb + (i-1)
     if (m > 0) {
-        GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(0, 0), nb, B2, s_slot_e), bs,
-                              bp_two_level(wz, nb, 0, s_w), nr, 0.0,
-                              bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
-        gemm_run(ctx, g, nE * nb, GEMM_BIG, EPI_STD);
-        GemmArgs g2 = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(1, 1), nb, B2, s_slot_e), bs,
-                               bp_two_level(wz + (long long)bs * nr, nb, 0, s_w), nr, 1.0,
-                               bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
-        gemm_run(ctx, g2, nE * nb, GEMM_BIG, EPI_STD);
+        if (G.cols & 1) {
+            GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(0, 0), nb, B2, s_slot_e), bs,
+                                  bp_two_level(wz, nb, 0, s_w), nr, 0.0,
+                                  bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
+            gemm_run(ctx, g, nE * nb, GEMM_BIG, EPI_STD);
+        }
+        if (G.cols & 2) {
+            GemmArgs g2 = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(1, 1), nb, B2, s_slot_e), bs,
+                                   bp_two_level(wz + (long long)bs * nr, nb, 0, s_w), nr, (G.cols & 1) ? 1.0 : 0.0,
+                                   bp_two_level(X, nb, (long long)bs * m, (long long)nb * bs * m), m);
+            gemm_run(ctx, g2, nE * nb, GEMM_BIG, EPI_STD);
+        }
     }
     // a7: G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22;  T = Re Tr(Gamma_L G Gamma_R G^H)
     if (h->want_T) {
-        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(0, 0), s_slot_e), bs, bp_strided(wz + m, s_w), nr, 0.0,
+        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[0][0], cor_s[0]), bs, bp_strided(wz + m, s_w), nr, 0.0,
                               bp_strided(g1n, B2), bs);
         gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
-        GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(slot(1, 1), s_slot_e), bs,
+        GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[1][0], cor_s[1]), bs,
                                bp_strided(wz + (long long)bs * nr + m, s_w), nr, 1.0, bp_strided(g1n, B2), bs);
         gemm_run(ctx, g2, nE, GEMM_BIG, EPI_STD);
         dim3 gg((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)nE);
@@ -507,12 +542,19 @@ static bool ensure_groups(ss_handle_t h, int n) {
 }
 
 // Everything ss_solve puts on the device, enqueued on `stream` (a non-default stream the handle owns).
-static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx* Sigma_L, const cplx* Sigma_R,
-                                 const cplx* Inj_first, const cplx* Inj_last, int nrhs, cplx* X) {
+enum { PH_SWEEP = 1, PH_POST = 2 };
+static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, int phases, int cols, const cplx* Sigma_L,
+                                 const cplx* Sigma_R, const cplx* Inj_first, const cplx* Inj_last, int nrhs, cplx* X,
+                                 const cplx* peer) {
     auto mark = [&](cudaEvent_t ev) { return cudaEventRecord(ev, stream); };
-    if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * (size_t)h->n_energy, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-        cudaMemsetAsync(h->info, 0, sizeof(int) * 5 * (size_t)h->n_energy, stream) != cudaSuccess)
+    const size_t nEs = (size_t)h->n_energy;
+    if (phases & PH_SWEEP) {
+        if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * nEs, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
+            cudaMemsetAsync(h->info, 0, sizeof(int) * 6 * nEs, stream) != cudaSuccess)
+            return cudaErrorUnknown;
+    } else if (cudaMemsetAsync(h->info + 2 * nEs, 0, sizeof(int) * nEs, stream) != cudaSuccess) {   // the corner's records
         return cudaErrorUnknown;
+    }
     // Energy points are independent: split them over stream groups.  Group g owns the energies
     // [e0, e0 + nE); the host interleaves the groups' launches step by step so that every group's streams stay fed.
     const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
@@ -520,6 +562,7 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx*
     for (int g = 0; g < nG; g++) {
         G[g].e0 = (int)((long long)h->n_energy * g / nG);
         G[g].nE = (int)((long long)h->n_energy * (g + 1) / nG) - G[g].e0;
+        G[g].cols = cols;
         Ctx& c = G[g].ctx;
         c.variant = h->gemm_variant;
         c.group = g;
@@ -541,10 +584,12 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx*
     if (h->want_trace)
         for (int g = 0; g < nG; g++) { G[g].ctx.trace = &h->trace; G[g].ctx.trace_open(); }
     const int nb = h->nb;
-    for (int s = 0; s < nb; s++)
-        for (int g = 0; g < nG; g++) sweep_step(h, G[g], s);
-    for (int r = 1; r < nb; r++)
-        for (int g = 0; g < nG; g++) recursion_step(h, G[g], r);
+    if (phases & PH_SWEEP) {
+        for (int s = 0; s < nb; s++)
+            for (int g = 0; g < nG; g++) sweep_step(h, G[g], s);
+        for (int r = 1; r < nb; r++)
+            for (int g = 0; g < nG; g++) recursion_step(h, G[g], r);
+    }
     if (nG > 1)
         for (int g = 0; g < nG; g++) {                     // marks the end of the sweep phase; the groups do not wait
             G[g].ctx.use(CLS_LO);
@@ -552,7 +597,8 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx*
             cudaStreamWaitEvent(stream, h->groups[g].ev_mark, 0);
         }
     mark(h->ev[1]);
-    for (int g = 0; g < nG; g++) run_post(h, G[g], Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X);
+    if (phases & PH_POST)
+        for (int g = 0; g < nG; g++) run_post(h, G[g], Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X, peer);
     if (nG > 1)
         for (int g = 0; g < nG; g++) {
             G[g].ctx.use(CLS_LO);
@@ -570,12 +616,14 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, const cplx*
     return err;
 }
 
-extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L, const ss_cplx* Sigma_R,
-                                const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs, ss_cplx* X,
-                                void* cuda_stream) {
-    if (!h || !E_host || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
-    if (nrhs > 0 && (!Inj_first || !X)) return SS_ERR_INVALID_ARG;
+static ss_status_t check_info(ss_handle_t h);
+
+// Common body of ss_solve (both phases, both columns) and of the split-phase calls of SURVEY.md 8(f2).
+static ss_status_t run_phases(ss_handle_t h, const ss_cplx* E_host, int phases, int cols, const ss_cplx* Sigma_L,
+                              const ss_cplx* Sigma_R, const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs, ss_cplx* X,
+                              const ss_cplx* peer, void* cuda_stream) {
     if (!h->have_h) return SS_ERR_NOT_READY;
+    if (h->launched) cudaEventSynchronize(h->ev[2]);      // the previous call may still use the scratch this one may re-allocate
     ss_status_t st = ensure_workspace(h, nrhs);
     if (st != SS_OK) return st;
     const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
@@ -586,10 +634,11 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
             cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     }
     cudaStream_t user = (cudaStream_t)cuda_stream, main = h->main_stream;
-    if (h->launched) cudaEventSynchronize(h->ev[2]);      // E_pinned of the previous call is free again
-    if (h->upload_consumed) { h->upload_pending = false; h->upload_consumed = false; }   // that solve saw the whole upload
-    if ((const void*)E_host != (const void*)h->E_pinned) memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
-    {   // A = E S - H is Hermitian when every energy is real
+    if (h->launched) cudaEventSynchronize(h->ev[2]);      // E_pinned and the per-solve scratch of the previous call are free again
+    if (phases & PH_SWEEP) {
+        if (h->upload_consumed) { h->upload_pending = false; h->upload_consumed = false; }   // that solve saw the whole upload
+        if ((const void*)E_host != (const void*)h->E_pinned) memcpy(h->E_pinned, E_host, sizeof(cplx) * (size_t)h->n_energy);
+        // A = E S - H is Hermitian when every energy is real
         bool all_real = true;
         for (int e = 0; e < h->n_energy; e++) all_real = all_real && (E_host[e].im == 0.0);
         int mode = all_real ? h->hermitian : 0;
@@ -597,28 +646,69 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
         if (h->force_general) mode = 0;
         h->mode = mode;
         if (!h->force_general) h->retried = 0;
+        h->swept_cols = cols;
     }
-    h->last_args = {Sigma_L, Sigma_R, Inj_first, Inj_last, X, nrhs, cuda_stream};
+    if (phases == (PH_SWEEP | PH_POST)) h->last_args = {Sigma_L, Sigma_R, Inj_first, Inj_last, X, nrhs, cuda_stream};
     h->prof.used = 0; h->prof.flops = 0.0; h->prof.launches = 0;
     // the solve runs on a stream of the handle, ordered after the caller's stream and joined back to it
     cudaEventRecord(h->ev_in, user);
     cudaStreamWaitEvent(main, h->ev_in, 0);
 
-    cudaError_t err = enqueue_solve(h, main, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first,
-                                    (const cplx*)Inj_last, nrhs, (cplx*)X);
+    cudaError_t err = enqueue_solve(h, main, phases, cols, (const cplx*)Sigma_L, (const cplx*)Sigma_R, (const cplx*)Inj_first,
+                                    (const cplx*)Inj_last, nrhs, (cplx*)X, (const cplx*)peer);
     cudaEventRecord(h->ev_out, main);
     cudaStreamWaitEvent(user, h->ev_out, 0);
-    if (h->upload_pending) h->upload_consumed = true;
+    if ((phases & PH_SWEEP) && h->upload_pending) h->upload_consumed = true;
     h->last_stream = user;
-    h->last_nrhs = nrhs;
-    h->solved = true;
     h->launched = true;
+    if (phases & PH_POST) { h->last_nrhs = nrhs; h->solved = true; h->whole_solve = (phases & PH_SWEEP) != 0; }
+    else h->solved = false;
     if (err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }
 
+extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_cplx* Sigma_L, const ss_cplx* Sigma_R,
+                                const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs, ss_cplx* X,
+                                void* cuda_stream) {
+    if (!h || !E_host || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
+    if (nrhs > 0 && (!Inj_first || !X)) return SS_ERR_INVALID_ARG;
+    return run_phases(h, E_host, PH_SWEEP | PH_POST, 3, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X, nullptr, cuda_stream);
+}
+
+// ---- one energy batch on two GPUs, one block column of A^-1 each ----------------
+extern "C" ss_status_t ss_sweep_column(ss_handle_t h, const ss_cplx* E_host, int column, void* cuda_stream) {
+    if (!h || !E_host || column < 0 || column > 1) return SS_ERR_INVALID_ARG;
+    return run_phases(h, E_host, PH_SWEEP, 1 << column, nullptr, nullptr, nullptr, nullptr, 0, nullptr, nullptr, cuda_stream);
+}
+
+extern "C" ss_status_t ss_get_corner_blocks(ss_handle_t h, int column, ss_cplx* out_dev, void* cuda_stream) {
+    if (!h || !out_dev || column < 0 || column > 1) return SS_ERR_INVALID_ARG;
+    if (!h->launched || !(h->swept_cols & (1 << column))) return SS_ERR_NOT_READY;
+    const size_t B2 = (size_t)h->bs * h->bs, nb = h->nb;
+    const cplx* base = h->slots + (column ? (nb + 1) * B2 + B2 : 0);          // block 1 of that column of energy 0
+    // [n_energy][2][bs][bs]: blocks 1 and nb; one strided 2-D copy per block position
+    for (int q = 0; q < 2; q++) {
+        const cplx* src = base + (q ? (nb - 1) * B2 : 0);
+        if (cudaMemcpy2DAsync((cplx*)out_dev + q * B2, 2 * B2 * sizeof(cplx), src, 2 * (nb + 1) * B2 * sizeof(cplx), B2 * sizeof(cplx),
+                              (size_t)h->n_energy, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream) != cudaSuccess) {
+            cudaGetLastError(); return SS_ERR_CUDA;
+        }
+    }
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_post_column(ss_handle_t h, int column, const ss_cplx* peer_corner_dev, const ss_cplx* Sigma_L,
+                                      const ss_cplx* Sigma_R, const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs,
+                                      ss_cplx* X_part, void* cuda_stream) {
+    if (!h || !peer_corner_dev || !Sigma_L || !Sigma_R || nrhs < 0 || column < 0 || column > 1) return SS_ERR_INVALID_ARG;
+    if (nrhs > 0 && (!Inj_first || !X_part)) return SS_ERR_INVALID_ARG;
+    if (!h->launched || h->swept_cols != (1 << column)) return SS_ERR_NOT_READY;
+    return run_phases(h, nullptr, PH_POST, 1 << column, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X_part, peer_corner_dev,
+                      cuda_stream);
+}
+
 static ss_status_t check_info(ss_handle_t h) {
-    const int nE = h->n_energy, n = 5 * nE;
+    const int nE = h->n_energy, n = 6 * nE;
     int* host = (int*)malloc(sizeof(int) * (size_t)n);
     if (!host) return SS_ERR_ALLOC;
     cudaError_t e = cudaMemcpy(host, h->info, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost);
@@ -626,10 +716,10 @@ static ss_status_t check_info(ss_handle_t h) {
     bool grown = false;
     if (e != cudaSuccess) { cudaGetLastError(); st = SS_ERR_CUDA; }
     else {
-        for (int i = 0; i < 3 * nE; i++) if (host[i] != 0) { st = SS_ERR_SINGULAR; break; }
+        for (int i = 0; i < n; i++) if ((i < 3 * nE || i >= 5 * nE) && host[i] != 0) { st = SS_ERR_SINGULAR; break; }
         if (h->mode == 2) {
             const float lim = (float)h->growth_limit;
-            for (int i = 3 * nE; i < n; i++) {
+            for (int i = 3 * nE; i < 5 * nE; i++) {
                 float g; memcpy(&g, &host[i], sizeof(float));
                 if (!(g <= lim)) grown = true;
             }
@@ -637,6 +727,7 @@ static ss_status_t check_info(ss_handle_t h) {
     }
     free(host);
     if (st != SS_ERR_CUDA && h->mode == 2 && (grown || st == SS_ERR_SINGULAR) && !h->force_general) {
+        if (!h->whole_solve) return SS_ERR_UNSTABLE;          // split-phase calls: the caller redoes both phases with "hermitian" = 0
         // the no-pivot L Delta L^H met a multiplier above the limit (or a zero pivot): its results are discarded and the
         // whole solve is redone on the general path (mode 0), same arguments, same stream
         h->force_general = true;
@@ -675,7 +766,7 @@ extern "C" ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int*
     if (!h->solved) return SS_ERR_NOT_READY;
     *energy = *block = *column = -1;
     if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
-    const int nE = h->n_energy, n = 3 * nE;
+    const int nE = h->n_energy, n = 6 * nE;
     int* host = (int*)malloc(sizeof(int) * (size_t)n);
     if (!host) return SS_ERR_ALLOC;
     if (cudaMemcpy(host, h->info, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost) != cudaSuccess) {
@@ -683,11 +774,13 @@ extern "C" ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int*
     }
     const int info_stride = 2 * h->bs + 2;
     for (int i = 0; i < n; i++) {
-        if (!host[i]) continue;
-        if (i < 2 * nE) {
+        if (!host[i] || (i >= 3 * nE && i < 5 * nE)) continue;     // [3 nE, 5 nE) are the growth monitors
+        if (i < 2 * nE || i >= 5 * nE) {
+            const bool single = i >= 5 * nE;                       // ss_sweep_column: one record per energy
             int s = (host[i] - 1) / info_stride;
-            *energy = i >> 1; *column = i & 1;
-            *block = (i & 1) ? s + 1 : h->nb - s;
+            *energy = single ? i - 5 * nE : i >> 1;
+            *column = single ? (h->swept_cols == 2 ? 1 : 0) : (i & 1);
+            *block = *column ? s + 1 : h->nb - s;
         } else {
             *energy = i - 2 * nE; *column = -1; *block = 0;
         }

@@ -18,17 +18,18 @@ struct FormSide {
     int mode;
 };
 
-// dst(z)[r][c] (ld) for the bs x bs block; z = 2*e + column; side = s0 for column 0, s1 for column 1.
+// dst(z)[r][c] (ld) for the bs x bs block.  eshift = 1: z = 2*e + column, side = s0 for column 0, s1 for column 1 (both
+// sweeps in lockstep); eshift = 0: z = e, side s0 (one sweep only: SURVEY.md 8(f2), one column per GPU).
 __global__ void __launch_bounds__(256)
-form_kernel(FormSide s0, FormSide s1, const cplx* __restrict__ E, BPtr dst, int ld, int bs) {
+form_kernel(FormSide s0, FormSide s1, const cplx* __restrict__ E, BPtr dst, int ld, int bs, int eshift) {
     __shared__ cplx tile[32][33];
     const int z = blockIdx.z;
-    const FormSide s = (z & 1) ? s1 : s0;
+    const FormSide s = (eshift && (z & 1)) ? s1 : s0;
     if (s.mode == FORM_NONE) return;
     cplx* __restrict__ D = bptr(dst, z);
     const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;      // 32 x 8
-    const cplx Ee = E[z >> 1];
+    const cplx Ee = E[z >> eshift];
     if (s.mode == FORM_PLAIN) {
         for (int rr = ty; rr < 32; rr += 8) {
             int r = r0 + rr, c = c0 + tx;

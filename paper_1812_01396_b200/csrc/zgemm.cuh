@@ -28,8 +28,8 @@ struct GemmArgs {
     BPtr C; int ldc;
     BPtr Cin; int ldcin;       // EPI_STD: C = alpha*acc + beta*Cin (Cin may alias C; ignored when beta == 0)
     double alpha, beta;
-    BPtr S; BPtr H; int lds;   // EPI_SCHUR: C = (E[z>>1]*S - H) - acc   (a0 fused into a1's epilogue)
-    const cplx* E;
+    BPtr S; BPtr H; int lds;   // EPI_SCHUR: C = (E[z>>eshift]*S - H) - acc   (a0 fused into a1's epilogue)
+    const cplx* E; int eshift; // eshift 1: batch entry z = 2*energy + column, 0: z = energy
     int tiles_m, tiles_n;
     // tri != 0: only the tiles that touch the lower triangle are computed (Hermitian updates): element
     // (i, j) of C is at global position (tri_row0 + i, tri_col0 + j); a tile whose every column lies right of its last row is skipped
@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(Cfg::NT, MINB) zgemm_kernel(const GemmArgs p) 
             }
         }
     } else {
-        const cplx Ee = p.E[z >> 1];
+        const cplx Ee = p.E[z >> p.eshift];
         const cplx* __restrict__ Sg = bptr(p.S, z);
         const cplx* __restrict__ Hg = bptr(p.H, z);
 #pragma unroll

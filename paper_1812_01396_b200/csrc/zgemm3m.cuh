@@ -17,14 +17,47 @@
 // chosen so that both fragment LDS.128 patterns are bank-conflict-free: A stride == 8 (mod 16) doubles, B stride
 // == 4 (mod 16) doubles.
 #pragma once
+#include <cuda.h>
+#include <cstring>
 #include "zgemm.cuh"
 
 namespace ss {
 
-template <int BM_, int BN_, int WARPS_M_, int WARPS_N_, int KC_, int STAGES_, int MINB_, int PF_ = 0>
+// ---- TMA staging (experiment, profiles/r02_gemm_tma.md): cp.async.bulk.tensor + mbarrier instead of cp.async
+__device__ __forceinline__ void g_mbar_init(unsigned bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void g_mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void g_mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(unsigned smem_dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+
+template <int BM_, int BN_, int WARPS_M_, int WARPS_N_, int KC_, int STAGES_, int MINB_, int PF_ = 0, int TMA_ = 0>
 struct Gemm3Cfg {
     static constexpr int BM = BM_, BN = BN_, WARPS_M = WARPS_M_, WARPS_N = WARPS_N_, KC = KC_, STAGES = STAGES_, MINB = MINB_;
     static constexpr int PF = PF_;     // 1: fragments of the next k-step are prefetched across the stage boundary
+    // 1: operand tiles staged by TMA (cp.async.bulk.tensor, SWIZZLE_128B boxes of 128-byte rows: the A tile as one box of
+    // BM rows x 8 complex k, the B tile as BN/8 boxes of 8 k-rows x 8 complex columns) and published by one mbarrier per
+    // stage; unpadded tiles, fragment addresses XOR-swizzled; the 8 k of a stage are consumed as {0,2,4,6} then {1,3,5,7}
+    // so that both fragment LDS.128 patterns stay bank-conflict-free under the swizzle.  Needs PF = 1 and KC = 8.
+    static constexpr int TMA = TMA_;
+    static_assert(TMA_ == 0 || (PF_ == 1 && KC_ == 8 && BN_ % 8 == 0), "TMA staging");
+    static constexpr int TMA_STAGE_D = BM * 16 + (BN / 8) * 128;          // doubles per stage (unpadded boxes)
+    static constexpr int TMA_SMEM_BYTES = STAGES * TMA_STAGE_D * 8 + 1024 + 8 * STAGES;   // + alignment slack + mbarriers
     static_assert(PF_ == 0 || STAGES_ >= 3, "cross-stage prefetch shortens the cp.async distance by one stage");
     static constexpr int NT = WARPS_M * WARPS_N * 32;
     static constexpr int WM = BM / WARPS_M, WN = BN / WARPS_N;   // warp tile, complex elements
@@ -40,12 +73,16 @@ struct Gemm3Cfg {
     static_assert(LDA_S % 16 == 8 && LDB_S % 16 == 4, "bank layout");
 };
 
+struct GemmTmaMaps { CUtensorMap a, b; };
+
 template <class Cfg, int EPI>
-__global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmArgs p) {
-    extern __shared__ __align__(16) double smem[];
+__global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmArgs p, const __grid_constant__ GemmTmaMaps tm) {
+    extern __shared__ __align__(16) double smem_raw[];
     constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = Cfg::KC, STAGES = Cfg::STAGES;
     constexpr int NT = Cfg::NT, MI = Cfg::MI, NJ = Cfg::NJ, LDA_S = Cfg::LDA_S, LDB_S = Cfg::LDB_S;
-    constexpr int STAGE_D = Cfg::STAGE_D;
+    constexpr int STAGE_D = Cfg::TMA ? Cfg::TMA_STAGE_D : Cfg::STAGE_D;
+    // TMA boxes with the 128-byte swizzle need 1024-byte aligned destinations
+    double* smem = Cfg::TMA ? reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023) : smem_raw;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, t = lane & 3;
@@ -180,9 +217,27 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
         }
     };
 
+    const unsigned tma_bars = (unsigned)__cvta_generic_to_shared(smem + STAGES * STAGE_D);     // STAGES mbarriers behind the tiles
     auto load_stage = [&](int kt, int stage) {
-        if constexpr (LEAN) load_stage_lean(kt, stage); else load_stage_desc(kt, stage);
+        if constexpr (Cfg::TMA) {
+            if (tid == 0) {
+                const unsigned bar = tma_bars + 8u * stage;
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(smem + stage * STAGE_D);
+                g_mbar_expect_tx(bar, (unsigned)(STAGE_D * 8));
+                tma_load_3d(dst, &tm.a, 2 * kt * KC, m0, z, bar);
+#pragma unroll
+                for (int jb = 0; jb < BN / 8; jb++)
+                    tma_load_3d(dst + (unsigned)((BM * 16 + jb * 128) * 8), &tm.b, 2 * (n0 + 8 * jb), kt * KC, z, bar);
+            }
+        } else if constexpr (LEAN) load_stage_lean(kt, stage); else load_stage_desc(kt, stage);
     };
+    if constexpr (Cfg::TMA) {
+        if (tid == 0) {
+            for (int i = 0; i < STAGES; i++) g_mbar_init(tma_bars + 8u * i, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+    }
 
     // ---- fragment offsets (doubles, within a stage)
     const int wm0 = (warp / Cfg::WARPS_N) * Cfg::WM, wn0 = (warp % Cfg::WARPS_N) * Cfg::WN;
@@ -245,19 +300,41 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
         // stage kt's last DMMAs issue -- no warp starts a stage by waiting for its LDS.
         constexpr int KS = KC / 4;
         double fa[2][MI][2], fb[2][NJ][2];
+        // TMA layout (doubles within a stage): A row r at 16 r, complex k chunk c at ((c ^ (r & 7)) << 1); B box jb at
+        // 16 BM + 128 jb, k row kk at 16 kk, complex column cc at ((cc ^ (kk & 7)) << 1).  k-step ks uses the chunks 2t + ks.
+        const int ta_off0 = (wm0 + g) * 16 + (((2 * t) ^ g) << 1), ta_off1 = (wm0 + g) * 16 + (((2 * t + 1) ^ g) << 1);
+        const int tb_off0 = BM * 16 + (wn0 >> 3) * 128 + (2 * t) * 16 + ((g ^ (2 * t)) << 1);
+        const int tb_off1 = BM * 16 + (wn0 >> 3) * 128 + (2 * t + 1) * 16 + ((g ^ (2 * t + 1)) << 1);
         auto load_frag = [&](int buf, const double* sS, int ks) {
+            if constexpr (Cfg::TMA) {
+                const int ao = ks ? ta_off1 : ta_off0, bo = ks ? tb_off1 : tb_off0;
 #pragma unroll
-            for (int i = 0; i < MI; i++) {
-                double2 v = *reinterpret_cast<const double2*>(sS + a_off + 8 * i * LDA_S + 8 * ks);
-                fa[buf][i][0] = v.x; fa[buf][i][1] = v.y;
-            }
+                for (int i = 0; i < MI; i++) {
+                    double2 v = *reinterpret_cast<const double2*>(sS + ao + 8 * 16 * i);
+                    fa[buf][i][0] = v.x; fa[buf][i][1] = v.y;
+                }
 #pragma unroll
-            for (int j = 0; j < NJ; j++) {
-                double2 v = *reinterpret_cast<const double2*>(sS + b_off + 16 * j + 4 * ks * LDB_S);
-                fb[buf][j][0] = v.x; fb[buf][j][1] = v.y;
+                for (int j = 0; j < NJ; j++) {
+                    double2 v = *reinterpret_cast<const double2*>(sS + bo + 128 * j);
+                    fb[buf][j][0] = v.x; fb[buf][j][1] = v.y;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < MI; i++) {
+                    double2 v = *reinterpret_cast<const double2*>(sS + a_off + 8 * i * LDA_S + 8 * ks);
+                    fa[buf][i][0] = v.x; fa[buf][i][1] = v.y;
+                }
+#pragma unroll
+                for (int j = 0; j < NJ; j++) {
+                    double2 v = *reinterpret_cast<const double2*>(sS + b_off + 16 * j + 4 * ks * LDB_S);
+                    fb[buf][j][0] = v.x; fb[buf][j][1] = v.y;
+                }
             }
         };
-        cp_async_wait<STAGES - 2>();
+        auto stage_landed = [&](int kt) {                 // stage kt is complete in shared memory (for this thread)
+            if constexpr (Cfg::TMA) g_mbar_wait(tma_bars + 8u * (kt % STAGES), (unsigned)((kt / STAGES) & 1));
+        };
+        if constexpr (Cfg::TMA) { if (KT > 0) stage_landed(0); } else cp_async_wait<STAGES - 2>();
         __syncthreads();
         if (KT > 0) load_frag(0, smem, 0);
         int cur = 0;
@@ -267,7 +344,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
             for (int ks = 0; ks < KS; ks++) {
                 if (ks == KS - 1) {
                     // stage kt+1 must have landed (groups committed so far: STAGES-1+kt; needed complete: kt+2)
-                    cp_async_wait<STAGES - 3>();
+                    if constexpr (Cfg::TMA) { if (kt + 1 < KT) stage_landed(kt + 1); } else cp_async_wait<STAGES - 3>();
                     __syncthreads();
                     int nk = kt + STAGES - 1;
                     if (nk < KT) load_stage(nk, nk % STAGES);      // slot (kt-1) % STAGES: everyone is past stage kt-1
@@ -340,7 +417,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
             }
         }
     } else {
-        const cplx Ee = p.E[z >> 1];
+        const cplx Ee = p.E[z >> p.eshift];
         const cplx* __restrict__ Sg = bptr(p.S, z);
         const cplx* __restrict__ Hg = bptr(p.H, z);
 #pragma unroll
@@ -365,20 +442,56 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
     }
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*TmapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static TmapEncodeFn tmap_encode_fn() {
+    static TmapEncodeFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = (TmapEncodeFn)p;
+    }
+    return fn;
+}
+// rows x cols complex (row-major, ld) x batch (stride in complex elements) seen as FLOAT64 [batch][rows][2 cols]
+static bool tmap_make(CUtensorMap* m, const cplx* base, long long rows, long long cols, long long ld, long long bstride, int batch,
+                      int box_rows) {
+    TmapEncodeFn fn = tmap_encode_fn();
+    if (!fn || rows < 1 || cols < 1) return false;
+    if (batch <= 1 || bstride <= 0) bstride = rows * ld;
+    cuuint64_t dims[3] = {(cuuint64_t)(2 * cols), (cuuint64_t)rows, (cuuint64_t)(batch < 1 ? 1 : batch)};
+    cuuint64_t strides[2] = {(cuuint64_t)ld * 16, (cuuint64_t)bstride * 16};
+    cuuint32_t box[3] = {16, (cuuint32_t)box_rows, 1}, es[3] = {1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <class Cfg, int EPI>
 static cudaError_t gemm3m_launch_t(GemmArgs a, int batch, cudaStream_t st) {
     auto kern = zgemm3m_kernel<Cfg, EPI>;
+    constexpr int SMEM = Cfg::TMA ? Cfg::TMA_SMEM_BYTES : Cfg::SMEM_BYTES;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     a.tiles_m = (a.M + Cfg::BM - 1) / Cfg::BM;
     a.tiles_n = (a.N + Cfg::BN - 1) / Cfg::BN;
     if (a.tiles_m == 0 || a.tiles_n == 0 || batch == 0) return cudaSuccess;
+    GemmTmaMaps tm;
+    if constexpr (Cfg::TMA) {
+        if (!tmap_make(&tm.a, a.A.p0, a.M, a.K, a.lda, a.A.s_in, batch, Cfg::BM) ||
+            !tmap_make(&tm.b, a.B.p0, a.K, a.N, a.ldb, a.B.s_in, batch, 8))
+            return cudaErrorInvalidValue;
+    } else {
+        memset(&tm, 0, sizeof(tm));
+    }
     dim3 grid((unsigned)(a.tiles_m * a.tiles_n), (unsigned)batch, 1);
-    kern<<<grid, Cfg::NT, Cfg::SMEM_BYTES, st>>>(a);
+    kern<<<grid, Cfg::NT, SMEM, st>>>(a, tm);
     return cudaGetLastError();
 }
 
@@ -389,11 +502,13 @@ static cudaError_t gemm3m_launch_t(GemmArgs a, int batch, cudaStream_t st) {
 // ring) are recorded in that file and are no longer built.
 using C3_64x32s4 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3>;      // 4 warps of 32x16, 4-stage ring, 3 CTAs/SM
 using C3_64x32pf = Gemm3Cfg<64, 32, 2, 2, 8, 4, 2, 1>;   // 4 warps of 32x16, cross-stage fragment prefetch, 220 registers, 2 CTAs/SM
+using C3_64x32tma = Gemm3Cfg<64, 32, 2, 2, 8, 4, 2, 1, 1>;  // the same main loop, operand tiles staged by TMA (experiment)
+using C3_64x32tma3 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3, 1, 1>; // same at 3 CTAs/SM (the TMA build needs 168 registers)
 using C3_Tall = Gemm3Cfg<128, 16, 4, 1, 8, 4, 2>;        // one CTA owns all (<=128) rows of its 16 columns: in-place L^-1 * A12
 
 // GEMM variants: 0 = 4M (zgemm.cuh), 1 = 3M, kernel chosen by K (the default), 2 / 3 = the two 3M kernels for every K.
 // GEMM_TALL always maps to the one-CTA-per-column configuration of the same arithmetic.
-enum { GV_4M = 0, GV_3M = 1, GV_3M_LEAN = 2, GV_3M_PF = 3, GV_COUNT = 4 };
+enum { GV_4M = 0, GV_3M = 1, GV_3M_LEAN = 2, GV_3M_PF = 3, GV_3M_TMA = 4, GV_3M_TMA3 = 5, GV_COUNT = 6 };
 
 template <class Cfg>
 static cudaError_t gemm3m_epi(const GemmArgs& a, int batch, int epi, cudaStream_t st) {
@@ -409,6 +524,13 @@ static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, c
     // another 1-2 % faster (44.2 / 44.6 at 2048^3 / 4096^3); the crossover measured on isolated launches lies near
     // K = 1200, inside the solve (4 stream groups) K >= 768 is at least as good (profiles/r01_gemm_variants.md)
     if (variant == GV_3M) variant = (a.K >= 768) ? GV_3M_PF : GV_3M_LEAN;
+    if (variant == GV_3M_TMA || variant == GV_3M_TMA3) {
+        // TMA tensor maps describe uniformly strided batches of whole matrices; anything else takes the cp.async kernel
+        const bool ok = !a.A.two && !a.B.two && a.A.n_in >= batch && a.B.n_in >= batch && a.K > 0 &&
+                        (batch <= 1 || (a.A.s_in > 0 && a.B.s_in > 0));
+        if (ok) return variant == GV_3M_TMA3 ? gemm3m_epi<C3_64x32tma3>(a, batch, epi, st) : gemm3m_epi<C3_64x32tma>(a, batch, epi, st);
+        variant = GV_3M_PF;
+    }
     if (variant == GV_3M_PF) return gemm3m_epi<C3_64x32pf>(a, batch, epi, st);
     return gemm3m_epi<C3_64x32s4>(a, batch, epi, st);
 }

@@ -69,3 +69,61 @@ def broadcast_hamiltonian(tensors, src: int, world: int):
         v = torch.view_as_real(t) if t.is_complex() else t
         dist.broadcast(v, src=src)
     return tensors
+
+
+# ---------------------------------------------------------------------------------------------------------
+# ONE energy batch on TWO GPUs, one block column of A^-1 per GPU
+# ---------------------------------------------------------------------------------------------------------
+# computing the first and the last block column of A^-1 "naturally scale[s] to two accelerators"; L175:
+# R and Cy are built on the accelerators holding the first / last partition, z is solved for and distributed.
+#
+# Partition (world = 2, or pairs of ranks of a larger job):  rank 0 of the pair runs the first-column sweep (Q_i), rank 1
+# the last-column sweep (P_i), both with a full replica of H and S.  Exchange: the corner blocks (blocks 1 and nb of each
+# column, [n_energy][2][bs][bs] per rank) by one all-gather inside the pair; the 2bs x 2bs corner system is then built and
+# solved REDUNDANTLY on both ranks (it needs all four corner blocks and costs ~1/nb of a sweep), so no broadcast of its
+# solution is needed; each rank forms its share of X = Q w_top + P w_bot and one sum-all-reduce inside the pair completes
+# X on both.  Bytes crossing the link per energy: 4 bs^2 * 16 (corners) + nb * bs * nrhs * 16 (X shares).
+#
+# `engine` supplies the per-rank work, so that the same orchestration runs over the CUDA library on GPUs (nccl) and over
+# a CPU stand-in in the world-size-2 gloo test:
+#     engine.sweep(column)                           a0-a4 for that block column
+#     engine.corners(column)        -> tensor [n_energy, 2, bs, bs]
+#     engine.post(column, peer_corners) -> (X_part tensor [n_energy, n, nrhs], T numpy [n_energy])
+
+def column_of_rank(rank: int) -> int:
+    """Which block column a rank of a pair owns: even ranks the first (Q), odd ranks the last (P)."""
+    return rank & 1
+
+
+def column_split_solve(engine, rank: int, group=None):
+    """Runs the two-GPU split of one energy batch on this rank and returns (X, T) complete on both ranks of the pair.
+    `group`: the process group of the pair (None = the default group, which must then have exactly 2 ranks)."""
+    import torch
+    import torch.distributed as dist
+    col = column_of_rank(rank)
+    engine.sweep(col)
+    mine = engine.corners(col).contiguous()
+    both = [torch.empty_like(mine), torch.empty_like(mine)]
+    dist.all_gather([torch.view_as_real(t) for t in both], torch.view_as_real(mine), group=group)
+    X_part, T = engine.post(col, both[1 - col])
+    if X_part is not None:
+        dist.all_reduce(torch.view_as_real(X_part), op=dist.ReduceOp.SUM, group=group)
+    return X_part, T
+
+
+class LibraryColumnEngine:
+    """The CUDA library behind column_split_solve: one SplitSolve handle per rank, device tensors, the current stream."""
+
+    def __init__(self, ss, E, Sigma_L, Sigma_R, Inj_first, Inj_last=None):
+        self.ss, self.E = ss, E
+        self.args = (Sigma_L, Sigma_R, Inj_first, Inj_last)
+
+    def sweep(self, column):
+        self.ss.sweep_column(self.E, column)
+
+    def corners(self, column):
+        return self.ss.corner_blocks(column)
+
+    def post(self, column, peer):
+        X = self.ss.post_column(column, peer.contiguous(), *self.args)
+        return X, self.ss.transmission()

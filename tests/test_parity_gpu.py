@@ -57,9 +57,9 @@ def check_against_oracle(p, out, energies=None, solver=dense):
 @pytest.mark.parametrize("M,N,K,batch", [(64, 64, 64, 1), (1, 1, 1, 2), (37, 53, 29, 3), (130, 70, 200, 2),
                                          (200, 16, 3, 2), (5, 300, 17, 1), (64, 64, 0, 1),
                                          (520, 530, 1030, 1)])
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
 def test_zgemm_batched_vs_numpy(lib, M, N, K, batch, variant):
-    """Every GEMM variant (0 = 4M, 1 = 3M chosen by K, 2 / 3 = the two 3M kernels) against numpy.matmul, normwise bound (3M's error bound is
+    """Every GEMM variant (0 = 4M, 1 = 3M chosen by K, 2 / 3 = the two 3M kernels, 4 / 5 = the TMA-staged experiment) against numpy.matmul, normwise bound (3M's error bound is
     normwise, not componentwise: Higham, Accuracy and Stability of Numerical Algorithms, §23.2.4)."""
     A = inputs.complex_gaussian(1, 50, M, (batch, M, K), 1.0)
     B = inputs.complex_gaussian(1, 51, N, (batch, K, N), 1.0)
@@ -629,3 +629,45 @@ def test_config2_definite_real_energy_variant(lib):
             assert residual.backward_error(*oracle_args(p, e), out["X"][e]) <= TOL_BWD, (mode, e)
         assert residual.rel_frobenius(out["X"][1], rb["X"]) <= TOL_X
         assert residual.rel_T(out["T"][1], rb["T_LR"]) <= TOL_T
+
+
+# ------------------------------------------------------------------------------------------------------
+# one block column of A^-1 per GPU -- the library's split-phase calls, both "ranks"
+# emulated on one GPU (two handles, the exchange by tensor copies); the 2-rank orchestration itself runs in
+# tests/test_column_split_gloo.py
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb,n_e,nrhs,inj_last,groups", [(16, 8, 4, 4, False, 4), (150, 4, 3, 21, True, 2), (70, 5, 5, 9, True, 1)])
+def test_column_split_calls_vs_oracle(lib, bs, nb, n_e, nrhs, inj_last, groups):
+    p = inputs.random_problem(bs, nb, n_e, nrhs, seed=42, inj_last=inj_last)
+    sl, sr, i1, i2 = dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first), dev(p.Inj_last)
+    hs = [dev(a) for a in (p.H_diag, p.H_upper, p.S_diag, p.S_upper)]
+    ranks = []
+    for col in range(2):
+        ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+        ss.set_option("stream_groups", groups)
+        ss.set_hamiltonian(*hs)
+        with pytest.raises(lib.SplitSolveError):                   # post before sweep
+            ss.post_column(col, torch.zeros((n_e, 2, bs, bs), dtype=torch.complex128, device="cuda"), sl, sr, i1, i2)
+        ss.sweep_column(p.E, col)
+        ranks.append((ss, ss.corner_blocks(col)))
+    parts, Ts = [], []
+    for col in range(2):
+        ss = ranks[col][0]
+        with pytest.raises(lib.SplitSolveError):                   # the other column was not swept on this handle
+            ss.post_column(1 - col, ranks[col][1], sl, sr, i1, i2)
+        parts.append(ss.post_column(col, ranks[1 - col][1], sl, sr, i1, i2))
+        Ts.append(ss.transmission())
+    X = (parts[0] + parts[1]).cpu().numpy()
+    assert np.array_equal(Ts[0], Ts[1])                            # the corner system is solved redundantly, same arithmetic
+    check_against_oracle(p, dict(X=X, T=Ts[0]))
+    # corner blocks are blocks 1 and nb of the inverse block columns
+    for e in range(n_e):
+        Q, P = dense.inverse_columns(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+        c0, c1 = ranks[0][1][e].cpu().numpy(), ranks[1][1][e].cpu().numpy()
+        assert residual.rel_frobenius(c0[0], Q[0]) <= TOL_X and residual.rel_frobenius(c0[1], Q[-1]) <= TOL_X
+        assert residual.rel_frobenius(c1[0], P[0]) <= TOL_X and residual.rel_frobenius(c1[1], P[-1]) <= TOL_X
+    # and the whole solve on one handle still gives the same X (different summation order of the two shares: rounding only)
+    ref = run_gpu(lib, p)
+    assert np.abs(ref["X"] - X).max() <= 1e-12 * np.abs(X).max() and np.allclose(ref["T"], Ts[0], rtol=1e-12)
+    for ss, _ in ranks:
+        ss.close()
