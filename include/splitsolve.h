@@ -251,6 +251,10 @@ ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X_dev, int nrhs, doubl
  * 2 CTAs/SM from K = 768);  2 / 3 = those two 3M kernels for every K.  The process-wide default (initially 1) applies to
  * handles created afterwards and to the handle-less building blocks above. */
 ss_status_t ss_set_default_gemm_variant(int variant);
+
+/* Tile rows per raster group of the GEMM kernels (1..64, default 8; process-wide): the CTAs of that many tile rows run
+ * side by side and share the B column tiles in L2.  Tuning knob; profiles/r02_gemm_tma.md has the DRAM traffic it controls. */
+ss_status_t ss_set_gemm_raster(int tile_rows);
 int ss_get_default_gemm_variant(void);
 
 /* FP64 pipe microbenchmark (register-resident mma.sync.m8n8k4.f64 chains on all SMs): returns sustained

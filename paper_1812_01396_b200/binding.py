@@ -53,6 +53,7 @@ SIGNATURES = {
     "ss_bond_current": (c_int, [c_void_p, c_void_p, c_int, c_void_p]),
     "ss_set_default_gemm_variant": (c_int, [c_int]),
     "ss_get_default_gemm_variant": (c_int, []),
+    "ss_set_gemm_raster": (c_int, [c_int]),
 }
 
 _lib = None
@@ -325,6 +326,10 @@ GEMM_VARIANTS = {0: "4M 64x64", 1: "3M 64x32 (3 CTAs/SM for K<768, software-pipe
 
 def set_default_gemm_variant(variant: int):
     _check(load().ss_set_default_gemm_variant(int(variant)), "ss_set_default_gemm_variant")
+
+
+def set_gemm_raster(tile_rows: int):
+    _check(load().ss_set_gemm_raster(int(tile_rows)), "ss_set_gemm_raster")
 
 
 def get_default_gemm_variant() -> int:

@@ -281,6 +281,10 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         h->growth_limit = value; return SS_OK;
     }
     if (!strcmp(name, "panel_fused")) { g_panel_fused = value ? 1 : 0; return SS_OK; }      // process-wide (tuning)
+    if (!strcmp(name, "gemm_raster")) {                                                       // process-wide (tuning)
+        if (value < 1 || value > 64) return SS_ERR_INVALID_ARG;
+        g_gemm_raster = value; return SS_OK;
+    }
     if (!strcmp(name, "gemm_variant")) {
         if (value < 0 || value >= GV_COUNT) return SS_ERR_INVALID_ARG;
         h->gemm_variant = value; return SS_OK;
@@ -1011,6 +1015,12 @@ extern "C" ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X, int nrhs
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx.st);
     cudaFree(J_dev);
     if (e != cudaSuccess || ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_set_gemm_raster(int tile_rows) {
+    if (tile_rows < 1 || tile_rows > 64) return SS_ERR_INVALID_ARG;
+    g_gemm_raster = tile_rows;
     return SS_OK;
 }
 

@@ -34,7 +34,10 @@ struct GemmArgs {
     // tri != 0: only the tiles that touch the lower triangle are computed (Hermitian updates): element
     // (i, j) of C is at global position (tri_row0 + i, tri_col0 + j); a tile whose every column lies right of its last row is skipped
     int tri, tri_row0, tri_col0;
+    int raster_gm;             // tile rows per raster group (set by the launcher)
 };
+
+static int g_gemm_raster = 8;  // process-wide (tuning): profiles/r02_gemm_tma.md
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc, int src_bytes) {
     unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -76,10 +79,10 @@ __global__ void __launch_bounds__(Cfg::NT, MINB) zgemm_kernel(const GemmArgs p) 
     const int g = lane >> 2, t = lane & 3;
     const int z = blockIdx.y;
 
-    // grouped rasterisation: 8 tile rows share the B columns in L2
+    // grouped rasterisation: raster_gm tile rows share the B columns in L2
     int tile_m, tile_n;
     {
-        constexpr int GM = 8;
+        const int GM = p.raster_gm;
         int pid = blockIdx.x;
         int per_group = GM * p.tiles_n;
         int group = pid / per_group;
@@ -245,6 +248,7 @@ static cudaError_t gemm_launch_t(GemmArgs a, int batch, cudaStream_t st) {
     }
     a.tiles_m = (a.M + BM - 1) / BM;
     a.tiles_n = (a.N + BN - 1) / BN;
+    a.raster_gm = g_gemm_raster;
     if (a.tiles_m == 0 || a.tiles_n == 0 || batch == 0) return cudaSuccess;
     dim3 grid((unsigned)(a.tiles_m * a.tiles_n), (unsigned)batch, 1);
     kern<<<grid, Cfg::NT, Cfg::SMEM_BYTES, st>>>(a);

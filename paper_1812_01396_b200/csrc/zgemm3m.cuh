@@ -88,10 +88,10 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
     const int g = lane >> 2, t = lane & 3;
     const int z = blockIdx.y;
 
-    // grouped rasterisation: 8 tile rows share the B columns in L2
+    // grouped rasterisation: raster_gm tile rows share the B columns in L2
     int tile_m, tile_n;
     {
-        constexpr int GM = 8;
+        const int GM = p.raster_gm;
         int pid = blockIdx.x;
         int per_group = GM * p.tiles_n;
         int group = pid / per_group;
@@ -481,6 +481,7 @@ static cudaError_t gemm3m_launch_t(GemmArgs a, int batch, cudaStream_t st) {
     }
     a.tiles_m = (a.M + Cfg::BM - 1) / Cfg::BM;
     a.tiles_n = (a.N + Cfg::BN - 1) / Cfg::BN;
+    a.raster_gm = g_gemm_raster;
     if (a.tiles_m == 0 || a.tiles_n == 0 || batch == 0) return cudaSuccess;
     GemmTmaMaps tm;
     if constexpr (Cfg::TMA) {

@@ -1041,7 +1041,7 @@ struct LuCall {
 static void lu_perm_build(const LuCall& L, int piv_lo, int piv_hi) {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(perm_build_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        cudaFuncSetAttribute(perm_build_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);   // n, npiv <= 8192: (2 * 8192 + 1) ints
         configured = true;
     }
     const int n = L.n, npiv = piv_hi - piv_lo;
