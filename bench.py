@@ -82,7 +82,7 @@ def parse():
     ap.add_argument("--dims", type=int, nargs="*", default=[], help="--kernel gemm: M N K batch [reps]; --kernel density: "
                     "n_energy n nrhs [reps]")
     ap.add_argument("--beta", type=float, default=0.0, help="--kernel gemm: C = A B + beta C (1 = the in-place update form)")
-    ap.add_argument("--raster", type=int, default=None, help="--kernel gemm: tile rows per raster group (library default 8)")
+    ap.add_argument("--raster", type=int, default=None, help="--kernel gemm: tile rows per raster group (library default 16)")
     ap.add_argument("--variants", default=None, help="--kernel gemm: comma-separated GEMM variants (default: library default)")
     ap.add_argument("--calibrate-oracle", action="store_true", help="time the oracle on the full and on the truncated C2 "
                     "device (one energy, Inj columns only) and print the ratio that the extrapolated cpu_baseline rests on")

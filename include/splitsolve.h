@@ -155,7 +155,10 @@ double ss_flops_sweep(ss_handle_t h);
  * Meaningful after ss_synchronize / ss_transmission. */
 ss_status_t ss_last_mode(ss_handle_t h, int* mode, int* retried);
 
-/* Device bytes the handle allocates for (nb, bs, n_energy, nrhs), excluding caller-owned inputs/outputs. */
+/* Device bytes the handle allocates for the solve workspace of (nb, bs, n_energy, nrhs) in the default (fully device-
+ * resident) mode.  Not included: caller-owned inputs/outputs; the device copies of H, S that ss_set_hamiltonian_host makes
+ * (4 nb bs^2 * 16 B) and the staging buffers of ss_solve_host (Sigma, Inj, X); with option "offload_columns" the block
+ * columns shrink from 2 (nb+1) to 2 * ring blocks per energy and move to pinned host memory instead. */
 size_t ss_workspace_bytes(int nb, int bs, int n_energy, int nrhs);
 
 /* Device time in milliseconds of the phases of the last ss_solve (CUDA events on its stream):
@@ -189,6 +192,13 @@ ss_status_t ss_gemm_profile(ss_handle_t h, double* ms, double* flops, long long*
  * modes 1 and 2 lose digits in proportion to kappa(A) (backward errors 1e-11 .. 1e-4 on the random test devices against
  * 1e-15 .. 1e-12 for mode 0).  They are exact on the perfect chain (config 1) and meet the tolerances when A is
  * definite (energies outside the spectrum).  Hence off by default.
+ * "offload_columns" (0, 1 or a ring size 6..64; default 0; only before the first solve of the handle; SURVEY.md 8(f4),
+ * part of Q kept on the host, "the time to transfer ... hidden"): the 2 nb blocks X_i / Y_i -> Q_i / P_i of
+ * every energy live in pinned HOST memory owned by the handle (n_energy * 2 (nb+1) bs^2 * 16 B) and the device keeps a ring of
+ * `ring` blocks per chain (default 6): every block is written back as soon as it is produced, fetched back two steps ahead
+ * for the column recursion a4 and block by block for a6, on a copy stream per stream group, ordered by events only.
+ * Device memory for the block columns drops from 2 (nb+1) to 2 * ring blocks per energy; results are bit-identical.
+ * ss_inverse_columns is not available in this mode (use ss_copy_inverse_columns).
  * "transmission" (0/1, default 1:
  * compute T(E) in ss_solve), "profile_gemm" (0/1, default 0), "gemm_variant" (see ss_set_default_gemm_variant;
  * default = the process-wide default at ss_create), "trace" (0/1, default 0: record a CUDA-event
@@ -252,7 +262,7 @@ ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X_dev, int nrhs, doubl
  * handles created afterwards and to the handle-less building blocks above. */
 ss_status_t ss_set_default_gemm_variant(int variant);
 
-/* Tile rows per raster group of the GEMM kernels (1..64, default 8; process-wide): the CTAs of that many tile rows run
+/* Tile rows per raster group of the GEMM kernels (1..64, default 16; process-wide): the CTAs of that many tile rows run
  * side by side and share the B column tiles in L2.  Tuning knob; profiles/r02_gemm_tma.md has the DRAM traffic it controls. */
 ss_status_t ss_set_gemm_raster(int tile_rows);
 int ss_get_default_gemm_variant(void);

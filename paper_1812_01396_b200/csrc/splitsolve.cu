@@ -24,6 +24,14 @@ struct ss_handle_s {
     int hermitian = 0;               // SURVEY 8(f1) at real energies: 0 off, 1 Hermitian Schur update, 2 + no-pivot L Delta L^H
     int growth_limit = 64;           // mode 2: largest multiplier tolerated before the solve is redone with the pivoted LU
     int mode = 0;                    // what the last ss_solve used
+    // block columns kept in pinned HOST memory, a ring of device slots per chain
+    int offload = 0;                 // option "offload_columns"
+    int ring = 6;                    // device slots per chain in that mode (>= 6: 3 in use + 2 prefetched + 1 slack)
+    cplx* host_cols = nullptr;       // pinned [n_energy][2][nb+1][bs*bs]
+    cplx* corner = nullptr;          // device [n_energy][2 columns][first / last block][bs*bs]
+    struct GroupCopy { cudaStream_t st = nullptr; std::vector<cudaEvent_t> ev_slot[2]; std::vector<cudaEvent_t> ev_step; };
+    std::vector<GroupCopy> gcopy;    // per stream group: its copy stream, one event per (column, ring slot), step events
+    int slots_per_chain() const { return offload ? ring : nb + 1; }
     int swept_cols = 0;              // block columns the last sweep computed (3 = both; 1 / 2: ss_sweep_column)
     bool whole_solve = true;         // the last post-processing belonged to an ss_solve (so a redo is possible)
     bool force_general = false;      // set while a solve is being redone
@@ -80,7 +88,9 @@ static void free_dev(void* p) { if (p) cudaFree(p); }
 static void free_workspace(ss_handle_t h) {
     free_dev(h->slots); free_dev(h->aug); free_dev(h->aop); free_dev(h->tinv); free_dev(h->raug); free_dev(h->wz);
     free_dev(h->gam_l); free_dev(h->gam_r); free_dev(h->g1n); free_dev(h->w1); free_dev(h->w2); free_dev(h->E_dev);
-    free_dev(h->tpart); free_dev(h->T_dev); free_dev(h->ipiv); free_dev(h->info); free_dev(h->perm);
+    free_dev(h->tpart); free_dev(h->T_dev); free_dev(h->ipiv); free_dev(h->info); free_dev(h->perm); free_dev(h->corner);
+    if (h->host_cols) cudaFreeHost(h->host_cols);
+    h->corner = nullptr; h->host_cols = nullptr;
     h->slots = h->aug = h->aop = h->tinv = h->raug = h->wz = nullptr;
     h->gam_l = h->gam_r = h->g1n = h->w1 = h->w2 = h->E_dev = nullptr;
     h->tpart = h->T_dev = nullptr; h->ipiv = h->info = h->perm = nullptr;
@@ -96,10 +106,10 @@ struct WsSizes {
 // system (n = 2bs); every stream group owns the slice of its energies
 static inline size_t perm_ints_per_energy(int bs) { return ((size_t)2 * (3 * (size_t)bs + 1) + 7) / 4 * 4 + 4; }
 
-static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
+static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs, int slots_per_chain = 0) {
     WsSizes w;
     const size_t B2 = (size_t)bs * bs, C = sizeof(cplx);
-    w.slots = (size_t)nE * 2 * (nb + 1) * B2 * C;
+    w.slots = (size_t)nE * 2 * (slots_per_chain ? slots_per_chain : nb + 1) * B2 * C;
     w.aug = (size_t)nE * 2 * bs * pad_ld(2 * bs) * C;
     w.aop = (size_t)nE * 2 * B2 * C;
     // the sweep and the corner system own disjoint regions: stream groups do not wait for one another between the two
@@ -123,7 +133,7 @@ static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs) {
 // allocated once and survives a later call with more right-hand sides (ss_sweep_column knows no nrhs yet, and the sweep's
 // results must outlive the allocation ss_post_column makes).
 static ss_status_t ensure_workspace(ss_handle_t h, int nrhs) {
-    WsSizes w = ws_sizes(h->nb, h->bs, h->n_energy, nrhs);
+    WsSizes w = ws_sizes(h->nb, h->bs, h->n_energy, nrhs, h->slots_per_chain());
     bool ok = true;
     auto A = [&](void** p, size_t bytes) { if (ok && cudaMalloc(p, bytes ? bytes : 16) != cudaSuccess) ok = false; };
     if (!h->slots) {
@@ -131,6 +141,11 @@ static ss_status_t ensure_workspace(ss_handle_t h, int nrhs) {
         A((void**)&h->gam_l, w.sq); A((void**)&h->gam_r, w.sq); A((void**)&h->g1n, w.sq); A((void**)&h->w1, w.sq);
         A((void**)&h->w2, w.sq); A((void**)&h->E_dev, w.E); A((void**)&h->tpart, w.tpart); A((void**)&h->T_dev, w.T);
         A((void**)&h->ipiv, w.ipiv); A((void**)&h->info, w.info); A((void**)&h->perm, w.perm);
+        if (h->offload) {
+            A((void**)&h->corner, (size_t)h->n_energy * 4 * h->bs * h->bs * sizeof(cplx));
+            if (ok && cudaMallocHost((void**)&h->host_cols, (size_t)h->n_energy * 2 * (h->nb + 1) * h->bs * h->bs * sizeof(cplx)) != cudaSuccess)
+                ok = false;
+        }
         if (!ok) { cudaGetLastError(); free_workspace(h); return SS_ERR_ALLOC; }
     }
     if (h->ws_nrhs < nrhs) {
@@ -200,6 +215,11 @@ extern "C" ss_status_t ss_destroy(ss_handle_t h) {
         if (g.ev_mark) cudaEventDestroy(g.ev_mark);
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    for (auto& c : h->gcopy) {
+        if (c.st) cudaStreamDestroy(c.st);
+        for (int q = 0; q < 2; q++) for (cudaEvent_t e : c.ev_slot[q]) cudaEventDestroy(e);
+        for (cudaEvent_t e : c.ev_step) cudaEventDestroy(e);
+    }
     if (h->main_stream) cudaStreamDestroy(h->main_stream);
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     for (cudaEvent_t e : h->up_ev) cudaEventDestroy(e);
@@ -272,6 +292,14 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         h->stream_groups = value; return SS_OK;
     }
     if (!strcmp(name, "trace")) { h->want_trace = value ? 1 : 0; return SS_OK; }
+    if (!strcmp(name, "offload_columns")) {
+        // changes the layout of the workspace: only before the first solve
+        if (h->slots) return SS_ERR_NOT_READY;
+        if (value != 0 && (value < 6 || value > 64) && value != 1) return SS_ERR_INVALID_ARG;
+        h->offload = value ? 1 : 0;
+        h->ring = value > 1 ? value : 6;
+        return SS_OK;
+    }
     if (!strcmp(name, "hermitian")) {
         if (value < 0 || value > 2) return SS_ERR_INVALID_ARG;
         h->hermitian = value; return SS_OK;
@@ -335,6 +363,41 @@ static void launch_form(Ctx& ctx, FormSide s0, FormSide s1, const cplx* E, BPtr 
     ctx.note(cudaGetLastError());
 }
 
+// ---- slot addressing.  Full mode: [n_energy][2][nb+1] blocks, logical slot = physical slot.  Offload mode (SURVEY.md 8(f4),
+// part of Q on the host, "transfers overlapped"): [n_energy][2][ring] blocks, logical slot idx lives in
+// ring slot idx % ring while it is in use; every block is also written to the pinned host array host_cols[e][col][idx].
+static inline long long slot_stride_e(const ss_handle_s* h) { return 2LL * h->slots_per_chain() * h->bs * h->bs; }
+static inline cplx* slot_ptr(const ss_handle_s* h, int e0, int col, int idx) {
+    const long long B2 = (long long)h->bs * h->bs;
+    const int spc = h->slots_per_chain();
+    return h->slots + (long long)e0 * slot_stride_e(h) + ((long long)col * spc + (h->offload ? idx % spc : idx)) * B2;
+}
+static inline cplx* host_ptr(const ss_handle_s* h, int e0, int col, int idx) {
+    const long long B2 = (long long)h->bs * h->bs;
+    return h->host_cols + ((long long)e0 * 2 * (h->nb + 1) + (long long)col * (h->nb + 1) + idx) * B2;
+}
+
+static bool ensure_offload(ss_handle_t h, int nG) {
+    while ((int)h->gcopy.size() < nG) {
+        ss_handle_s::GroupCopy c;
+        bool ok = cudaStreamCreateWithFlags(&c.st, cudaStreamNonBlocking) == cudaSuccess;
+        for (int q = 0; q < 2 && ok; q++)
+            for (int i = 0; i < h->ring && ok; i++) {
+                cudaEvent_t e;
+                ok = cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+                if (ok) c.ev_slot[q].push_back(e);
+            }
+        for (int i = 0; i < 4 && ok; i++) {
+            cudaEvent_t e;
+            ok = cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+            if (ok) c.ev_step.push_back(e);
+        }
+        h->gcopy.push_back(c);
+        if (!ok) return false;
+    }
+    return true;
+}
+
 // a0-a4: Algorithm 1 and its mirror (L167) for the energies [e0, e0 + nEg) of one stream group, both
 // columns in lockstep.  Chain z = 2*e + col.  Slot layout per chain (nb+1 slots of bs x bs): column 0 keeps X_i in slot i
 // (X_1 in slot 0) and ends with Q_i in slot i-1; column 1 keeps Y_i in slot i-1 (Y_nb in slot nb) and ends with P_i in
@@ -351,14 +414,44 @@ struct Group {
     BPtr ch(const cplx* p0, const cplx* p1, long long s_energy) const {
         return dual() ? bp_chain(p0, p1, s_energy) : bp_strided(cols == 1 ? p0 : p1, s_energy);
     }
+    // ---- offload mode: transfers of logical slot idx of column col for this group's energies, on the group's copy stream
+    ss_handle_s::GroupCopy* cp = nullptr;
+    std::vector<char>* slot_used = nullptr;           // [2][ring]: a transfer event has been recorded for that ring slot in this solve
+    void wait_slot(ss_handle_t h, int col, int idx) { // the compute stream waits for the last transfer that touched that ring slot
+        const int rs = idx % h->ring;
+        if ((*slot_used)[col * h->ring + rs]) cudaStreamWaitEvent(ctx.st, cp->ev_slot[col][rs], 0);
+    }
+    void copy_after_compute(int which) {              // the copy stream waits for everything enqueued so far on the compute stream
+        cudaEventRecord(cp->ev_step[which], ctx.st);
+        cudaStreamWaitEvent(cp->st, cp->ev_step[which], 0);
+    }
+    void xfer(ss_handle_t h, int col, int idx, bool to_host) {
+        const size_t B2b = sizeof(cplx) * (size_t)h->bs * h->bs;
+        cplx* d = slot_ptr(h, e0, col, idx);
+        cplx* hp = host_ptr(h, e0, col, idx);
+        const size_t dp = sizeof(cplx) * (size_t)slot_stride_e(h), hpitch = 2 * (size_t)(h->nb + 1) * B2b;
+        cudaError_t e = to_host ? cudaMemcpy2DAsync(hp, hpitch, d, dp, B2b, (size_t)nE, cudaMemcpyDeviceToHost, cp->st)
+                                : cudaMemcpy2DAsync(d, dp, hp, hpitch, B2b, (size_t)nE, cudaMemcpyHostToDevice, cp->st);
+        if (ctx.err == cudaSuccess && e != cudaSuccess) ctx.err = e;
+        const int rs = idx % h->ring;
+        cudaEventRecord(cp->ev_slot[col][rs], cp->st);
+        (*slot_used)[col * h->ring + rs] = 1;
+    }
+    void save_corner(ss_handle_t h, int col, int which, int idx) {     // block 1 / nb of a column -> h->corner (compute stream)
+        const size_t B2b = sizeof(cplx) * (size_t)h->bs * h->bs;
+        cplx* dst = h->corner + (((long long)e0 * 2 + col) * 2 + which) * (long long)h->bs * h->bs;
+        cudaError_t e = cudaMemcpy2DAsync(dst, 4 * B2b, slot_ptr(h, e0, col, idx), sizeof(cplx) * (size_t)slot_stride_e(h), B2b,
+                                          (size_t)nE, cudaMemcpyDeviceToDevice, ctx.st);
+        if (ctx.err == cudaSuccess && e != cudaSuccess) ctx.err = e;
+    }
 };
 
 static void sweep_step(ss_handle_t h, Group& G, int s) {
     Ctx& ctx = G.ctx;
     const int nb = h->nb, bs = h->bs, e0 = G.e0, batch = G.batch(), eshift = G.dual() ? 1 : 0;
     const long long B2 = (long long)bs * bs;
-    const long long s_slot_e = 2LL * (nb + 1) * B2;
-    auto slot = [&](int col, int idx) { return h->slots + (long long)e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
+    const long long s_slot_e = slot_stride_e(h);
+    auto slot = [&](int col, int idx) { return slot_ptr(h, e0, col, idx); };
     const int ldg = pad_ld(2 * bs);
     const long long s_aug_e = 2LL * bs * ldg;
     const BPtr aug = G.ch(h->aug + e0 * s_aug_e, h->aug + e0 * s_aug_e + (long long)bs * ldg, s_aug_e);
@@ -385,7 +478,11 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
     FormSide r1 = (i_m < nb) ? FormSide{h->Su + (long long)(i_m - 1) * B2, h->Hu + (long long)(i_m - 1) * B2, FORM_PLAIN}
                              : FormSide{nullptr, nullptr, FORM_IDENT};
     if (G.cols == 2) r0 = r1;                                  // one sweep only: its side goes first
-    const BPtr out = G.ch(slot(0, i_f >= 2 ? i_f : 0), slot(1, i_m <= nb - 1 ? i_m - 1 : nb), s_slot_e);
+    const int widx[2] = {i_f >= 2 ? i_f : 0, i_m <= nb - 1 ? i_m - 1 : nb};      // logical slots X_i / Y_i go to
+    const BPtr out = G.ch(slot(0, widx[0]), slot(1, widx[1]), s_slot_e);
+    if (h->offload)
+        for (int c = 0; c < 2; c++)
+            if (G.cols & (1 << c)) G.wait_slot(h, c, widx[c]);   // the ring slot's previous content has reached the host
     if (mode == 2) launch_form(ctx, r0, r1, E, bp_offset(aug, bs), ldg, bs, batch, eshift);    // no interchanges: straight into [D | B]
     else launch_form(ctx, r0, r1, E, out, bs, bs, batch, eshift);
     GemmArgs g{};
@@ -417,23 +514,52 @@ static void sweep_step(ss_handle_t h, Group& G, int s) {
     }
     // U half of a3: X_i / Y_i into its slot
     back_substitute(ctx, aug, ldg, bs, bs, out, bs, batch, w);
+    if (h->offload) {
+        if ((G.cols & 1) && i_f == 1) G.save_corner(h, 0, 0, 0);        // Q_1 = X_1
+        if ((G.cols & 2) && i_m == nb) G.save_corner(h, 1, 1, nb);      // P_nb = Y_nb
+        G.copy_after_compute(s & 3);
+        for (int c = 0; c < 2; c++)
+            if (G.cols & (1 << c)) G.xfer(h, c, widx[c], true);
+    }
 }
 
 // a4: Q_i = -X_i Q_{i-1} (i = 2..nb), P_i = -Y_i P_{i+1} (i = nb-1..1); r = 1..nb-1
 static void recursion_step(ss_handle_t h, Group& G, int r) {
     const int nb = h->nb, bs = h->bs, batch = G.batch();
-    const long long B2 = (long long)bs * bs;
-    const long long s_slot_e = 2LL * (nb + 1) * B2;
-    auto slot = [&](int col, int idx) { return h->slots + (long long)G.e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
+    const long long s_slot_e = slot_stride_e(h);
+    auto slot = [&](int col, int idx) { return slot_ptr(h, G.e0, col, idx); };
     const int i0 = r + 1, i1 = nb - r;
+    // logical slots of the product C = -A B: column 0 (X_i0, Q_{i0-1}) -> Q_i0, column 1 (Y_i1, P_{i1+1}) -> P_i1
+    const int ia[2] = {i0, i1 - 1}, ib[2] = {i0 - 2, i1 + 1}, ic[2] = {i0 - 1, i1};
     G.ctx.use(CLS_LO);
-    GemmArgs g = gemm_std(bs, bs, bs, -1.0, G.ch(slot(0, i0), slot(1, i1 - 1), s_slot_e), bs,
-                          G.ch(slot(0, i0 - 2), slot(1, i1 + 1), s_slot_e), bs, 0.0,
-                          G.ch(slot(0, i0 - 1), slot(1, i1), s_slot_e), bs);
+    if (h->offload) {
+        // prefetch the X / Y of step r + 2 from the host into its ring slot: that slot's last reader was step r - 2's product
+        // and its last write-back is earlier on the same copy stream; the first two steps use blocks still resident from the sweep
+        const int L = 2, rp = r + L;
+        if (rp <= nb - 1) {
+            G.copy_after_compute((r + 3) & 3);
+            const int pa[2] = {rp + 1, nb - rp - 1};
+            for (int c = 0; c < 2; c++)
+                if (G.cols & (1 << c)) G.xfer(h, c, pa[c], false);
+        }
+        for (int c = 0; c < 2; c++)
+            if (G.cols & (1 << c)) { G.wait_slot(h, c, ia[c]); G.wait_slot(h, c, ic[c]); }
+    }
+    GemmArgs g = gemm_std(bs, bs, bs, -1.0, G.ch(slot(0, ia[0]), slot(1, ia[1]), s_slot_e), bs,
+                          G.ch(slot(0, ib[0]), slot(1, ib[1]), s_slot_e), bs, 0.0,
+                          G.ch(slot(0, ic[0]), slot(1, ic[1]), s_slot_e), bs);
     gemm_run(G.ctx, g, batch, GEMM_BIG, EPI_STD);
+    if (h->offload) {
+        if (r == nb - 1) {
+            if (G.cols & 1) G.save_corner(h, 0, 1, ic[0]);              // Q_nb
+            if (G.cols & 2) G.save_corner(h, 1, 0, ic[1]);              // P_1
+        }
+        G.copy_after_compute(r & 3);
+        for (int c = 0; c < 2; c++)
+            if (G.cols & (1 << c)) G.xfer(h, c, ic[c], true);
+    }
 }
 
-// a5-a7: corner system, solution, transmission (north_star for T).
 // G.cols == 3: both block columns are in this handle's slots.  G.cols == 1 / 2: only the first / last one
 // is; blocks 1 and nb of the other column come from `peer` ([n_energy][2][bs][bs], written there by the caller after the
 // exchange with the GPU that owns that column), and X receives only this column's share Q_i w_top resp. P_i w_bot.
@@ -442,11 +568,15 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     Ctx& ctx = G.ctx;
     const int nb = h->nb, bs = h->bs, nE = G.nE, e0 = G.e0;
     const long long B2 = (long long)bs * bs;
-    const long long s_slot_e = 2LL * (nb + 1) * B2;
-    auto slot = [&](int col, int idx) { return h->slots + (long long)e0 * s_slot_e + ((long long)col * (nb + 1) + idx) * B2; };
+    const long long s_slot_e = slot_stride_e(h);
+    auto slot = [&](int col, int idx) { return slot_ptr(h, e0, col, idx); };
     // corner blocks [column][first / last block] with their energy strides
     const cplx* cor[2][2] = {{slot(0, 0), slot(0, nb - 1)}, {slot(1, 1), slot(1, nb)}};
     long long cor_s[2] = {s_slot_e, s_slot_e};
+    if (h->offload)                                   // saved aside when they were produced (the ring has moved on)
+        for (int c = 0; c < 2; c++) {
+            cor[c][0] = h->corner + ((long long)e0 * 2 + c) * 2 * B2; cor[c][1] = cor[c][0] + B2; cor_s[c] = 4 * B2;
+        }
     if (G.cols != 3) {
         const int other = (G.cols == 1) ? 1 : 0;
         cor[other][0] = peer + (long long)e0 * 2 * B2; cor[other][1] = cor[other][0] + B2; cor_s[other] = 2 * B2;
@@ -489,7 +619,31 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     lu_factor(ctx, bp_strided(raug, s_r), ldW, 2 * bs, W, nE, w, 0);
     back_substitute(ctx, bp_strided(raug, s_r), ldW, 2 * bs, nr, bp_strided(wz, s_w), nr, nE, w);
     // a6: X_i = Q_i w_top + P_i w_bot, batch z = e*nb + (i-1)
-    if (m > 0) {
+    if (m > 0 && h->offload) {
+        // the block columns come back from the host block by block, two ring slots per column alternating: the copy of
+        // block i+1 runs under the products of block i
+        for (int i = 0; i < nb; i++) {
+            const int li[2] = {i, i + 1};                        // logical slots of Q_{i+1}, P_{i+1}
+            const long long xoff = (long long)i * bs * m, xs = (long long)nb * bs * m;
+            if (i >= 2) cudaStreamWaitEvent(G.cp->st, G.cp->ev_step[i & 1], 0);   // the products of block i-2 are done with this ring slot
+            else if (i == 0) G.copy_after_compute(3);            // ... and the recursion with all of them
+            for (int c = 0; c < 2; c++) {
+                if (!(G.cols & (1 << c))) continue;
+                const size_t B2b = sizeof(cplx) * (size_t)B2;
+                cplx* d = h->slots + (long long)e0 * s_slot_e + ((long long)c * h->ring + (i & 1)) * B2;
+                cudaError_t e = cudaMemcpy2DAsync(d, sizeof(cplx) * (size_t)s_slot_e, host_ptr(h, e0, c, li[c]),
+                                                  2 * (size_t)(nb + 1) * B2b, B2b, (size_t)nE, cudaMemcpyHostToDevice, G.cp->st);
+                if (ctx.err == cudaSuccess && e != cudaSuccess) ctx.err = e;
+                cudaEventRecord(G.cp->ev_slot[c][i & 1], G.cp->st);
+                cudaStreamWaitEvent(ctx.st, G.cp->ev_slot[c][i & 1], 0);
+                GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_strided(d, s_slot_e), bs,
+                                      bp_strided(wz + (c ? (long long)bs * nr : 0), s_w), nr, (c == 1 && (G.cols & 1)) ? 1.0 : 0.0,
+                                      bp_strided(X + xoff, xs), m);
+                gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
+            }
+            cudaEventRecord(G.cp->ev_step[i & 1], ctx.st);
+        }
+    } else if (m > 0) {
         if (G.cols & 1) {
             GemmArgs g = gemm_std(bs, m, bs, 1.0, bp_two_level(slot(0, 0), nb, B2, s_slot_e), bs,
                                   bp_two_level(wz, nb, 0, s_w), nr, 0.0,
@@ -563,10 +717,12 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, int phases,
     // [e0, e0 + nE); the host interleaves the groups' launches step by step so that every group's streams stay fed.
     const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
     std::vector<Group> G((size_t)nG);
+    std::vector<std::vector<char>> slot_used((size_t)nG, std::vector<char>((size_t)2 * h->ring, 0));
     for (int g = 0; g < nG; g++) {
         G[g].e0 = (int)((long long)h->n_energy * g / nG);
         G[g].nE = (int)((long long)h->n_energy * (g + 1) / nG) - G[g].e0;
         G[g].cols = cols;
+        if (h->offload) { G[g].cp = &h->gcopy[g]; G[g].slot_used = &slot_used[g]; }
         Ctx& c = G[g].ctx;
         c.variant = h->gemm_variant;
         c.group = g;
@@ -582,6 +738,10 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, int phases,
             c.st = c.s_lo; c.cls = CLS_LO;
             cudaStreamWaitEvent(c.s_lo, h->ev_fork, 0);
         }
+    }
+    if (h->offload) {                                      // the copy streams join the solve behind its starting point
+        cudaEventRecord(h->ev_in, stream);
+        for (int g = 0; g < nG; g++) cudaStreamWaitEvent(h->gcopy[g].st, h->ev_in, 0);
     }
     for (auto& r : h->trace) { cudaEventDestroy(r.t0); cudaEventDestroy(r.t1); }
     h->trace.clear();
@@ -609,6 +769,11 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, int phases,
             cudaEventRecord(h->groups[g].ev_mark, G[g].ctx.st);
             cudaStreamWaitEvent(stream, h->groups[g].ev_mark, 0);
         }
+    if (h->offload)                                        // the write-backs to the host belong to the solve
+        for (int g = 0; g < nG; g++) {
+            cudaEventRecord(h->gcopy[g].ev_step[0], h->gcopy[g].st);
+            cudaStreamWaitEvent(stream, h->gcopy[g].ev_step[0], 0);
+        }
     for (int g = 0; g < nG; g++) G[g].ctx.trace_close();
     mark(h->ev[2]);
     h->launches = 0;
@@ -632,6 +797,7 @@ static ss_status_t run_phases(ss_handle_t h, const ss_cplx* E_host, int phases, 
     if (st != SS_OK) return st;
     const int nG = h->stream_groups < h->n_energy ? h->stream_groups : h->n_energy;
     if (nG > 1 && !ensure_groups(h, nG)) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (h->offload && !ensure_offload(h, nG)) { cudaGetLastError(); return SS_ERR_CUDA; }
     if (!h->main_stream) {
         if (cudaStreamCreateWithFlags(&h->main_stream, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming) != cudaSuccess ||
@@ -689,11 +855,13 @@ extern "C" ss_status_t ss_get_corner_blocks(ss_handle_t h, int column, ss_cplx* 
     if (!h || !out_dev || column < 0 || column > 1) return SS_ERR_INVALID_ARG;
     if (!h->launched || !(h->swept_cols & (1 << column))) return SS_ERR_NOT_READY;
     const size_t B2 = (size_t)h->bs * h->bs, nb = h->nb;
-    const cplx* base = h->slots + (column ? (nb + 1) * B2 + B2 : 0);          // block 1 of that column of energy 0
+    const cplx* base = h->offload ? h->corner + (size_t)column * 2 * B2      // saved aside when produced: [e][column][2][B2]
+                                  : h->slots + (column ? (nb + 1) * B2 + B2 : 0);   // block 1 of that column of energy 0
+    const size_t spitch = (h->offload ? 4 * B2 : 2 * (nb + 1) * B2) * sizeof(cplx);
     // [n_energy][2][bs][bs]: blocks 1 and nb; one strided 2-D copy per block position
     for (int q = 0; q < 2; q++) {
-        const cplx* src = base + (q ? (nb - 1) * B2 : 0);
-        if (cudaMemcpy2DAsync((cplx*)out_dev + q * B2, 2 * B2 * sizeof(cplx), src, 2 * (nb + 1) * B2 * sizeof(cplx), B2 * sizeof(cplx),
+        const cplx* src = base + (q ? (h->offload ? B2 : (nb - 1) * B2) : 0);
+        if (cudaMemcpy2DAsync((cplx*)out_dev + q * B2, 2 * B2 * sizeof(cplx), src, spitch, B2 * sizeof(cplx),
                               (size_t)h->n_energy, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream) != cudaSuccess) {
             cudaGetLastError(); return SS_ERR_CUDA;
         }
@@ -796,7 +964,7 @@ extern "C" ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int*
 
 extern "C" ss_status_t ss_inverse_columns(ss_handle_t h, int energy, const ss_cplx** Q_first, const ss_cplx** Q_last) {
     if (!h || !Q_first || !Q_last || energy < 0 || energy >= h->n_energy) return SS_ERR_INVALID_ARG;
-    if (!h->solved) return SS_ERR_NOT_READY;
+    if (!h->solved || h->offload) return SS_ERR_NOT_READY;    // offload mode: the columns are on the host (ss_copy_inverse_columns)
     const long long B2 = (long long)h->bs * h->bs;
     const cplx* base = h->slots + (long long)energy * 2 * (h->nb + 1) * B2;
     *Q_first = (const ss_cplx*)base;                                   // column 0, slots 0..nb-1
@@ -805,16 +973,20 @@ extern "C" ss_status_t ss_inverse_columns(ss_handle_t h, int energy, const ss_cp
 }
 
 extern "C" ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cplx* Q_out, ss_cplx* P_out) {
-    const ss_cplx *q = nullptr, *p = nullptr;
-    ss_status_t s = ss_inverse_columns(h, energy, &q, &p);
-    if (s != SS_OK) return s;
-    const size_t bytes = sizeof(cplx) * (size_t)h->nb * h->bs * h->bs;
-    if (Q_out && cudaMemcpyAsync(Q_out, q, bytes, cudaMemcpyDeviceToDevice, h->last_stream) != cudaSuccess) {
-        cudaGetLastError(); return SS_ERR_CUDA;
+    if (!h || energy < 0 || energy >= h->n_energy) return SS_ERR_INVALID_ARG;
+    if (!h->solved) return SS_ERR_NOT_READY;
+    const size_t B2 = (size_t)h->bs * h->bs, bytes = sizeof(cplx) * (size_t)h->nb * B2;
+    const cplx *q, *p;
+    cudaMemcpyKind kind = cudaMemcpyDeviceToDevice;
+    if (h->offload) {                                     // the block columns live in the handle's pinned host array
+        q = host_ptr(h, energy, 0, 0); p = host_ptr(h, energy, 1, 1);
+        kind = cudaMemcpyHostToDevice;
+    } else {
+        const cplx* base = h->slots + (size_t)energy * 2 * (h->nb + 1) * B2;
+        q = base; p = base + (size_t)(h->nb + 1) * B2 + B2;
     }
-    if (P_out && cudaMemcpyAsync(P_out, p, bytes, cudaMemcpyDeviceToDevice, h->last_stream) != cudaSuccess) {
-        cudaGetLastError(); return SS_ERR_CUDA;
-    }
+    if (Q_out && cudaMemcpyAsync(Q_out, q, bytes, kind, h->last_stream) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (P_out && cudaMemcpyAsync(P_out, p, bytes, kind, h->last_stream) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }
 

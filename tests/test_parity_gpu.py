@@ -671,3 +671,62 @@ def test_column_split_calls_vs_oracle(lib, bs, nb, n_e, nrhs, inj_last, groups):
     assert np.abs(ref["X"] - X).max() <= 1e-12 * np.abs(X).max() and np.allclose(ref["T"], Ts[0], rtol=1e-12)
     for ss, _ in ranks:
         ss.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# block columns offloaded to pinned host memory, ring of device slots
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb,n_e,nrhs,groups,ring", [(16, 8, 4, 4, 4, 1), (40, 13, 3, 9, 2, 6), (70, 20, 5, 11, 4, 7),
+                                                         (150, 9, 2, 21, 1, 6), (8, 2, 2, 3, 2, 1), (8, 3, 1, 3, 1, 6)])
+def test_offload_columns_is_bit_identical(lib, bs, nb, n_e, nrhs, groups, ring):
+    """Same arithmetic, other storage: with the block columns on the host and only a ring of device slots, X, T(E) and the
+    inverse block columns must equal the fully resident run bit for bit (nb above, at and below the ring size), and match
+    the oracle."""
+    p = inputs.random_problem(bs, nb, n_e, nrhs, seed=51, inj_last=True)
+    ref = run_gpu(lib, p, want_inverse=True, options={"stream_groups": groups})
+    check_against_oracle(p, ref)
+    for rep in range(2):
+        out = run_gpu(lib, p, want_inverse=True, options={"stream_groups": groups, "offload_columns": ring})
+        assert np.array_equal(out["X"], ref["X"]) and np.array_equal(out["T"], ref["T"]), rep
+        for e in range(n_e):
+            assert np.array_equal(out["QP"][e][0], ref["QP"][e][0]) and np.array_equal(out["QP"][e][1], ref["QP"][e][1]), (rep, e)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    for bad in (2, 5, 65):
+        with pytest.raises(lib.SplitSolveError):
+            ss.set_option("offload_columns", bad)
+    ss.close()
+    assert lib.workspace_bytes(nb, bs, n_e, nrhs) > 0
+
+
+def test_offload_columns_repeated_solves_and_column_split(lib):
+    """Second solve on the same offloading handle with other energies; and the split-phase calls (one block column per
+    handle) on top of the offload."""
+    p = inputs.random_problem(33, 11, 3, 5, seed=52)
+    ss = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+    ss.set_option("offload_columns", 1)
+    ss.set_hamiltonian(dev(p.H_diag), dev(p.H_upper), dev(p.S_diag), dev(p.S_upper))
+    sl, sr, inj = dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first)
+    X1 = ss.solve(p.E, sl, sr, inj).cpu().numpy(); T1 = ss.transmission()
+    with pytest.raises(lib.SplitSolveError):
+        ss.set_option("offload_columns", 0)                   # the workspace layout is fixed after the first solve
+    check_against_oracle(p, dict(X=X1, T=T1))
+    E2 = p.E[::-1].copy()
+    X2 = ss.solve(E2, sl, sr, inj).cpu().numpy(); T2 = ss.transmission()
+    for e in range(p.n_energy):
+        a = (E2[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], None)
+        r = dense.solve_energy(*a)
+        assert residual.rel_frobenius(X2[e], r["X"]) <= TOL_X and residual.rel_T(T2[e], r["T_LR"]) <= TOL_T
+    ss.close()
+    hs = [dev(a) for a in (p.H_diag, p.H_upper, p.S_diag, p.S_upper)]
+    ranks = []
+    for col in range(2):
+        s2 = lib.SplitSolve(p.nb, p.bs, p.n_energy)
+        s2.set_option("offload_columns", 6)
+        s2.set_hamiltonian(*hs)
+        s2.sweep_column(p.E, col)
+        ranks.append((s2, s2.corner_blocks(col)))
+    parts = [ranks[c][0].post_column(c, ranks[1 - c][1], sl, sr, inj) for c in range(2)]
+    T = ranks[0][0].transmission()
+    check_against_oracle(p, dict(X=(parts[0] + parts[1]).cpu().numpy(), T=T))
+    for s2, _ in ranks:
+        s2.close()
