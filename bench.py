@@ -74,6 +74,8 @@ def parse():
     ap.add_argument("--split", default="energy", choices=["energy", "column"], help="N > 1: 'energy' = every rank its own "
                     "energies (default, SURVEY 8(e)); 'column' = pairs of ranks share their energies, first block column of "
                     "A^-1 on the even rank, last on the odd one (SURVEY 8(f2), PAPER.md L167)")
+    ap.add_argument("--real-energies", action="store_true", help="variant of the workload with Im E = 0 and the energy grid moved "
+                    "above the spectrum ([3.5, 4.5]: A definite), for the Hermitian modes of SURVEY 8(f1) (--option hermitian=1|2)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the second block (C3) of the default C4 line")
@@ -549,6 +551,9 @@ def kernel_density(args):
 def main():
     args = parse()
     cfg = inputs.CONFIGS[args.workload]
+    if args.real_energies:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, name=cfg.name + " (real energies 3.5..4.5)", e_lo=3.5, e_hi=4.5, eta=0.0)
     if args.calibrate_oracle:
         calibrate_oracle()
         return

@@ -60,7 +60,7 @@ struct ss_handle_s {
     int ws_nrhs = -1;
     cplx *slots = nullptr, *aug = nullptr, *aop = nullptr, *tinv = nullptr, *raug = nullptr, *wz = nullptr;
     cplx *gam_l = nullptr, *gam_r = nullptr, *g1n = nullptr, *w1 = nullptr, *w2 = nullptr, *E_dev = nullptr;
-    double *tpart = nullptr, *T_dev = nullptr;
+    double *tpart = nullptr, *T_dev = nullptr, *J_dev = nullptr;
     int *ipiv = nullptr, *info = nullptr, *perm = nullptr;
     cplx* E_pinned = nullptr;
     // host-path buffers
@@ -207,6 +207,7 @@ extern "C" ss_status_t ss_destroy(ss_handle_t h) {
     for (cudaEvent_t e : h->prof.ev) cudaEventDestroy(e);
     for (auto& r : h->trace) { cudaEventDestroy(r.t0); cudaEventDestroy(r.t1); }
     if (h->E_pinned) cudaFreeHost(h->E_pinned);
+    free_dev(h->J_dev);
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
     for (auto& g : h->groups) {
         if (g.hi) cudaStreamDestroy(g.hi);
@@ -308,7 +309,6 @@ extern "C" ss_status_t ss_set_option(ss_handle_t h, const char* name, int value)
         if (value < 1) return SS_ERR_INVALID_ARG;
         h->growth_limit = value; return SS_OK;
     }
-    if (!strcmp(name, "panel_fused")) { g_panel_fused = value ? 1 : 0; return SS_OK; }      // process-wide (tuning)
     if (!strcmp(name, "gemm_raster")) {                                                       // process-wide (tuning)
         if (value < 1 || value > 64) return SS_ERR_INVALID_ARG;
         g_gemm_raster = value; return SS_OK;
@@ -1166,8 +1166,10 @@ extern "C" ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X, int nrhs
     if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     const int nb = h->nb, bs = h->bs, nE = h->n_energy, m = nrhs;
     const long long B2 = (long long)bs * bs, sX = (long long)nb * bs * m, sW = (long long)bs * m;
-    double* J_dev = nullptr;
-    if (cudaMalloc((void**)&J_dev, sizeof(double) * (size_t)nE * (nb - 1)) != cudaSuccess) { cudaGetLastError(); return SS_ERR_ALLOC; }
+    if (!h->J_dev && cudaMalloc((void**)&h->J_dev, sizeof(double) * (size_t)nE * (nb - 1)) != cudaSuccess) {
+        cudaGetLastError(); return SS_ERR_ALLOC;                  // handle-owned, allocated on first use
+    }
+    double* J_dev = h->J_dev;
     Ctx ctx; ctx.st = h->main_stream ? h->main_stream : h->last_stream; ctx.variant = h->gemm_variant;
     const BPtr aop = bp_chain(h->aop, h->aop + B2, 2 * B2);
     const int parts = (int)min((long long)TRACE_PARTS, cdiv(sW, 256));
@@ -1184,8 +1186,7 @@ extern "C" ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X, int nrhs
         ctx.note(cudaGetLastError());
     }
     cudaError_t e = cudaMemcpyAsync(J_host, J_dev, sizeof(double) * (size_t)nE * (nb - 1), cudaMemcpyDeviceToHost, ctx.st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx.st);
-    cudaFree(J_dev);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx.st);    // J_host is a host result: the call returns it complete
     if (e != cudaSuccess || ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     return SS_OK;
 }

@@ -159,9 +159,9 @@ lu_leaf_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restri
     }
 }
 
-// ---- helpers of the second leaf panel kernel (lu_leaf3_kernel below): 256 rows per CTA, cluster of up to 16 CTAs = 4096
-// rows.  Warp arg-max by three redux.sync on the bit pattern of |re|+|im| (non-negative doubles order like unsigned
-// integers) and the row position.
+// ---- helpers of the fused panel kernel (lu_panel_kernel below): 256 rows per CTA, cluster of up to 16 CTAs = 4096 rows.
+// Warp arg-max by three redux.sync on the bit pattern of |re|+|im| (non-negative doubles order like unsigned integers)
+// and the row position.
 constexpr int LEAF2_TPB = 256;
 constexpr int LEAF2_MAXC = 16;
 
@@ -192,113 +192,6 @@ __device__ __forceinline__ bool warp_argmax(double v, int pos, double& wv, int& 
     wv = mk ? __longlong_as_double((long long)(mk - 1ull)) : -1.0;
     wp = (int)mp;
     return cand && (unsigned)pos == mp && mk != 0ull;
-}
-
-// ---- leaf panel for up to 4096 rows: one thread = one row, 16 columns in registers, sized to run in the shadow of the
-// GEMM kernel of other stream groups (256 threads x 80 registers = one GEMM CTA slot).  Per column: the warp winner
-// deposits (value, position, row) in shared memory; warp 0 picks the CTA winner and pushes only its 16-byte key (value,
-// position, warp slot) to every CTA of the cluster (distributed shared memory); one cluster barrier; each warp finds the
-// global winner with one redux pass over the keys and warp 0 PULLS the winner's row (16 x 16 B) out of the winning
-// CTA's shared memory; rank-1 update in registers.  Measured 2.7 (4 CTAs) - 4.3 (16 CTAs) us per column against 4.9 - 9.0
-// for lu_leaf_kernel, which remains for panels of more than 4096 rows (the 2bs corner system at bs = 4096).
-struct LeafKey { double val; int pos; int warp; };
-
-__global__ void __launch_bounds__(LEAF2_TPB, 3)
-lu_leaf3_kernel(BPtr Ab, int ld, int row0, int col0, int m, int jb, int* __restrict__ ipiv, int ipiv_stride,
-                int* __restrict__ info, int info_base) {
-    cg::cluster_group cluster = cg::this_cluster();
-    const int csize = (int)cluster.num_blocks();
-    const int crank = (int)cluster.block_rank();
-    const int z = blockIdx.y;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NW = LEAF2_TPB / 32;
-
-    __shared__ __align__(16) LeafCand wcand[2][NW];
-    __shared__ __align__(16) LeafKey keys[2][LEAF2_MAXC];
-    __shared__ __align__(16) cplx prow[LEAF_JB];
-
-    cplx* __restrict__ A = bptr(Ab, z) + (long long)row0 * ld + col0;
-    const int r = crank * LEAF2_TPB + tid;       // my row inside the panel
-    const bool valid = r < m;
-
-    cplx a[LEAF_JB];
-#pragma unroll
-    for (int k = 0; k < LEAF_JB; k++) a[k] = make_c(0.0, 0.0);
-    if (valid) {
-        const cplx* src = A + (long long)r * ld;
-#pragma unroll
-        for (int k = 0; k < LEAF_JB; k++)
-            if (k < jb) a[k] = src[k];
-    }
-    int cur_pos = r;
-    bool done = !valid;
-    int final_pos = r;
-
-#pragma unroll
-    for (int j = 0; j < LEAF_JB; j++) {
-        if (j < jb) {
-            const int par = j & 1;
-            double wv; int wp;
-            const double myv = done ? -1.0 : (fabs(a[j].re) + fabs(a[j].im));
-            if (warp_argmax(myv, cur_pos, wv, wp)) {
-                LeafCand* c = &wcand[par][warp];
-                c->val = myv; c->pos = cur_pos;
-#pragma unroll
-                for (int k = 0; k < LEAF_JB; k++) c->row[k] = a[k];
-            }
-            if (lane == 0 && wv < 0.0) { wcand[par][warp].val = -1.0; wcand[par][warp].pos = 0x7fffffff; }
-            __syncthreads();
-            if (warp == 0) {
-                double v2 = lane < NW ? wcand[par][lane].val : -1.0;
-                int p2 = lane < NW ? wcand[par][lane].pos : 0x7fffffff;
-                double cv; int cp;
-                bool win = warp_argmax(v2, p2, cv, cp);
-                unsigned bal = __ballot_sync(0xffffffffu, win);
-                LeafKey k; k.val = cv; k.pos = cp; k.warp = bal ? (__ffs(bal) - 1) : 0;
-                if (lane < csize) *cluster.map_shared_rank(&keys[par][crank], lane) = k;
-            }
-            cluster.sync();
-            // ---- winner among the csize keys (every warp, one redux pass)
-            double kv = -1.0; int kp = 0x7fffffff, kw = 0;
-            if (lane < csize) { LeafKey k = keys[par][lane]; kv = k.val; kp = k.pos; kw = k.warp; }
-            double gv; int gp;
-            bool gwin = warp_argmax(kv, kp, gv, gp);
-            unsigned gbal = __ballot_sync(0xffffffffu, gwin);
-            const int wcta = gbal ? (__ffs(gbal) - 1) : 0;
-            const int wslot = __shfl_sync(0xffffffffu, kw, wcta);
-            if (warp == 0 && lane < LEAF_JB && gv >= 0.0)
-                prow[lane] = cluster.map_shared_rank(&wcand[par][wslot], wcta)->row[lane];
-            if (gv < 0.0) { gp = j; }                     // no rows left (m < jb): nothing to do
-            const bool singular = !(gv > 0.0);
-            if (crank == 0 && tid == 0) {
-                ipiv[(long long)z * ipiv_stride + row0 + j] = row0 + gp;
-                if (singular && gv >= 0.0) atomicCAS(&info[z], 0, info_base + row0 + j + 1);
-            }
-            __syncthreads();
-            if (!done) {
-                if (cur_pos == gp && gv >= 0.0) {
-                    done = true; final_pos = j;           // I am the pivot row: becomes row j of U
-                } else {
-                    if (cur_pos == j) cur_pos = gp;       // LAPACK swap bookkeeping
-                    if (!singular) {
-                        cplx rinv = crecip_fast(prow[j]);
-                        cplx l = cmul(a[j], rinv);
-                        a[j] = l;
-#pragma unroll
-                        for (int k = j + 1; k < LEAF_JB; k++) a[k] = cfnma(a[k], l, prow[k]);
-                    }
-                }
-            }
-        }
-    }
-    cluster.sync();                                   // no CTA may exit while another still reads its shared memory
-    if (valid) {
-        if (!done) final_pos = cur_pos;
-        cplx* dst = A + (long long)final_pos * ld;
-#pragma unroll
-        for (int k = 0; k < LEAF_JB; k++)
-            if (k < jb) dst[k] = a[k];
-    }
 }
 
 // ---- cluster-scope mbarrier / distributed-shared-memory primitives of the fused panel kernel
@@ -353,6 +246,52 @@ __device__ __forceinline__ void st_async_16(unsigned remote_addr, unsigned long 
 // At the end the rows that moved (at most 2 x 128) are carried to their final positions, 16 columns at a time through
 // registers with a cluster barrier between the reads and the writes of a chunk.
 constexpr int PANEL_W = 128;
+// Rank-jb update of up to 32 rows (bit mask act) of one warp: x[row][col] -= sum_k L[k][row] * U[k][col], 4 rows at a time,
+// lane l owns columns l + 32 t, t < NT.  L: per-warp tile [16][32], U: [16][112] (shared memory).
+template <int NT>
+__device__ __forceinline__ void panel_rank_update(cplx* Awarp, int ld, const cplx* Lw, const cplx* U, unsigned act, int jb,
+                                                  int wrest, int lane) {
+    constexpr int UW = 128 - LEAF_JB;
+    while (act) {
+        int rho[4]; bool on[4];
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+            on[i] = act != 0u;
+            rho[i] = on[i] ? (__ffs(act) - 1) : 0;
+            if (on[i]) act &= act - 1u;
+        }
+        cplx x[4][NT];
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+#pragma unroll
+            for (int t = 0; t < NT; t++) {
+                const int col = lane + 32 * t;
+                x[i][t] = (on[i] && col < wrest) ? Awarp[(long long)rho[i] * ld + col] : make_c(0.0, 0.0);
+            }
+#pragma unroll 4
+        for (int k = 0; k < LEAF_JB; k++) {
+            if (k < jb) {
+                cplx l[4], u[NT];
+#pragma unroll
+                for (int i = 0; i < 4; i++) l[i] = Lw[k * 32 + rho[i]];
+#pragma unroll
+                for (int t = 0; t < NT; t++) u[t] = U[k * UW + min(lane + 32 * t, UW - 1)];
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+#pragma unroll
+                    for (int t = 0; t < NT; t++) x[i][t] = cfnma(x[i][t], l[i], u[t]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+#pragma unroll
+            for (int t = 0; t < NT; t++) {
+                const int col = lane + 32 * t;
+                if (on[i] && col < wrest) Awarp[(long long)rho[i] * ld + col] = x[i][t];
+            }
+    }
+}
+
 constexpr int PANEL_DYN_SMEM = (LEAF2_TPB / 32) * LEAF_JB * 32 * (int)sizeof(cplx);   // Lsm: 64 KB
 
 #ifdef SS_PANEL_TIMING
@@ -557,52 +496,20 @@ lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv,
             // ---- A22 -= L21 U12 on the rows of this warp.  A thread walking along its own row touches 32 different cache
             // lines per warp instruction (measured: half of the whole panel time went here), so the warp works row-wise
             // instead: the multipliers go through a per-warp shared-memory tile Lsm[k][lane], then 4 rows at a time, lane
-            // l owns columns l, l+32, l+64, l+96 of each (512-byte coalesced accesses), 4 + 4 shared loads per 16 complex
-            // multiply-adds.
+            // l owns columns l, l+32, .. of each (512-byte coalesced accesses), 4 + NT shared loads per 4 NT complex
+            // multiply-adds; NT = ceil(wrest / 32) column slots, so that narrow remainders do no masked work.
             {
                 cplx* Lw = Lsm + (size_t)warp * (JB * 32);
 #pragma unroll
                 for (int k = 0; k < JB; k++) Lw[k * 32 + lane] = a[k];
-                unsigned act = __ballot_sync(0xffffffffu, valid && !done);
+                const unsigned act = __ballot_sync(0xffffffffu, valid && !done);
                 __syncwarp();
                 cplx* Awarp = A + (long long)(crank * LEAF2_TPB + warp * 32) * ld + cr;
-                while (act) {
-                    int rho[4]; bool on[4];
-#pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        on[i] = act != 0u;
-                        rho[i] = on[i] ? (__ffs(act) - 1) : 0;
-                        if (on[i]) act &= act - 1u;
-                    }
-                    cplx x[4][4];
-#pragma unroll
-                    for (int i = 0; i < 4; i++)
-#pragma unroll
-                        for (int t = 0; t < 4; t++) {
-                            const int col = lane + 32 * t;
-                            x[i][t] = (on[i] && col < wrest) ? Awarp[(long long)rho[i] * ld + col] : make_c(0.0, 0.0);
-                        }
-#pragma unroll 4
-                    for (int k = 0; k < JB; k++) {
-                        if (k < jb) {
-                            cplx l[4], u[4];
-#pragma unroll
-                            for (int i = 0; i < 4; i++) l[i] = Lw[k * 32 + rho[i]];
-#pragma unroll
-                            for (int t = 0; t < 4; t++) u[t] = U12[k][min(lane + 32 * t, PANEL_W - JB - 1)];
-#pragma unroll
-                            for (int i = 0; i < 4; i++)
-#pragma unroll
-                                for (int t = 0; t < 4; t++) x[i][t] = cfnma(x[i][t], l[i], u[t]);
-                        }
-                    }
-#pragma unroll
-                    for (int i = 0; i < 4; i++)
-#pragma unroll
-                        for (int t = 0; t < 4; t++) {
-                            const int col = lane + 32 * t;
-                            if (on[i] && col < wrest) Awarp[(long long)rho[i] * ld + col] = x[i][t];
-                        }
+                switch ((wrest + 31) >> 5) {
+                    case 1: panel_rank_update<1>(Awarp, ld, Lw, &U12[0][0], act, jb, wrest, lane); break;
+                    case 2: panel_rank_update<2>(Awarp, ld, Lw, &U12[0][0], act, jb, wrest, lane); break;
+                    case 3: panel_rank_update<3>(Awarp, ld, Lw, &U12[0][0], act, jb, wrest, lane); break;
+                    default: panel_rank_update<4>(Awarp, ld, Lw, &U12[0][0], act, jb, wrest, lane); break;
                 }
                 __syncwarp();
             }
@@ -985,24 +892,19 @@ static inline GemmArgs gemm_std(int M, int N, int K, double alpha, BPtr A, int l
     return g;
 }
 
-static int g_leaf_version = 3;       // 1 = always lu_leaf_kernel (512 rows / CTA), 3 = lu_leaf3_kernel (256 rows / CTA) up to 4096 rows
-
+// The 16-column leaf kernel (512 rows per CTA, cluster of up to 16 CTAs): panels of more than 4096 rows only
 static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, int jb, const LuWork& w, int info_base,
                         int batch) {
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(lu_leaf_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        cudaFuncSetAttribute(lu_leaf3_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         configured = true;
     }
-    const bool v3 = (g_leaf_version == 3) && m <= LEAF2_TPB * LEAF2_MAXC;
-    const int tpb = v3 ? LEAF2_TPB : LEAF_TPB;
-    int need = (m + tpb - 1) / tpb;
-    int csize = 1;
+    int need = (m + LEAF_TPB - 1) / LEAF_TPB, csize = 1;
     while (csize < need) csize <<= 1;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)csize, (unsigned)batch, 1);
-    cfg.blockDim = dim3((unsigned)tpb, 1, 1);
+    cfg.blockDim = dim3((unsigned)LEAF_TPB, 1, 1);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = ctx.st;
     cudaLaunchAttribute attr[1];
@@ -1012,10 +914,7 @@ static void launch_leaf(Ctx& ctx, BPtr Ab, int ld, int row0, int col0, int m, in
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (v3)
-        ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf3_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
-    else
-        ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
+    ctx.note(cudaLaunchKernelEx(&cfg, lu_leaf_kernel, Ab, ld, row0, col0, m, jb, w.ipiv, w.ipiv_stride, w.info, info_base));
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -1085,8 +984,6 @@ static void lu_swaps(const LuCall& L, int piv_lo, int piv_hi, int c_lo, int c_hi
     }
 }
 
-static int g_panel_fused = 1;        // 1: lu_panel_kernel for panels of up to 4096 rows; 0: always the per-16-column launches
-
 static void launch_panel_fused(Ctx& ctx, BPtr Ab, int ld, int j0, int m, int nbw, const LuWork& w, int info_base, int batch,
                                int nopiv = 0) {
     static bool configured = false;
@@ -1119,7 +1016,7 @@ static void launch_panel_fused(Ctx& ctx, BPtr Ab, int ld, int j0, int m, int nbw
 static void lu_panel(const LuCall& L, int j0, int nbw) {
     Ctx& ctx = L.ctx;
     ctx.use(CLS_HI);
-    if (g_panel_fused && L.n - j0 <= LEAF2_TPB * LEAF2_MAXC) {
+    if (L.n - j0 <= LEAF2_TPB * LEAF2_MAXC) {
         launch_panel_fused(ctx, L.Ab, L.ld, j0, L.n - j0, nbw, L.w, L.info_base, L.batch);
     } else {
         for (int c = j0; c < j0 + nbw; c += LEAF_JB) {
