@@ -150,7 +150,7 @@ def config_dict(cfg, world):
             "small workload: inputs fit L2 (launch-bound config)"}
 
 
-def oracle_sample(cfg):
+def oracle_sample(cfg, repeats=1):
     """Times the oracle, as it stands, on a bounded sample of the workload: ONE energy point of the same generator
     with the device truncated to nb_s blocks (nb_s = 2 for bs >= 1024, else min(nb, 4)), solved by the plain definition
     (LU of the full matrix: oracle/dense.py when the truncated matrix is <= 8192 rows -- with 2 blocks the band of the
@@ -158,21 +158,28 @@ def oracle_sample(cfg):
     form that fits the host) costs 64 nb bs^3 flops for the factorisation, linear in nb, so the per-energy time is
     EXTRAPOLATED by nb / nb_s and flagged as such; `--calibrate-oracle` measures that ratio on C2, and the full-size
     Tier B times of one energy point of C3 / C4 are in the headers of tests/golden/c{3,4}_fingerprint.txt.
+    `repeats` = how many times the caller will time the sample (--impl reference: warm-up + steps): when repeats x the
+    estimated cost of a sample (LU flops at 100 GFLOP/s) exceeds 200 s, the blocks of the sample are halved too (bs_s = bs/2
+    or bs/4; cost ~ bs^3, the extrapolation factor says so), so that the whole run stays within a few minutes.
     Returns (sample seconds, scale, description)."""
     from oracle import banded, dense
     nb_s = 2 if cfg.bs >= 1024 else min(cfg.nb, 4)
+    bs_s = cfg.bs
+    while bs_s > 256 and repeats * (8.0 / 3.0) * (nb_s * bs_s) ** 3 / 1e11 > 200.0:
+        bs_s //= 2
     if cfg.kind == "chain":
-        p = inputs.perfect_chain_problem(cfg.bs, nb_s, 1)
+        p = inputs.perfect_chain_problem(bs_s, nb_s, 1)
     else:
-        p = inputs.random_problem(cfg.bs, nb_s, 1, cfg.nrhs, seed=cfg.seed, threads=os.cpu_count() or 1)
-    solver = dense if cfg.bs * nb_s <= 8192 else banded
+        p = inputs.random_problem(bs_s, nb_s, 1, cfg.nrhs, seed=cfg.seed, threads=os.cpu_count() or 1)
+    solver = dense if bs_s * nb_s <= 8192 else banded
     t0 = time.perf_counter()
     solver.solve_energy(p.E[0], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[0], p.Sigma_R[0], p.Inj_first[0], None)
     dt = time.perf_counter() - t0
-    scale = cfg.nb / nb_s
-    desc = (f"1 energy point, device truncated to nb={nb_s} of {cfg.nb} blocks (bs={cfg.bs}, nrhs={cfg.nrhs}), "
+    scale = (cfg.nb / nb_s) * (cfg.bs / bs_s) ** 3
+    desc = (f"1 energy point, device truncated to nb={nb_s} of {cfg.nb} blocks" +
+            (f" of bs={bs_s} instead of {cfg.bs}" if bs_s != cfg.bs else f" (bs={cfg.bs})") + f", nrhs={cfg.nrhs}, "
             f"oracle/{'dense' if solver is dense else 'banded'}.py LU of the full matrix; solves/s EXTRAPOLATED to the full device "
-            f"by x{scale:g} (cost linear in nb; see profiles/r02_oracle_scaling.md)")
+            f"by x{scale:g} (cost linear in nb" + (", cubic in bs" if bs_s != cfg.bs else "") + "; see profiles/r02_oracle_scaling.md)")
     return dt, scale, desc
 
 
@@ -190,7 +197,7 @@ def run_reference(args, cfg):
         return
     times, desc, scale = [], "", 1.0
     for i in range(args.warmup + args.steps):
-        dt, scale, desc = oracle_sample(cfg)
+        dt, scale, desc = oracle_sample(cfg, repeats=args.warmup + args.steps)
         if i >= args.warmup:
             times.append(dt)
     mean = sum(times) / max(1, len(times))
