@@ -1,0 +1,49 @@
+"""CPU checks of bench.py's contract: the reference arm (the oracle timed on the host cores) prints one JSON line with the
+keys the driver reads, flags its extrapolation, reports the time it actually ran, and spells `config` exactly like the
+CUDA arm does (both go through bench.config_dict)."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_reference_arm_line():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "C0", "--steps", "2",
+                          "--warmup", "1"], capture_output=True, text=True, cwd=ROOT, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    line = json.loads(lines[0])
+    for k in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert k in line, k
+    assert line["impl"] == "reference" and line["metric"] == "energy_point_solves_per_s" and line["higher_is_better"] is True
+    cb = line["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and "sample" in cb
+    assert cb["extrapolated"] is True and cb["scale"] == 2.0            # C0: nb = 8 truncated to 4 blocks
+    # the line's time is the time that elapsed, the value is that time extrapolated by `scale`
+    assert abs(line["value"] * (line["ms_per_step"] * 1e-3) * cb["scale"] - 1.0) < 1e-9
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
+
+
+def test_both_arms_spell_config_the_same():
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1812_01396_b200 import inputs
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count('"config": config_dict(cfg,') >= 2                  # reference arm and CUDA arm
+    d = bench.config_dict(inputs.CONFIGS["C4"], 1)
+    assert d["workload"] == "C4" and d["bs"] == 4096 and d["nb"] == 24 and d["n_energy_per_gpu"] == 4 and d["nrhs"] == 512
+    assert "L2" in d["l2"]
+
+
+def test_reference_sample_shrinks_with_the_number_of_repeats():
+    sys.path.insert(0, ROOT)
+    import bench
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert "repeats=args.warmup + args.steps" in src
+    # cost model of oracle_sample: LU of the truncated matrix at 100 GFLOP/s; 23 repeats of C4's 8192^2 sample exceed 200 s
+    assert 23 * (8.0 / 3.0) * (2 * 4096) ** 3 / 1e11 > 200.0 > 6 * (8.0 / 3.0) * (2 * 4096) ** 3 / 1e11
+    assert bench.parse.__module__ == "bench"
