@@ -84,6 +84,7 @@ def parse():
     ap.add_argument("--dims", type=int, nargs="*", default=[], help="--kernel gemm: M N K batch [reps]; --kernel density: "
                     "n_energy n nrhs [reps]")
     ap.add_argument("--beta", type=float, default=0.0, help="--kernel gemm: C = A B + beta C (1 = the in-place update form)")
+    ap.add_argument("--sumplane", action="store_true", help="--kernel gemm: pass re + im planes of A and B (ss_zgemm_batched_sums)")
     ap.add_argument("--raster", type=int, default=None, help="--kernel gemm: tile rows per raster group (library default 16)")
     ap.add_argument("--variants", default=None, help="--kernel gemm: comma-separated GEMM variants (default: library default)")
     ap.add_argument("--calibrate-oracle", action="store_true", help="time the oracle on the full and on the truncated C2 "
@@ -497,6 +498,14 @@ def kernel_gemm(args):
     B = torch.randn((batch, K, N), dtype=torch.complex128, device="cuda", generator=g)
     C = torch.zeros((batch, M, N), dtype=torch.complex128, device="cuda")
     ref = A[0] @ B[0]
+    if args.sumplane:
+        As, Bs = (A.real + A.imag).contiguous(), (B.real + B.imag).contiguous()
+        Cs = torch.zeros((batch, M, N), dtype=torch.float64, device="cuda")
+        plain = binding.zgemm_batched
+
+        def with_sums(A_, B_, C_, alpha, beta):
+            return binding.zgemm_batched_sums(A_, As, B_, Bs, C_, Cs, alpha, beta)
+        binding.zgemm_batched = with_sums
     for v in variants:
         binding.set_default_gemm_variant(v)
         C.zero_()

@@ -227,6 +227,15 @@ ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const ss_cplx* A
                              const ss_cplx* B_dev, int ldb, long long strideB, double beta, ss_cplx* C_dev, int ldc,
                              long long strideC, int batch, void* cuda_stream);
 
+/* The same product with SUM PLANES: the 3M arithmetic needs re + im of every operand element; A_sum_dev / B_sum_dev (doubles,
+ * same leading dimensions and batch strides as A / B, both or neither) supply them, so that the kernel stages them beside
+ * the operands instead of adding per fragment on the FP64 pipe; C_sum_dev (or NULL) receives re + im of every element of C,
+ * for use as an operand's sum plane later.  Needs K, N, lda, ldb and the strides even to take effect (else ignored). */
+ss_status_t ss_zgemm_batched_sums(int M, int N, int K, double alpha, const ss_cplx* A_dev, const double* A_sum_dev, int lda,
+                                  long long strideA, const ss_cplx* B_dev, const double* B_sum_dev, int ldb, long long strideB,
+                                  double beta, ss_cplx* C_dev, double* C_sum_dev, int ldc, long long strideC, int batch,
+                                  void* cuda_stream);
+
 /* Batched blocked LU with partial pivoting (ZGETRF) of the leading n x n part of the n x ncols (ncols >= n, ld)
  * row-major matrices AB[z]; the row interchanges and the L-solve are applied to the trailing ncols - n columns too (so
  * that AB[:, n:] becomes L^-1 P B).  Recursive over column ranges down to 128-column panels (leaf panels of 16 columns

@@ -43,6 +43,8 @@ SIGNATURES = {
     "ss_strerror": (c_char_p, [c_int]),
     "ss_zgemm_batched": (c_int, [c_int, c_int, c_int, c_double, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong,
                                  c_double, c_void_p, c_int, c_longlong, c_int, c_void_p]),
+    "ss_zgemm_batched_sums": (c_int, [c_int, c_int, c_int, c_double, c_void_p, c_void_p, c_int, c_longlong, c_void_p, c_void_p, c_int,
+                                      c_longlong, c_double, c_void_p, c_void_p, c_int, c_longlong, c_int, c_void_p]),
     "ss_lu_workspace_bytes": (c_size_t, [c_int, c_int]),
     "ss_zgetrf_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_void_p, c_int, c_void_p, c_size_t,
                                   c_void_p]),
@@ -269,6 +271,17 @@ def zgemm_batched(A, B, C, alpha=1.0, beta=0.0):
     N = B.shape[2]
     _check(load().ss_zgemm_batched(M, N, K, alpha, _dev(A, "A"), K, M * K, _dev(B, "B"), N, K * N, beta,
                                    _dev(C, "C"), N, M * N, batch, _stream()), "ss_zgemm_batched")
+    return C
+
+
+def zgemm_batched_sums(A, As, B, Bs, C, Cs=None, alpha=1.0, beta=0.0):
+    """zgemm_batched with sum planes As = A.real + A.imag, Bs likewise (float64 CUDA tensors, same shapes); Cs (optional,
+    float64 [batch, M, N]) receives C.real + C.imag."""
+    batch, M, K = A.shape
+    N = B.shape[2]
+    _check(load().ss_zgemm_batched_sums(M, N, K, alpha, _dev(A, "A"), As.data_ptr(), K, M * K, _dev(B, "B"), Bs.data_ptr(), N, K * N,
+                                        beta, _dev(C, "C"), None if Cs is None else Cs.data_ptr(), N, M * N, batch, _stream()),
+           "ss_zgemm_batched_sums")
     return C
 
 

@@ -1117,6 +1117,22 @@ extern "C" size_t ss_lu_workspace_bytes(int n, int batch) {
     return (lu_tinv_elems(n, batch) + (size_t)lu_tmp_elems_default(n) * batch) * sizeof(cplx) + lu_perm_ints(n, batch) * sizeof(int);
 }
 
+// Same product with sum planes (zgemm.cuh, GemmArgs::sh*): A_sum / B_sum hold re + im of every element of A / B (same leading
+// dimensions and batch strides, doubles), C_sum receives re + im of every element of C; any of the three may be NULL.
+extern "C" ss_status_t ss_zgemm_batched_sums(int M, int N, int K, double alpha, const ss_cplx* A, const double* A_sum, int lda,
+                                             long long sA, const ss_cplx* B, const double* B_sum, int ldb, long long sB,
+                                             double beta, ss_cplx* C, double* C_sum, int ldc, long long sC, int batch, void* stream) {
+    if (M < 0 || N < 0 || K < 0 || batch < 0 || !C || (K > 0 && (!A || !B))) return SS_ERR_INVALID_ARG;
+    if (lda < K || ldb < N || ldc < N) return SS_ERR_INVALID_ARG;
+    GemmArgs g = gemm_std(M, N, K, alpha, bp_strided((const cplx*)(A ? A : C), sA), lda, bp_strided((const cplx*)(B ? B : C), sB), ldb,
+                          beta, bp_strided((cplx*)C, sC), ldc);
+    if (A_sum && B_sum) { g.shA_c = (const cplx*)A; g.shA_d = A_sum; g.shB_c = (const cplx*)B; g.shB_d = B_sum; }
+    if (C_sum) { g.shC_c = (const cplx*)C; g.shC_d = C_sum; }
+    cudaError_t e = gemm_launch(g, batch, GEMM_BIG, EPI_STD, (cudaStream_t)stream, g_default_variant);
+    if (e != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
 static ss_status_t lu_common(int n, int nrhs_solve, int ncols, ss_cplx* AB, int ld, long long stride, ss_cplx* X, int ldx,
                              long long sX, int* ipiv, int* info, int batch, void* work, size_t work_bytes, void* stream) {
     if (n < 1 || n > LEAF_TPB * LEAF_MAXC || ncols < n || ld < ncols || batch < 1 || !AB || !ipiv || !info || !work)

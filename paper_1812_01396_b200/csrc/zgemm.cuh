@@ -35,6 +35,14 @@ struct GemmArgs {
     // (i, j) of C is at global position (tri_row0 + i, tri_col0 + j); a tile whose every column lies right of its last row is skipped
     int tri, tri_row0, tri_col0;
     int raster_gm;             // tile rows per raster group (set by the launcher)
+    // Sum planes (3M only).  The three real products of 3M need re + im of every operand element; formed per fragment in the
+    // main loop these DADDs share the FP64 pipe with the DMMAs and cost 9 % of it (profiles/r02_gemm_sumplane.md).  An
+    // operand that lies inside a region with a "shadow" array of doubles holding re + im of every element (same element
+    // offsets: shadow address = sh*_d + (element pointer - sh*_c)) is staged together with its sum tile instead.  shC:
+    // the epilogue also writes re + im of every output element (the producer side of the same scheme).
+    const cplx* shA_c; const double* shA_d;
+    const cplx* shB_c; const double* shB_d;
+    const cplx* shC_c; double* shC_d;
 };
 
 static int g_gemm_raster = 16; // process-wide (tuning): 16 tile rows read 20 % less DRAM than 8 at equal speed, 32 thrash L2 (profiles/r02_gemm_tma.md)

@@ -46,8 +46,12 @@ __device__ __forceinline__ void tma_load_3d(unsigned smem_dst, const CUtensorMap
                  ::"r"(smem_dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
 
-template <int BM_, int BN_, int WARPS_M_, int WARPS_N_, int KC_, int STAGES_, int MINB_, int PF_ = 0, int TMA_ = 0>
+template <int BM_, int BN_, int WARPS_M_, int WARPS_N_, int KC_, int STAGES_, int MINB_, int PF_ = 0, int TMA_ = 0, int SH_ = 0>
 struct Gemm3Cfg {
+    // 1: both operands come with a sum plane (GemmArgs::shA / shB): a tile of re + im is staged beside every operand tile
+    // (row strides LDAS_S, LDBS_S == 4 mod 16 doubles: conflict-free LDS.64 fragments) and the main loop issues no DADD
+    static constexpr int SH = SH_;
+    static_assert(SH_ == 0 || (PF_ == 1 && TMA_ == 0), "sum planes: software-pipelined cp.async build only");
     static constexpr int BM = BM_, BN = BN_, WARPS_M = WARPS_M_, WARPS_N = WARPS_N_, KC = KC_, STAGES = STAGES_, MINB = MINB_;
     static constexpr int PF = PF_;     // 1: fragments of the next k-step are prefetched across the stage boundary
     // 1: operand tiles staged by TMA (cp.async.bulk.tensor, SWIZZLE_128B boxes of 128-byte rows: the A tile as one box of
@@ -64,8 +68,15 @@ struct Gemm3Cfg {
     static constexpr int MI = WM / 8, NJ = WN / 8;               // m8 / n8 tiles per warp
     static constexpr int LDA_S = 2 * KC + 8;                     // doubles
     static constexpr int LDB_S = 2 * BN + 4;                     // doubles
-    static constexpr int STAGE_D = BM * LDA_S + KC * LDB_S;      // doubles per stage
+    static constexpr int LDAS_S = KC + 4, LDBS_S = BN + 4;       // doubles: sum tiles
+    static constexpr int SUM_A_OFF = BM * LDA_S + KC * LDB_S, SUM_B_OFF = SUM_A_OFF + BM * LDAS_S;
+    static constexpr int STAGE_D = BM * LDA_S + KC * LDB_S + (SH_ ? BM * LDAS_S + KC * LDBS_S : 0);      // doubles per stage
     static constexpr int SMEM_BYTES = STAGES * STAGE_D * 8;
+    static constexpr int CH_AS = BM * KC / 2, CH_BS = KC * BN / 2;   // 16-byte chunks (2 sums) of the sum tiles per stage
+    static constexpr int ITER_AS = (CH_AS + (WARPS_M_ * WARPS_N_ * 32) - 1) / (WARPS_M_ * WARPS_N_ * 32);
+    static constexpr int ITER_BS = (CH_BS + (WARPS_M_ * WARPS_N_ * 32) - 1) / (WARPS_M_ * WARPS_N_ * 32);
+    static_assert(SH_ == 0 || (LDAS_S % 16 == 4 || LDAS_S % 16 == 12) , "bank layout of the A sum tile");
+    static_assert(SH_ == 0 || (LDBS_S % 16 == 4 || LDBS_S % 16 == 12), "bank layout of the B sum tile");
     static constexpr int CH_A = BM * KC, CH_B = KC * BN;         // 16-byte chunks per stage
     static constexpr int ITER_A = (CH_A + NT - 1) / NT, ITER_B = (CH_B + NT - 1) / NT;
     static_assert(WM % 8 == 0 && WN % 8 == 0 && KC % 4 == 0, "warp tile");
@@ -107,6 +118,8 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
 
     const cplx* __restrict__ Ag = bptr(p.A, z);
     const cplx* __restrict__ Bg = bptr(p.B, z);
+    const double* __restrict__ As_g = Cfg::SH ? p.shA_d + (Ag - p.shA_c) : nullptr;      // re + im of the operands' elements
+    const double* __restrict__ Bs_g = Cfg::SH ? p.shB_d + (Bg - p.shB_c) : nullptr;
 
     // ---- per-thread staging state (chunk c of the A tile: row c / KC, k c % KC; of the B tile: k c / BN, col c % BN).
     // Stages are loaded in increasing k order, so each chunk keeps a running global pointer; shared-memory destinations
@@ -215,6 +228,26 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
             bool ok = b_ok[q] && (k0 + b_kr[q] < K);
             cp_async16(sbase + b_dst[q], ok ? (const void*)(b_src[q] + (long long)k0 * p.ldb) : (const void*)Bg, ok ? 16 : 0);
         }
+        if constexpr (Cfg::SH) {                          // the sum tiles: 16-byte chunks = two sums (K, N, lda, ldb even)
+#pragma unroll
+            for (int q = 0; q < Cfg::ITER_AS; q++) {
+                const int c = tid + q * NT;
+                if (c >= Cfg::CH_AS) continue;
+                const int row = c / (KC / 2), k2 = 2 * (c % (KC / 2));
+                const bool ok = (m0 + row) < M && (k0 + k2) < K;
+                cp_async16(sbase + Cfg::SUM_A_OFF + row * Cfg::LDAS_S + k2,
+                           ok ? (const void*)(As_g + (long long)(m0 + row) * p.lda + k0 + k2) : (const void*)Ag, ok ? 16 : 0);
+            }
+#pragma unroll
+            for (int q = 0; q < Cfg::ITER_BS; q++) {
+                const int c = tid + q * NT;
+                if (c >= Cfg::CH_BS) continue;
+                const int kr = c / (BN / 2), c2 = 2 * (c % (BN / 2));
+                const bool ok = (k0 + kr) < K && (n0 + c2) < N;
+                cp_async16(sbase + Cfg::SUM_B_OFF + kr * Cfg::LDBS_S + c2,
+                           ok ? (const void*)(Bs_g + (long long)(k0 + kr) * p.ldb + n0 + c2) : (const void*)Bg, ok ? 16 : 0);
+            }
+        }
     };
 
     const unsigned tma_bars = (unsigned)__cvta_generic_to_shared(smem + STAGES * STAGE_D);     // STAGES mbarriers behind the tiles
@@ -300,6 +333,8 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
         // stage kt's last DMMAs issue -- no warp starts a stage by waiting for its LDS.
         constexpr int KS = KC / 4;
         double fa[2][MI][2], fb[2][NJ][2];
+        double fsa[2][Cfg::SH ? MI : 1], fsb[2][Cfg::SH ? NJ : 1];
+        const int sa_off = Cfg::SUM_A_OFF + (wm0 + g) * Cfg::LDAS_S + t, sb_off = Cfg::SUM_B_OFF + t * Cfg::LDBS_S + wn0 + g;
         // TMA layout (doubles within a stage): A row r at 16 r, complex k chunk c at ((c ^ (r & 7)) << 1); B box jb at
         // 16 BM + 128 jb, k row kk at 16 kk, complex column cc at ((cc ^ (kk & 7)) << 1).  k-step ks uses the chunks 2t + ks.
         const int ta_off0 = (wm0 + g) * 16 + (((2 * t) ^ g) << 1), ta_off1 = (wm0 + g) * 16 + (((2 * t + 1) ^ g) << 1);
@@ -329,6 +364,12 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
                     double2 v = *reinterpret_cast<const double2*>(sS + b_off + 16 * j + 4 * ks * LDB_S);
                     fb[buf][j][0] = v.x; fb[buf][j][1] = v.y;
                 }
+                if constexpr (Cfg::SH) {
+#pragma unroll
+                    for (int i = 0; i < MI; i++) fsa[buf][i] = sS[sa_off + 8 * i * Cfg::LDAS_S + 4 * ks];
+#pragma unroll
+                    for (int j = 0; j < NJ; j++) fsb[buf][j] = sS[sb_off + 4 * ks * Cfg::LDBS_S + 8 * j];
+                }
             }
         };
         auto stage_landed = [&](int kt) {                 // stage kt is complete in shared memory (for this thread)
@@ -354,10 +395,25 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
                     load_frag(cur ^ 1, sS, ks + 1);
                 }
                 double as[MI], bs[NJ];
+#ifdef SS_EXP_NOSUM          // experiment only (WRONG results): the main loop without the fragment-sum DADDs, profiles/r02_gemm_sumplane.md
+                if constexpr (true) {
 #pragma unroll
-                for (int i = 0; i < MI; i++) as[i] = fa[cur][i][0] + fa[cur][i][1];
+                    for (int i = 0; i < MI; i++) as[i] = fa[cur][i][0];
 #pragma unroll
-                for (int j = 0; j < NJ; j++) bs[j] = fb[cur][j][0] + fb[cur][j][1];
+                    for (int j = 0; j < NJ; j++) bs[j] = fb[cur][j][1];
+                } else
+#endif
+                if constexpr (Cfg::SH) {                  // the sums were staged with the operands: no DADD on the DMMA pipe
+#pragma unroll
+                    for (int i = 0; i < MI; i++) as[i] = fsa[cur][i];
+#pragma unroll
+                    for (int j = 0; j < NJ; j++) bs[j] = fsb[cur][j];
+                } else {
+#pragma unroll
+                    for (int i = 0; i < MI; i++) as[i] = fa[cur][i][0] + fa[cur][i][1];
+#pragma unroll
+                    for (int j = 0; j < NJ; j++) bs[j] = fb[cur][j][0] + fb[cur][j][1];
+                }
 #pragma unroll
                 for (int i = 0; i < MI; i++)
 #pragma unroll
@@ -413,6 +469,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB) zgemm3m_kernel(const GemmA
                         o.im = fma(beta, c.im, o.im);
                     }
                     Cg[(long long)row * p.ldc + col] = o;
+                    if (p.shC_d) p.shC_d[(Cg - p.shC_c) + (long long)row * p.ldc + col] = o.re + o.im;
                 }
             }
         }
@@ -503,6 +560,7 @@ static cudaError_t gemm3m_launch_t(GemmArgs a, int batch, cudaStream_t st) {
 // ring) are recorded in that file and are no longer built.
 using C3_64x32s4 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3>;      // 4 warps of 32x16, 4-stage ring, 3 CTAs/SM
 using C3_64x32pf = Gemm3Cfg<64, 32, 2, 2, 8, 4, 2, 1>;   // 4 warps of 32x16, cross-stage fragment prefetch, 220 registers, 2 CTAs/SM
+using C3_64x32sh = Gemm3Cfg<64, 32, 2, 2, 8, 4, 2, 1, 0, 1>; // the same main loop fed with staged sum tiles (no fragment-sum DADDs)
 using C3_64x32tma = Gemm3Cfg<64, 32, 2, 2, 8, 4, 2, 1, 1>;  // the same main loop, operand tiles staged by TMA (experiment)
 using C3_64x32tma3 = Gemm3Cfg<64, 32, 2, 2, 8, 4, 3, 1, 1>; // same at 3 CTAs/SM (the TMA build needs 168 registers)
 using C3_Tall = Gemm3Cfg<128, 16, 4, 1, 8, 4, 2>;        // one CTA owns all (<=128) rows of its 16 columns: in-place L^-1 * A12
@@ -532,7 +590,16 @@ static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, c
         if (ok) return variant == GV_3M_TMA3 ? gemm3m_epi<C3_64x32tma3>(a, batch, epi, st) : gemm3m_epi<C3_64x32tma>(a, batch, epi, st);
         variant = GV_3M_PF;
     }
-    if (variant == GV_3M_PF) return gemm3m_epi<C3_64x32pf>(a, batch, epi, st);
+    if (variant == GV_3M_PF) {
+        // both operands inside regions with sum planes, everything even (two sums per 16-byte staging request)
+        auto even = [](const BPtr& b, const cplx* base) {
+            return ((b.p0 - base) % 2 == 0) && (!b.p1 || (b.p1 - base) % 2 == 0) && b.s_in % 2 == 0 && b.s_out % 2 == 0;
+        };
+        const bool sh = a.shA_d && a.shB_d && a.K % 2 == 0 && a.N % 2 == 0 && a.lda % 2 == 0 && a.ldb % 2 == 0 &&
+                        even(a.A, a.shA_c) && even(a.B, a.shB_c);
+        if (sh) return gemm3m_epi<C3_64x32sh>(a, batch, epi, st);
+        return gemm3m_epi<C3_64x32pf>(a, batch, epi, st);
+    }
     return gemm3m_epi<C3_64x32s4>(a, batch, epi, st);
 }
 

@@ -77,6 +77,28 @@ def test_zgemm_batched_vs_numpy(lib, M, N, K, batch, variant):
         lib.set_default_gemm_variant(default)
 
 
+@pytest.mark.parametrize("M,N,K,batch", [(128, 96, 64, 2), (200, 70, 1030, 1), (64, 32, 8, 3)])
+def test_zgemm_with_sum_planes_is_bit_identical(lib, M, N, K, batch):
+    """ss_zgemm_batched_sums: re + im of the operands staged beside them instead of added per fragment -- the same two
+    doubles are added either way, so C is bit-identical to the plain product; C_sum = re(C) + im(C)."""
+    A = inputs.complex_gaussian(1, 53, M, (batch, M, K), 1.0)
+    B = inputs.complex_gaussian(1, 54, N, (batch, K, N), 1.0)
+    default = lib.get_default_gemm_variant()
+    try:
+        lib.set_default_gemm_variant(3)                       # the software-pipelined build is the one with a sum-plane form
+        Ad, Bd = dev(A), dev(B)
+        C0 = torch.zeros((batch, M, N), dtype=torch.complex128, device="cuda")
+        C1 = torch.zeros_like(C0)
+        Cs = torch.zeros((batch, M, N), dtype=torch.float64, device="cuda")
+        lib.zgemm_batched(Ad, Bd, C0)
+        lib.zgemm_batched_sums(Ad, (Ad.real + Ad.imag).contiguous(), Bd, (Bd.real + Bd.imag).contiguous(), C1, Cs)
+        assert torch.equal(C0, C1)
+        assert torch.equal(Cs, C1.real + C1.imag)
+        assert np.abs(C1.cpu().numpy() - np.matmul(A, B)).max() <= 1e-13 * K
+    finally:
+        lib.set_default_gemm_variant(default)
+
+
 @pytest.mark.parametrize("variant", [0, 1, 2, 3])
 def test_hot_path_with_every_gemm_variant(lib, variant):
     p = inputs.random_problem(150, 3, 2, 37, seed=13, inj_last=True)
