@@ -126,3 +126,12 @@ def test_closed_form_flop_counts_match_survey_table():
     assert abs(f_total(64, 512, 128) / 1e12 - 0.505) < 1e-3
     assert abs(f_total(32, 2048, 256) / 1e12 - 16.0) < 5e-2
     assert abs(f_total(24, 4096, 512) / 1e12 - 97.4) < 5e-2
+
+
+def test_library_links_no_vendor_math_library(libpath):
+    """north_star: "no cuBLAS/cuSOLVER on the hot path" -- the shared library depends on the CUDA runtime only (statically
+    linked by nvcc), not on cuBLAS, cuSOLVER, cuFFT, NCCL or torch."""
+    import subprocess
+    out = subprocess.run(["ldd", libpath], capture_output=True, text=True).stdout.lower()
+    for name in ("cublas", "cusolver", "cufft", "nccl", "torch", "c10"):
+        assert name not in out, name
