@@ -71,9 +71,10 @@ def parse():
                     "(library default 4; 1 = single stream)")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=INT", help="extra ss_set_option calls (tuning)")
     ap.add_argument("--trace", default=None, help="write the phase timeline of the last timed step to this CSV")
-    ap.add_argument("--split", default="energy", choices=["energy", "column"], help="N > 1: 'energy' = every rank its own "
+    ap.add_argument("--split", default="energy", choices=["energy", "column", "spatial"], help="N > 1: 'energy' = every rank its own "
                     "energies (default, SURVEY 8(e)); 'column' = pairs of ranks share their energies, first block column of "
-                    "A^-1 on the even rank, last on the odd one (SURVEY 8(f2), PAPER.md L167)")
+                    "A^-1 on the even rank, last on the odd one; 'spatial' = pairs of ranks share their energies, top half of the device on the "
+                    "even rank, bottom half on the odd one, SPIKE-style merge (SURVEY 8(f2), PAPER.md L167, L169)")
     ap.add_argument("--real-energies", action="store_true", help="variant of the workload with Im E = 0 and the energy grid moved "
                     "above the spectrum ([3.5, 4.5]: A definite), for the Hermitian modes of SURVEY 8(f1) (--option hermitian=1|2)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -242,7 +243,8 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     from paper_1812_01396_b200 import binding, sharding
 
     nE, bs, nb, m = cfg.n_energy, cfg.bs, cfg.nb, cfg.nrhs
-    column_split = args.split == "column" and world > 1
+    spatial_split = args.split == "spatial" and world > 1
+    column_split = (args.split == "column" and world > 1) or spatial_split      # both: pairs of ranks share their energies
     if column_split:
         # ranks (2j, 2j+1) share the energies of shard j; every rank creates every pair's group
         if world % 2:
@@ -289,7 +291,15 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
 
     variant = binding.get_default_gemm_variant()
     is3m = variant != 0
-    ss = binding.SplitSolve(nb, bs, nE)
+    if spatial_split:
+        # this rank's half of the device: rows [lo, hi) of the block stacks (the whole H, S were generated / broadcast above;
+        # a production caller would only ever hold its slices)
+        hsplit = sharding.split_blocks(nb)
+        lo, hi = (0, hsplit) if (rank & 1) == 0 else (hsplit, nb)
+        S_c, H_c = devt["S_upper"][hsplit - 1].contiguous(), devt["H_upper"][hsplit - 1].contiguous()
+        ss = binding.SplitSolve(hi - lo, bs, nE)
+    else:
+        ss = binding.SplitSolve(nb, bs, nE)
     groups = 4 if args.stream_groups is None else args.stream_groups
     ss.set_option("stream_groups", groups)
     for kv in args.option:
@@ -297,11 +307,20 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
         ss.set_option(k, int(v))
     if args.trace:
         ss.set_option("trace", 1)
-    ss.set_hamiltonian(devt["H_diag"], devt["H_upper"], devt["S_diag"], devt["S_upper"])
+    if spatial_split:
+        ss.set_hamiltonian(devt["H_diag"][lo:hi].contiguous(), devt["H_upper"][lo:hi - 1].contiguous(),
+                           devt["S_diag"][lo:hi].contiguous(), devt["S_upper"][lo:hi - 1].contiguous())
+    else:
+        ss.set_hamiltonian(devt["H_diag"], devt["H_upper"], devt["S_diag"], devt["S_upper"])
     X = torch.empty((nE, nb * bs, m), dtype=torch.complex128, device="cuda")
 
     col_T = [None]
-    if column_split:
+    if spatial_split:
+        engine = sharding.LibraryPartitionEngine(ss, p.E, S_c, H_c, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None)
+
+        def step():
+            _, col_T[0] = sharding.spatial_split_solve(engine, rank, group=pair_group)
+    elif column_split:
         engine = sharding.LibraryColumnEngine(ss, p.E, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None)
 
         def step():
@@ -400,7 +419,7 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     kern = ("zgemm3m_kernel" if is3m else "zgemm_kernel") + f" [{binding.GEMM_VARIANTS[variant]}] (DMMA.8x8x4, mma.sync f64)"
     out = {
         "value": value, "ms_per_step": ms_step, "steps": steps, "warmup": warmup,
-        "config": config_dict(cfg, world), "launch": {"stream_groups": groups, "split": "column pairs" if column_split else "energy"},
+        "config": config_dict(cfg, world), "launch": {"stream_groups": groups, "split": ("spatial pairs" if spatial_split else "column pairs") if column_split else "energy"},
         "tflops": {"whole_solve": flops_step / (ms_step * 1e-3) / 1e12, "sweep_a1_a4": sweep_tf,
                    "sweep_executed": sweep_tf * ratio, "sweep_executed_frac_of_fp64_peak": sweep_tf * ratio / FP64_PEAK_NOMINAL_TFLOPS,
                    "flops_per_step": flops_step,

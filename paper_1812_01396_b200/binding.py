@@ -26,6 +26,10 @@ SIGNATURES = {
     "ss_sweep_column": (c_int, [c_void_p, c_void_p, c_int, c_void_p]),
     "ss_get_corner_blocks": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
     "ss_post_column": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]),
+    "ss_sweep_partition": (c_int, [c_void_p, c_void_p, c_void_p]),
+    "ss_get_edge_blocks": (c_int, [c_void_p, c_int, c_void_p, c_void_p]),
+    "ss_merge_partition": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "ss_post_partition": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p]),
     "ss_synchronize": (c_int, [c_void_p]),
     "ss_transmission": (c_int, [c_void_p, c_void_p]),
     "ss_inverse_columns": (c_int, [c_void_p, c_int, POINTER(c_void_p), POINTER(c_void_p)]),
@@ -186,6 +190,36 @@ class SplitSolve:
                                      _dev(X_part, "X_part"), _stream()), "ss_post_column")
         return X_part
 
+    # ---- SURVEY.md 8(f2): the device split into two halves, one per GPU (PAPER.md L167, L169) ----
+    def sweep_partition(self, E):
+        import numpy as np
+        E = np.ascontiguousarray(np.asarray(E, dtype=np.complex128))
+        assert E.shape == (self.n_energy,)
+        _check(load().ss_sweep_partition(self._h, E.ctypes.data, _stream()), "ss_sweep_partition")
+
+    def edge_blocks(self, edge: int):
+        """[n_energy, 2, bs, bs]: block `edge` (0 first, 1 last) of the first and of the last block column."""
+        import torch
+        out = torch.empty((self.n_energy, 2, self.bs, self.bs), dtype=torch.complex128, device="cuda")
+        _check(load().ss_get_edge_blocks(self._h, int(edge), out.data_ptr(), _stream()), "ss_get_edge_blocks")
+        return out
+
+    def merge_partition(self, part: int, peer_iface, S_couple, H_couple):
+        self._keep_merge = [peer_iface, S_couple, H_couple]
+        _check(load().ss_merge_partition(self._h, int(part), _dev(peer_iface, "peer_iface"), _dev(S_couple, "S_couple"),
+                                         _dev(H_couple, "H_couple"), _stream()), "ss_merge_partition")
+
+    def post_partition(self, peer_corner, Sigma_L, Sigma_R, Inj_first, Inj_last=None, X_rows=None):
+        import torch
+        nrhs = 0 if Inj_first is None else int(Inj_first.shape[-1])
+        if X_rows is None and nrhs > 0:
+            X_rows = torch.empty((self.n_energy, self.nb * self.bs, nrhs), dtype=torch.complex128, device=Sigma_L.device)
+        self._keep_solve = [peer_corner, Sigma_L, Sigma_R, Inj_first, Inj_last, X_rows]
+        _check(load().ss_post_partition(self._h, _dev(peer_corner, "peer_corner"), _dev(Sigma_L, "Sigma_L"), _dev(Sigma_R, "Sigma_R"),
+                                        _dev(Inj_first, "Inj_first"), _dev(Inj_last, "Inj_last"), nrhs, _dev(X_rows, "X_rows"),
+                                        _stream()), "ss_post_partition")
+        return X_rows
+
     def synchronize(self):
         _check(load().ss_synchronize(self._h), "ss_synchronize")
 
@@ -201,7 +235,7 @@ class SplitSolve:
         Q = torch.empty((self.nb, self.bs, self.bs), dtype=torch.complex128, device="cuda")
         P = torch.empty_like(Q)
         _check(load().ss_copy_inverse_columns(self._h, energy, Q.data_ptr(), P.data_ptr()), "ss_copy_inverse_columns")
-        self.synchronize()
+        torch.cuda.current_stream().synchronize()
         return Q, P
 
     def last_info(self):

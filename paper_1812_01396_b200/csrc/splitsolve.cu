@@ -32,6 +32,7 @@ struct ss_handle_s {
     struct GroupCopy { cudaStream_t st = nullptr; std::vector<cudaEvent_t> ev_slot[2]; std::vector<cudaEvent_t> ev_step; };
     std::vector<GroupCopy> gcopy;    // per stream group: its copy stream, one event per (column, ring slot), step events
     int slots_per_chain() const { return offload ? ring : nb + 1; }
+    int part = -1;                   // spatial split (ss_*_partition): -1 whole device, 0 top half, 1 bottom half; set by ss_merge_partition
     int swept_cols = 0;              // block columns the last sweep computed (3 = both; 1 / 2: ss_sweep_column)
     bool whole_solve = true;         // the last post-processing belonged to an ss_solve (so a redo is possible)
     bool force_general = false;      // set while a solve is being redone
@@ -573,6 +574,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     // corner blocks [column][first / last block] with their energy strides
     const cplx* cor[2][2] = {{slot(0, 0), slot(0, nb - 1)}, {slot(1, 1), slot(1, nb)}};
     long long cor_s[2] = {s_slot_e, s_slot_e};
+    long long cor_far_s = 0; int far_idx = -1;        // spatial split: stride of the peer's corner blocks, which end they are
     if (h->offload)                                   // saved aside when they were produced (the ring has moved on)
         for (int c = 0; c < 2; c++) {
             cor[c][0] = h->corner + ((long long)e0 * 2 + c) * 2 * B2; cor[c][1] = cor[c][0] + B2; cor_s[c] = 4 * B2;
@@ -580,6 +582,13 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     if (G.cols != 3) {
         const int other = (G.cols == 1) ? 1 : 0;
         cor[other][0] = peer + (long long)e0 * 2 * B2; cor[other][1] = cor[other][0] + B2; cor_s[other] = 2 * B2;
+    } else if (h->part >= 0) {
+        // spatial split: this handle holds the rows of one half of the device (merged, global Q_i / P_i); the corner blocks at
+        // the far end of the device, peer[e][column], come from the other half
+        const int far = h->part == 0 ? 1 : 0;
+        for (int c = 0; c < 2; c++) { cor[c][far] = peer + ((long long)e0 * 2 + c) * B2; }
+        // strides: own blocks keep the slot stride; the peer's are [n_energy][2][bs*bs]
+        cor_far_s = 2 * B2; far_idx = far;
     }
     const int zc = h->want_T ? bs : 0;                // columns of e_2 (for (R^-1)_{12}, (R^-1)_{22})
     const int W = 2 * bs + m + zc;
@@ -606,7 +615,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     const cplx* sig[2] = {SigL, SigR};
     for (int br = 0; br < 2; br++)
         for (int bc = 0; bc < 2; bc++) {
-            GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(cor[bc][br], cor_s[bc]), bs, 1.0,
+            GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(cor[bc][br], br == far_idx ? cor_far_s : cor_s[bc]), bs, 1.0,
                                   bp_strided(raug + (long long)br * bs * ldW + (long long)bc * bs, s_r), ldW);
             gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         }
@@ -659,10 +668,10 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     }
     // a7: G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22;  T = Re Tr(Gamma_L G Gamma_R G^H)
     if (h->want_T) {
-        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[0][0], cor_s[0]), bs, bp_strided(wz + m, s_w), nr, 0.0,
+        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[0][0], far_idx == 0 ? cor_far_s : cor_s[0]), bs, bp_strided(wz + m, s_w), nr, 0.0,
                               bp_strided(g1n, B2), bs);
         gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
-        GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[1][0], cor_s[1]), bs,
+        GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[1][0], far_idx == 0 ? cor_far_s : cor_s[1]), bs,
                                bp_strided(wz + (long long)bs * nr + m, s_w), nr, 1.0, bp_strided(g1n, B2), bs);
         gemm_run(ctx, g2, nE, GEMM_BIG, EPI_STD);
         dim3 gg((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)nE);
@@ -842,12 +851,14 @@ extern "C" ss_status_t ss_solve(ss_handle_t h, const ss_cplx* E_host, const ss_c
                                 void* cuda_stream) {
     if (!h || !E_host || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
     if (nrhs > 0 && (!Inj_first || !X)) return SS_ERR_INVALID_ARG;
+    h->part = -1;
     return run_phases(h, E_host, PH_SWEEP | PH_POST, 3, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X, nullptr, cuda_stream);
 }
 
 // ---- one energy batch on two GPUs, one block column of A^-1 each ----------------
 extern "C" ss_status_t ss_sweep_column(ss_handle_t h, const ss_cplx* E_host, int column, void* cuda_stream) {
     if (!h || !E_host || column < 0 || column > 1) return SS_ERR_INVALID_ARG;
+    h->part = -1;
     return run_phases(h, E_host, PH_SWEEP, 1 << column, nullptr, nullptr, nullptr, nullptr, 0, nullptr, nullptr, cuda_stream);
 }
 
@@ -867,6 +878,142 @@ extern "C" ss_status_t ss_get_corner_blocks(ss_handle_t h, int column, ss_cplx* 
         }
     }
     return SS_OK;
+}
+
+// ---- SURVEY.md 8(f2), second half: the device split into two halves along the transport axis ("horizontal
+// split", L169 SPIKE), one half per GPU.  Each GPU sweeps ITS OWN sub-device (ss_sweep_partition: first and last block
+// columns of A_T^-1 resp. A_B^-1); the halves are coupled only through U = A_{h,h+1} and L = A_{h+1,h}.  With
+//   QT, PT = first / last block column of A_T^-1 (h blocks),  QB, PB = those of A_B^-1,
+// the first block column x of the whole inverse solves  x_T = QT - PT U x_{B,1},  x_B = -QB L x_{T,h},  so the interface
+// blocks a = x_{T,h}, b = x_{B,1} obey  (1 - PT_h U QB_1 L) a = QT_h,  b = -QB_1 L a;  the last block column likewise with
+// (1 - QB_1 L PT_h U) b' = PB_1,  a' = -PT_h U b'.  Then
+//   top half:     Q_i = QT_i - PT_i (U b),      P_i = -PT_i (U b')              i = 1..h
+//   bottom half:  Q_{h+i} = -QB_i (L a),        P_{h+i} = PB_i - QB_i (L a')    i = 1..nb-h
+// Both GPUs solve the two bs x bs interface systems redundantly from own + peer interface blocks (2 blocks per energy each
+// way), then update their own rows; no other data crosses.  Afterwards each half holds the rows of the GLOBAL Q, P.
+static void edge_ptrs(ss_handle_t h, int edge, const cplx* out[2]) {      // first (0) / last (1) block of both columns, energy 0
+    out[0] = slot_ptr(h, 0, 0, edge ? h->nb - 1 : 0);
+    out[1] = slot_ptr(h, 0, 1, edge ? h->nb : 1);
+}
+
+extern "C" ss_status_t ss_sweep_partition(ss_handle_t h, const ss_cplx* E_host, void* cuda_stream) {
+    if (!h || !E_host) return SS_ERR_INVALID_ARG;
+    if (h->offload) return SS_ERR_NOT_READY;
+    h->part = -1;
+    return run_phases(h, E_host, PH_SWEEP, 3, nullptr, nullptr, nullptr, nullptr, 0, nullptr, nullptr, cuda_stream);
+}
+
+extern "C" ss_status_t ss_get_edge_blocks(ss_handle_t h, int edge, ss_cplx* out_dev, void* cuda_stream) {
+    if (!h || !out_dev || edge < 0 || edge > 1) return SS_ERR_INVALID_ARG;
+    if (!h->launched || h->swept_cols != 3 || h->offload) return SS_ERR_NOT_READY;
+    const size_t B2 = (size_t)h->bs * h->bs;
+    const cplx* src[2];
+    edge_ptrs(h, edge, src);
+    for (int c = 0; c < 2; c++)
+        if (cudaMemcpy2DAsync((cplx*)out_dev + c * B2, 2 * B2 * sizeof(cplx), src[c], sizeof(cplx) * (size_t)slot_stride_e(h),
+                              B2 * sizeof(cplx), (size_t)h->n_energy, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream) != cudaSuccess) {
+            cudaGetLastError(); return SS_ERR_CUDA;
+        }
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx* peer_iface_dev, const ss_cplx* S_couple_dev,
+                                          const ss_cplx* H_couple_dev, void* cuda_stream) {
+    if (!h || part < 0 || part > 1 || !peer_iface_dev || !S_couple_dev || !H_couple_dev) return SS_ERR_INVALID_ARG;
+    if (!h->launched || h->swept_cols != 3 || h->offload || h->part >= 0) return SS_ERR_NOT_READY;
+    const int nb = h->nb, bs = h->bs, nE = h->n_energy;
+    const long long B2 = (long long)bs * bs, sE = slot_stride_e(h);
+    cudaStream_t user = (cudaStream_t)cuda_stream, main = h->main_stream;
+    cudaEventSynchronize(h->ev[2]);
+    cudaEventRecord(h->ev_in, user);
+    cudaStreamWaitEvent(main, h->ev_in, 0);
+    Ctx ctx; ctx.st = main; ctx.variant = h->gemm_variant;
+    const cplx* peer = (const cplx*)peer_iface_dev;
+    // interface blocks (pointer of energy 0, energy stride): QT_h, PT_h of the top half, QB_1, PB_1 of the bottom half
+    const cplx* own[2];
+    edge_ptrs(h, part == 0 ? 1 : 0, own);
+    const cplx *QTh = part == 0 ? own[0] : peer, *PTh = part == 0 ? own[1] : peer + B2;
+    const cplx *QB1 = part == 1 ? own[0] : peer, *PB1 = part == 1 ? own[1] : peer + B2;
+    const long long sT = part == 0 ? sE : 2 * B2, sB = part == 1 ? sE : 2 * B2;
+    cplx *U = h->gam_l, *Lc = h->gam_r, *W1 = h->g1n, *V1 = h->w1, *W2 = h->w2;
+    auto gemm = [&](double alpha, const cplx* A, long long sA, const cplx* B, long long sB_, double beta, cplx* C, long long sC, int ldc) {
+        GemmArgs g = gemm_std(bs, bs, bs, alpha, bp_strided(A, sA), bs, bp_strided(B, sB_), bs, beta, bp_strided(C, sC), ldc);
+        gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
+    };
+    // U = E S_c - H_c, L = E S_c^H - H_c^H for every energy (eshift 0: batch entry = energy)
+    FormSide up{(const cplx*)S_couple_dev, (const cplx*)H_couple_dev, FORM_PLAIN}, lo{(const cplx*)S_couple_dev, (const cplx*)H_couple_dev, FORM_CONJT};
+    launch_form(ctx, up, up, h->E_dev, bp_strided(U, B2), bs, bs, nE, 0);
+    launch_form(ctx, lo, lo, h->E_dev, bp_strided(Lc, B2), bs, bs, nE, 0);
+    gemm(1.0, QB1, sB, Lc, B2, 0.0, W1, B2, bs);                          // W1 = QB_1 L
+    gemm(1.0, PTh, sT, U, B2, 0.0, V1, B2, bs);                           // V1 = PT_h U
+    gemm(1.0, U, B2, W1, B2, 0.0, W2, B2, bs);                            // W2 = U QB_1 L
+    // the two interface systems as chains z = 2 e + q of the sweep's work matrix: [1 - PT_h W2 | QT_h], [1 - W1 V1 | PB_1]
+    const int ldg = pad_ld(2 * bs);
+    const long long s_aug_e = 2LL * bs * ldg;
+    const BPtr aug = bp_chain(h->aug, h->aug + (long long)bs * ldg, s_aug_e);
+    {
+        dim3 grid((unsigned)min((long long)8, cdiv(2 * bs, 256)), (unsigned)bs, (unsigned)(2 * nE));
+        merge_init_kernel<<<grid, 256, 0, ctx.st>>>(aug, ldg, bs, QTh, sT, PB1, sB);
+        ctx.note(cudaGetLastError());
+    }
+    gemm(-1.0, PTh, sT, W2, B2, 1.0, h->aug, s_aug_e, ldg);
+    gemm(-1.0, W1, B2, V1, B2, 1.0, h->aug + (long long)bs * ldg, s_aug_e, ldg);
+    LuWork w2;                                                            // the sweep's scratch: all of it is free now
+    w2.tinv = h->tinv; w2.ipiv = h->ipiv; w2.ipiv_stride = 2 * bs; w2.info = h->info;   // zero pivots reported like a sweep's
+    w2.perm = h->perm; w2.tmp = h->aop; w2.tmp_elems = B2;
+    cudaMemsetAsync(h->info, 0, sizeof(int) * 2 * (size_t)nE, ctx.st);
+    lu_factor(ctx, aug, ldg, bs, 2 * bs, 2 * nE, w2, 0);
+    cplx *av = h->aop, *bpv = h->aop + B2;                                // a (chain 0) and b' (chain 1) per energy
+    back_substitute(ctx, aug, ldg, bs, bs, bp_chain(av, bpv, 2 * B2), bs, 2 * nE, w2);
+    // the two products each half needs: top U b, U b' (b = -W1 a); bottom L a, L a' (a' = -V1 b')
+    cplx *F1 = V1, *F2 = (part == 0) ? Lc : U;
+    if (part == 0) {
+        gemm(-1.0, W1, B2, av, 2 * B2, 0.0, W2, B2, bs);                  // b
+        gemm(1.0, U, B2, W2, B2, 0.0, F1, B2, bs);                        // F1 = U b    (V1 is free: a' is not needed here)
+        gemm(1.0, U, B2, bpv, 2 * B2, 0.0, F2, B2, bs);                   // F2 = U b'
+    } else {
+        gemm(-1.0, V1, B2, bpv, 2 * B2, 0.0, W2, B2, bs);                 // a'
+        gemm(1.0, Lc, B2, av, 2 * B2, 0.0, F1, B2, bs);                   // F1 = L a
+        gemm(1.0, Lc, B2, W2, B2, 0.0, F2, B2, bs);                       // F2 = L a'
+    }
+    // row updates.  Column 0 lives in slots 0..nb-1, column 1 in slots 1..nb.
+    const cplx* Qs = slot_ptr(h, 0, 0, 0);
+    const cplx* Ps = slot_ptr(h, 0, 1, 1);
+    auto batched = [&](double alpha, const cplx* A, const cplx* F, double beta, const cplx* C) {   // all blocks and energies at once
+        GemmArgs g = gemm_std(bs, bs, bs, alpha, bp_two_level(A, nb, B2, sE), bs, bp_two_level(F, nb, 0, B2), bs, beta,
+                              bp_two_level(C, nb, B2, sE), bs);
+        gemm_run(ctx, g, nE * nb, GEMM_BIG, EPI_STD);
+    };
+    auto in_place = [&](const cplx* Col, const cplx* F) {                 // Col_i = -Col_i F, block by block through a scratch block
+        for (int i = 0; i < nb; i++) {
+            gemm(-1.0, Col + (long long)i * B2, sE, F, B2, 0.0, W1, B2, bs);
+            ctx.note(cudaMemcpy2DAsync((cplx*)Col + (long long)i * B2, sizeof(cplx) * (size_t)sE, W1, sizeof(cplx) * (size_t)B2,
+                                       sizeof(cplx) * (size_t)B2, (size_t)nE, cudaMemcpyDeviceToDevice, ctx.st));
+        }
+    };
+    if (part == 0) {
+        batched(-1.0, Ps, F1, 1.0, Qs);                                   // Q_i = QT_i - PT_i (U b)
+        in_place(Ps, F2);                                                 // P_i = -PT_i (U b')
+    } else {
+        batched(-1.0, Qs, F2, 1.0, Ps);                                   // P_i = PB_i - QB_i (L a')
+        in_place(Qs, F1);                                                 // Q_i = -QB_i (L a)
+    }
+    cudaEventRecord(h->ev[2], main);
+    cudaEventRecord(h->ev_out, main);
+    cudaStreamWaitEvent(user, h->ev_out, 0);
+    h->part = part;
+    h->last_stream = user;
+    if (ctx.err != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_post_partition(ss_handle_t h, const ss_cplx* peer_corner_dev, const ss_cplx* Sigma_L,
+                                         const ss_cplx* Sigma_R, const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs,
+                                         ss_cplx* X_rows, void* cuda_stream) {
+    if (!h || !peer_corner_dev || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
+    if (nrhs > 0 && (!Inj_first || !X_rows)) return SS_ERR_INVALID_ARG;
+    if (!h->launched || h->part < 0) return SS_ERR_NOT_READY;
+    return run_phases(h, nullptr, PH_POST, 3, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X_rows, peer_corner_dev, cuda_stream);
 }
 
 extern "C" ss_status_t ss_post_column(ss_handle_t h, int column, const ss_cplx* peer_corner_dev, const ss_cplx* Sigma_L,
@@ -974,7 +1121,7 @@ extern "C" ss_status_t ss_inverse_columns(ss_handle_t h, int energy, const ss_cp
 
 extern "C" ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cplx* Q_out, ss_cplx* P_out) {
     if (!h || energy < 0 || energy >= h->n_energy) return SS_ERR_INVALID_ARG;
-    if (!h->solved) return SS_ERR_NOT_READY;
+    if (!h->launched || h->swept_cols != 3) return SS_ERR_NOT_READY;        // both block columns swept (ss_solve, ss_sweep_partition)
     const size_t B2 = (size_t)h->bs * h->bs, bytes = sizeof(cplx) * (size_t)h->nb * B2;
     const cplx *q, *p;
     cudaMemcpyKind kind = cudaMemcpyDeviceToDevice;

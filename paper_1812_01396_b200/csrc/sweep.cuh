@@ -118,6 +118,17 @@ corner_init_kernel(cplx* __restrict__ Raug, long long stride, int W, int ld, int
     }
 }
 
+// Spatial split: [M | rhs] of the two interface systems of the merge, per chain z = 2 e + q:
+// dst(z) (bs x 2bs, ld) = [ 1 | rhs_q[e] ]; the products are subtracted from the left half afterwards.
+__global__ void __launch_bounds__(256)
+merge_init_kernel(BPtr dst, int ld, int bs, const cplx* __restrict__ rhs0, long long s0, const cplx* __restrict__ rhs1, long long s1) {
+    const int z = blockIdx.z, r = blockIdx.y;
+    cplx* __restrict__ row = bptr(dst, z) + (long long)r * ld;
+    const cplx* __restrict__ rhs = ((z & 1) ? rhs1 + (long long)(z >> 1) * s1 : rhs0 + (long long)(z >> 1) * s0) + (long long)r * bs;
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < 2 * bs; c += gridDim.x * blockDim.x)
+        row[c] = (c < bs) ? make_c(c == r ? 1.0 : 0.0, 0.0) : rhs[c - bs];
+}
+
 // out[e][r][c] = i (Sigma[e][r][c] - conj(Sigma[e][c][r]))
 __global__ void __launch_bounds__(256)
 gamma_kernel(const cplx* __restrict__ Sigma, cplx* __restrict__ out, int bs) {

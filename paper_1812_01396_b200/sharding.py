@@ -127,3 +127,64 @@ class LibraryColumnEngine:
     def post(self, column, peer):
         X = self.ss.post_column(column, peer.contiguous(), *self.args)
         return X, self.ss.transmission()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f2), second half: ONE energy batch on TWO GPUs, the device split along the transport axis
+# ---------------------------------------------------------------------------------------------------------
+# PAPER.md L167 ("horizontal split into two halves"), L169 (SPIKE): rank 0 of a pair owns the top h blocks of the device,
+# rank 1 the other nb - h, each only ITS slices of H and S.  Per rank: sweep of the sub-device (first / last block column of
+# A_T^-1 resp. A_B^-1); exchange of the two interface blocks (top: last block of both columns, bottom: first); the
+# SPIKE-style merge (two bs x bs interface systems, solved redundantly; include/splitsolve.h has the equations) turns the
+# local columns into the rank's rows of the global Q, P; exchange of the two outer corner blocks; corner system and T(E)
+# redundantly, X for the own rows.  X ends up distributed by rows (no reduction).  Bytes over the link per energy:
+# 2 x 2 bs^2 x 16 each way.
+#
+# `engine` (per rank): sweep(); edge(edge) -> tensor [n_energy, 2, bs, bs]; merge(part, peer_iface);
+#                      post(peer_corner) -> (X_rows tensor, T numpy).
+
+def split_blocks(nb: int):
+    """Blocks of the top half: h = ceil(nb / 2); the bottom half gets the rest (both >= 1 for nb >= 2)."""
+    return (nb + 1) // 2
+
+
+def _exchange(mine, rank, group):
+    import torch
+    import torch.distributed as dist
+    mine = mine.contiguous()
+    both = [torch.empty_like(mine), torch.empty_like(mine)]
+    dist.all_gather([torch.view_as_real(t) for t in both], torch.view_as_real(mine), group=group)
+    return both[1 - (rank & 1)]
+
+
+def spatial_split_solve(engine, rank: int, group=None):
+    """Runs the two-partition split on this rank (part = rank & 1) and returns (X_rows of this half, T)."""
+    part = rank & 1
+    engine.sweep()
+    peer_iface = _exchange(engine.edge(1 if part == 0 else 0), rank, group)
+    engine.merge(part, peer_iface)
+    peer_corner = _exchange(engine.edge(0 if part == 0 else 1), rank, group)
+    return engine.post(peer_corner)
+
+
+class LibraryPartitionEngine:
+    """The CUDA library behind spatial_split_solve: a SplitSolve handle created for THIS rank's sub-device (with its
+    slices of H and S registered), the coupling blocks S_{h,h+1}, H_{h,h+1} and the (replicated) boundary inputs."""
+
+    def __init__(self, ss, E, S_couple, H_couple, Sigma_L, Sigma_R, Inj_first, Inj_last=None):
+        self.ss, self.E = ss, E
+        self.couple = (S_couple, H_couple)
+        self.args = (Sigma_L, Sigma_R, Inj_first, Inj_last)
+
+    def sweep(self):
+        self.ss.sweep_partition(self.E)
+
+    def edge(self, edge):
+        return self.ss.edge_blocks(edge)
+
+    def merge(self, part, peer_iface):
+        self.ss.merge_partition(part, peer_iface.contiguous(), *self.couple)
+
+    def post(self, peer_corner):
+        X = self.ss.post_partition(peer_corner.contiguous(), *self.args)
+        return X, self.ss.transmission()

@@ -89,3 +89,103 @@ def test_column_split_world2_matches_dense_oracle(tmp_path):
         assert np.abs(X - Xo).max() <= 1e-10 * np.abs(Xo).max(), rank
         assert np.abs(T - To).max() <= 1e-10 * np.abs(To).max(), rank
     assert sharding.column_of_rank(0) == 0 and sharding.column_of_rank(1) == 1 and sharding.column_of_rank(2) == 0
+
+
+# ------------------------------------------------------------------------------------------------------
+# spatial split (two halves of the device, SPIKE-style merge): sharding.spatial_split_solve on gloo
+# ------------------------------------------------------------------------------------------------------
+class OraclePartitionEngine:
+    """CPU stand-in for the library's partition calls.  Sub-device columns from oracle/stepwise.py on the rank's slices of H, S;
+    the merge written out in numpy from the interface equations (include/splitsolve.h, ss_merge_partition); the corner system
+    from the four corner blocks."""
+
+    def __init__(self, p, part):
+        h = sharding.split_blocks(p.nb)
+        self.p, self.part, self.h = p, part, h
+        lo, hi = (0, h) if part == 0 else (h, p.nb)
+        self.Hd, self.Sd = p.H_diag[lo:hi], p.S_diag[lo:hi]
+        self.Hu, self.Su = p.H_upper[lo:hi - 1], p.S_upper[lo:hi - 1]
+        self.Hc, self.Sc = p.H_upper[h - 1], p.S_upper[h - 1]                 # coupling blocks (h, h+1)
+
+    def sweep(self):
+        from oracle import stepwise
+        p = self.p
+        self.Q = np.stack([stepwise.algorithm1_first_column(p.E[e], self.Hd, self.Hu, self.Sd, self.Su)[0] for e in range(p.n_energy)])
+        self.P = np.stack([stepwise.algorithm1_last_column(p.E[e], self.Hd, self.Hu, self.Sd, self.Su)[0] for e in range(p.n_energy)])
+
+    def edge(self, edge):
+        i = -1 if edge else 0
+        return torch.from_numpy(np.ascontiguousarray(np.stack([self.Q[:, i], self.P[:, i]], axis=1)))
+
+    def merge(self, part, peer):
+        p, peer = self.p, peer.numpy()
+        for e in range(p.n_energy):
+            U = p.E[e] * self.Sc - self.Hc
+            L = p.E[e] * self.Sc.conj().T - self.Hc.conj().T
+            one = np.eye(p.bs)
+            if part == 0:
+                QTh, PTh, QB1, PB1 = self.Q[e, -1], self.P[e, -1], peer[e, 0], peer[e, 1]
+            else:
+                QTh, PTh, QB1, PB1 = peer[e, 0], peer[e, 1], self.Q[e, 0], self.P[e, 0]
+            a = np.linalg.solve(one - PTh @ U @ QB1 @ L, QTh)
+            b = -QB1 @ L @ a
+            b2 = np.linalg.solve(one - QB1 @ L @ PTh @ U, PB1)
+            a2 = -PTh @ U @ b2
+            if part == 0:
+                Qn = self.Q[e] - self.P[e] @ (U @ b)
+                Pn = -self.P[e] @ (U @ b2)
+            else:
+                Pn = self.P[e] - self.Q[e] @ (L @ a2)
+                Qn = -self.Q[e] @ (L @ a)
+            self.Q[e], self.P[e] = Qn, Pn
+
+    def post(self, peer):
+        from oracle import dense
+        p, bs, peer = self.p, self.p.bs, peer.numpy()
+        Xs, Ts = [], []
+        for e in range(p.n_energy):
+            if self.part == 0:
+                q1, p1, qn, pn = self.Q[e, 0], self.P[e, 0], peer[e, 0], peer[e, 1]
+            else:
+                q1, p1, qn, pn = peer[e, 0], peer[e, 1], self.Q[e, -1], self.P[e, -1]
+            R = np.eye(2 * bs, dtype=np.complex128)
+            R[:bs, :bs] -= p.Sigma_L[e] @ q1
+            R[:bs, bs:] -= p.Sigma_L[e] @ p1
+            R[bs:, :bs] -= p.Sigma_R[e] @ qn
+            R[bs:, bs:] -= p.Sigma_R[e] @ pn
+            b = np.concatenate([p.Inj_first[e], np.zeros_like(p.Inj_first[e]) if p.Inj_last is None else p.Inj_last[e]])
+            Rinv = np.linalg.inv(R)
+            w = Rinv @ b
+            Xs.append((self.Q[e] @ w[:bs] + self.P[e] @ w[bs:]).reshape(-1, b.shape[1]))
+            Ts.append(dense.transmission_from_G(p.Sigma_L[e], p.Sigma_R[e], q1 @ Rinv[:bs, bs:] + p1 @ Rinv[bs:, bs:]).real)
+        return torch.from_numpy(np.stack(Xs)), np.array(Ts)
+
+
+def _spatial_worker(rank, world, port, out_dir, nb):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        p = inputs.random_problem(4, nb, 2, 3, seed=43, inj_last=True)
+        X, T = sharding.spatial_split_solve(OraclePartitionEngine(p, rank & 1), rank)
+        np.save(os.path.join(out_dir, f"X_{rank}.npy"), X.numpy())
+        np.save(os.path.join(out_dir, f"T_{rank}.npy"), T)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("nb", [2, 5, 6])
+def test_spatial_split_world2_matches_dense_oracle(tmp_path, nb):
+    """The two halves' X rows stacked equal the dense oracle's X; T(E) is complete on both ranks; odd nb (uneven halves) and
+    the smallest device (one block per half) included."""
+    from oracle import dense
+    port = _free_port()
+    mp.spawn(_spatial_worker, args=(2, port, str(tmp_path), nb), nprocs=2, join=True)
+    p = inputs.random_problem(4, nb, 2, 3, seed=43, inj_last=True)
+    Xo, To = dense.solve_all(p)
+    X = np.concatenate([np.load(tmp_path / "X_0.npy"), np.load(tmp_path / "X_1.npy")], axis=1)
+    assert X.shape == Xo.shape
+    assert np.abs(X - Xo).max() <= 1e-10 * np.abs(Xo).max()
+    for rank in range(2):
+        assert np.abs(np.load(tmp_path / f"T_{rank}.npy") - To).max() <= 1e-10 * np.abs(To).max()
+    assert sharding.split_blocks(2) == 1 and sharding.split_blocks(5) == 3 and sharding.split_blocks(6) == 3

@@ -756,3 +756,45 @@ def test_offload_columns_repeated_solves_and_column_split(lib):
     check_against_oracle(p, dict(X=(parts[0] + parts[1]).cpu().numpy(), T=T))
     for s2, _ in ranks:
         s2.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# SURVEY.md 8(f2), second half: the device split into two halves with a SPIKE-style merge -- the
+# library's partition calls, both "ranks" emulated on one GPU (two handles on the two sub-devices, exchanges by tensor
+# copies); the 2-rank orchestration runs in tests/test_column_split_gloo.py
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("bs,nb,n_e,nrhs,inj_last,groups", [(16, 8, 4, 4, False, 4), (150, 5, 2, 21, True, 2), (70, 4, 3, 9, True, 1),
+                                                            (200, 7, 2, 33, False, 2)])
+def test_spatial_split_calls_vs_oracle(lib, bs, nb, n_e, nrhs, inj_last, groups):
+    from paper_1812_01396_b200 import sharding
+    p = inputs.random_problem(bs, nb, n_e, nrhs, seed=44, inj_last=inj_last)
+    h = sharding.split_blocks(nb)
+    sl, sr, i1, i2 = dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first), dev(p.Inj_last)
+    Sc, Hc = dev(p.S_upper[h - 1]), dev(p.H_upper[h - 1])
+    halves = []
+    for part, (lo, hi) in enumerate(((0, h), (h, nb))):
+        ss = lib.SplitSolve(hi - lo, bs, n_e)
+        ss.set_option("stream_groups", groups)
+        ss.set_hamiltonian(dev(p.H_diag[lo:hi]), dev(p.H_upper[lo:hi - 1]), dev(p.S_diag[lo:hi]), dev(p.S_upper[lo:hi - 1]))
+        with pytest.raises(lib.SplitSolveError):                   # merge before sweep
+            ss.merge_partition(part, torch.zeros((n_e, 2, bs, bs), dtype=torch.complex128, device="cuda"), Sc, Hc)
+        ss.sweep_partition(p.E)
+        halves.append(ss)
+    iface = [halves[0].edge_blocks(1), halves[1].edge_blocks(0)]
+    for part in range(2):
+        halves[part].merge_partition(part, iface[1 - part], Sc, Hc)
+    # after the merge each half holds its rows of the global inverse block columns
+    for e in range(n_e):
+        Q, P = dense.inverse_columns(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+        for part, (lo, hi) in enumerate(((0, h), (h, nb))):
+            q, pp = halves[part].inverse_columns(e)
+            assert residual.rel_frobenius(q.cpu().numpy(), Q[lo:hi]) <= TOL_X, (e, part)
+            assert residual.rel_frobenius(pp.cpu().numpy(), P[lo:hi]) <= TOL_X, (e, part)
+    corner = [halves[0].edge_blocks(0), halves[1].edge_blocks(1)]
+    parts = [halves[part].post_partition(corner[1 - part], sl, sr, i1, i2) for part in range(2)]
+    Ts = [halves[part].transmission() for part in range(2)]
+    X = torch.cat(parts, dim=1).cpu().numpy()
+    assert np.array_equal(Ts[0], Ts[1])
+    check_against_oracle(p, dict(X=X, T=Ts[0]))
+    for ss in halves:
+        ss.close()
