@@ -294,9 +294,7 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     if spatial_split:
         # this rank's half of the device: rows [lo, hi) of the block stacks (the whole H, S were generated / broadcast above;
         # a production caller would only ever hold its slices)
-        hsplit = sharding.split_blocks(nb)
-        lo, hi = (0, hsplit) if (rank & 1) == 0 else (hsplit, nb)
-        S_c, H_c = devt["S_upper"][hsplit - 1].contiguous(), devt["H_upper"][hsplit - 1].contiguous()
+        lo, hi = sharding.partition_bounds(nb, 2)[rank & 1]
         ss = binding.SplitSolve(hi - lo, bs, nE)
     else:
         ss = binding.SplitSolve(nb, bs, nE)
@@ -316,10 +314,12 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
 
     col_T = [None]
     if spatial_split:
-        engine = sharding.LibraryPartitionEngine(ss, p.E, S_c, H_c, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None)
+        def couple(hb):
+            return devt["S_upper"][hb - 1].contiguous(), devt["H_upper"][hb - 1].contiguous()
+        engine = sharding.LibraryPartitionEngine(ss, p.E, couple, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None)
 
         def step():
-            _, col_T[0] = sharding.spatial_split_solve(engine, rank, group=pair_group)
+            _, col_T[0] = sharding.spatial_split_solve(engine, nb, rank & 1, 2, group=pair_group)
     elif column_split:
         engine = sharding.LibraryColumnEngine(ss, p.E, devt["Sigma_L"], devt["Sigma_R"], devt["Inj_first"], None)
 

@@ -130,29 +130,36 @@ ss_status_t ss_post_column(ss_handle_t h, int column, const ss_cplx* peer_corner
                            const ss_cplx* Sigma_R_dev, const ss_cplx* Inj_first_dev, const ss_cplx* Inj_last_dev, int nrhs,
                            ss_cplx* X_part_dev, void* cuda_stream);
 
-/* ---- one energy batch on two GPUs, split ALONG THE DEVICE ("horizontal split", L169 SPIKE) --
- * GPU 0 owns the top h blocks of the device, GPU 1 the other nb - h: each creates a handle for ITS sub-device (its slices of
- * H_diag/S_diag, H_upper/S_upper) -- so neither holds the whole H, S nor the whole block columns.
- *     ss_sweep_partition(h, E)                       a0-a4 on the sub-device: first and last block column of A_T^-1 resp. A_B^-1
- *     ss_get_edge_blocks(h, edge, out)               out[e][0] / out[e][1] = block `edge` (0 first, 1 last) of the first / last column
- *     -- exchange the interface blocks: top sends edge 1, bottom sends edge 0 (2 blocks per energy each way) --
- *     ss_merge_partition(h, part, peer_iface, S_c, H_c)
- *                                                    part 0 = top, 1 = bottom; S_c, H_c = the coupling blocks S_{h,h+1},
- *                                                    H_{h,h+1} (device, [bs][bs]).  With U = E S_c - H_c, L = E S_c^H - H_c^H both
- *                                                    GPUs solve (1 - PT_h U QB_1 L) a = QT_h and (1 - QB_1 L PT_h U) b' = PB_1
- *                                                    redundantly and update their rows: top Q_i = QT_i - PT_i U b, P_i = -PT_i U b'
- *                                                    (b = -QB_1 L a), bottom Q_i = -QB_i L a, P_i = PB_i - QB_i L a' (a' = -PT_h U b').
- *                                                    Afterwards the handle holds its rows of the GLOBAL Q, P.
- *     -- exchange the outer corner blocks: top sends edge 0 (Q_1, P_1), bottom sends edge 1 (Q_nb, P_nb) --
- *     ss_post_partition(h, peer_corner, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X_rows)
- *                                                    a5, a7 redundantly on both GPUs, a6 for the own rows:
- *                                                    X_rows [n_energy][nb_local*bs][nrhs]; X is the two halves stacked.
- * Not available together with option "offload_columns".  Buffers: out_dev / peer_*_dev [n_energy][2][bs][bs], device. */
+/* ---- one energy batch on 2^k GPUs, split ALONG THE DEVICE ("horizontal split", L169 SPIKE:
+ * "power of 2" partitions merged recursively).  Every GPU owns a contiguous run of blocks and creates a handle for ITS
+ * sub-device (its slices of H_diag/S_diag, H_upper/S_upper; >= 2 blocks) -- none holds the whole H, S or whole block columns.
+ *     ss_sweep_partition(h, E)                       a0-a4 on the sub-device: first and last block column of its own inverse
+ *     ss_get_edge_blocks(h, edge, out)               out[e][0] / out[e][1] = block `edge` (0 first, 1 last) of the first / last
+ *                                                    block column the handle currently holds
+ *     per merge level (teams of 2, 4, ... partitions; top half = part 0, bottom half = part 1):
+ *       -- gather iface[e][0] = edge 1 of the LAST partition of the top half, iface[e][1] = edge 0 of the FIRST partition of the
+ *          bottom half ([n_energy][2][2][bs][bs]) on every GPU of the team --
+ *       ss_merge_partition(h, part, iface, S_c, H_c) S_c, H_c = the coupling blocks S_{h,h+1}, H_{h,h+1} of the boundary (device,
+ *                                                    [bs][bs]).  With U = E S_c - H_c, L = E S_c^H - H_c^H, (QT_h, PT_h) = iface[e][0],
+ *                                                    (QB_1, PB_1) = iface[e][1], every GPU solves
+ *                                                        (1 - PT_h U QB_1 L) a = QT_h,  b = -QB_1 L a,
+ *                                                        (1 - QB_1 L PT_h U) b' = PB_1, a' = -PT_h U b'
+ *                                                    redundantly and updates ITS rows: in the top half Q_i = QT_i - PT_i (U b),
+ *                                                    P_i = -PT_i (U b'); in the bottom half Q_i = -QB_i (L a), P_i = PB_i - QB_i (L a').
+ *                                                    Afterwards the handles of the team hold the rows of the first / last block
+ *                                                    column of the inverse of the JOINED sub-device.
+ *     -- gather corners[e][0] = edge 0 of the first partition (Q_1, P_1), corners[e][1] = edge 1 of the last (Q_nb, P_nb) --
+ *     ss_post_partition(h, corners, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X_rows)
+ *                                                    a5, a7 redundantly on every GPU, a6 for the own rows:
+ *                                                    X_rows [n_energy][nb_local*bs][nrhs]; X is the partitions stacked.
+ * (The paper gives no equations for the merge -- its Fig. 6 is not in PAPER.md; these follow from the two halves being
+ * coupled through U and L only: x_T = QT - PT U x_{B,1}, x_B = -QB L x_{T,h} for the first block column, and likewise for
+ * the last.)  Not available together with option "offload_columns".  Buffers are caller-owned device memory. */
 ss_status_t ss_sweep_partition(ss_handle_t h, const ss_cplx* E_host, void* cuda_stream);
 ss_status_t ss_get_edge_blocks(ss_handle_t h, int edge, ss_cplx* out_dev, void* cuda_stream);
-ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx* peer_iface_dev, const ss_cplx* S_couple_dev,
+ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx* iface_dev, const ss_cplx* S_couple_dev,
                                const ss_cplx* H_couple_dev, void* cuda_stream);
-ss_status_t ss_post_partition(ss_handle_t h, const ss_cplx* peer_corner_dev, const ss_cplx* Sigma_L_dev, const ss_cplx* Sigma_R_dev,
+ss_status_t ss_post_partition(ss_handle_t h, const ss_cplx* corners_dev, const ss_cplx* Sigma_L_dev, const ss_cplx* Sigma_R_dev,
                               const ss_cplx* Inj_first_dev, const ss_cplx* Inj_last_dev, int nrhs, ss_cplx* X_rows_dev,
                               void* cuda_stream);
 

@@ -204,12 +204,16 @@ class SplitSolve:
         _check(load().ss_get_edge_blocks(self._h, int(edge), out.data_ptr(), _stream()), "ss_get_edge_blocks")
         return out
 
-    def merge_partition(self, part: int, peer_iface, S_couple, H_couple):
-        self._keep_merge = [peer_iface, S_couple, H_couple]
-        _check(load().ss_merge_partition(self._h, int(part), _dev(peer_iface, "peer_iface"), _dev(S_couple, "S_couple"),
+    def merge_partition(self, part: int, iface, S_couple, H_couple):
+        """iface [n_energy, 2, 2, bs, bs]: [:, 0] = last block of both columns of the top partition, [:, 1] = first block of
+        both columns of the bottom partition."""
+        self._keep_merge = [iface, S_couple, H_couple]
+        _check(load().ss_merge_partition(self._h, int(part), _dev(iface, "iface"), _dev(S_couple, "S_couple"),
                                          _dev(H_couple, "H_couple"), _stream()), "ss_merge_partition")
 
-    def post_partition(self, peer_corner, Sigma_L, Sigma_R, Inj_first, Inj_last=None, X_rows=None):
+    def post_partition(self, corners, Sigma_L, Sigma_R, Inj_first, Inj_last=None, X_rows=None):
+        """corners [n_energy, 2, 2, bs, bs]: [:, 0] = first block, [:, 1] = last block of the global (Q, P) columns."""
+        peer_corner = corners
         import torch
         nrhs = 0 if Inj_first is None else int(Inj_first.shape[-1])
         if X_rows is None and nrhs > 0:

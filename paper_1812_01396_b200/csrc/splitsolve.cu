@@ -574,7 +574,6 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     // corner blocks [column][first / last block] with their energy strides
     const cplx* cor[2][2] = {{slot(0, 0), slot(0, nb - 1)}, {slot(1, 1), slot(1, nb)}};
     long long cor_s[2] = {s_slot_e, s_slot_e};
-    long long cor_far_s = 0; int far_idx = -1;        // spatial split: stride of the peer's corner blocks, which end they are
     if (h->offload)                                   // saved aside when they were produced (the ring has moved on)
         for (int c = 0; c < 2; c++) {
             cor[c][0] = h->corner + ((long long)e0 * 2 + c) * 2 * B2; cor[c][1] = cor[c][0] + B2; cor_s[c] = 4 * B2;
@@ -583,12 +582,11 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
         const int other = (G.cols == 1) ? 1 : 0;
         cor[other][0] = peer + (long long)e0 * 2 * B2; cor[other][1] = cor[other][0] + B2; cor_s[other] = 2 * B2;
     } else if (h->part >= 0) {
-        // spatial split: this handle holds the rows of one half of the device (merged, global Q_i / P_i); the corner blocks at
-        // the far end of the device, peer[e][column], come from the other half
-        const int far = h->part == 0 ? 1 : 0;
-        for (int c = 0; c < 2; c++) { cor[c][far] = peer + ((long long)e0 * 2 + c) * B2; }
-        // strides: own blocks keep the slot stride; the peer's are [n_energy][2][bs*bs]
-        cor_far_s = 2 * B2; far_idx = far;
+        // spatial split: this handle holds the rows of one partition of the device (merged: global Q_i, P_i); the corner
+        // blocks of the whole device come gathered in peer[e][first / last][column]
+        for (int c = 0; c < 2; c++)
+            for (int q = 0; q < 2; q++) cor[c][q] = peer + (((long long)e0 * 2 + q) * 2 + c) * B2;
+        cor_s[0] = cor_s[1] = 4 * B2;
     }
     const int zc = h->want_T ? bs : 0;                // columns of e_2 (for (R^-1)_{12}, (R^-1)_{22})
     const int W = 2 * bs + m + zc;
@@ -615,7 +613,7 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     const cplx* sig[2] = {SigL, SigR};
     for (int br = 0; br < 2; br++)
         for (int bc = 0; bc < 2; bc++) {
-            GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(cor[bc][br], br == far_idx ? cor_far_s : cor_s[bc]), bs, 1.0,
+            GemmArgs g = gemm_std(bs, bs, bs, -1.0, bp_strided(sig[br], B2), bs, bp_strided(cor[bc][br], cor_s[bc]), bs, 1.0,
                                   bp_strided(raug + (long long)br * bs * ldW + (long long)bc * bs, s_r), ldW);
             gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
         }
@@ -668,10 +666,10 @@ static void run_post(ss_handle_t h, Group& G, const cplx* SigL, const cplx* SigR
     }
     // a7: G_1N = Q_1 (R^-1)_12 + P_1 (R^-1)_22;  T = Re Tr(Gamma_L G Gamma_R G^H)
     if (h->want_T) {
-        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[0][0], far_idx == 0 ? cor_far_s : cor_s[0]), bs, bp_strided(wz + m, s_w), nr, 0.0,
+        GemmArgs g = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[0][0], cor_s[0]), bs, bp_strided(wz + m, s_w), nr, 0.0,
                               bp_strided(g1n, B2), bs);
         gemm_run(ctx, g, nE, GEMM_BIG, EPI_STD);
-        GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[1][0], far_idx == 0 ? cor_far_s : cor_s[1]), bs,
+        GemmArgs g2 = gemm_std(bs, bs, bs, 1.0, bp_strided(cor[1][0], cor_s[1]), bs,
                                bp_strided(wz + (long long)bs * nr + m, s_w), nr, 1.0, bp_strided(g1n, B2), bs);
         gemm_run(ctx, g2, nE, GEMM_BIG, EPI_STD);
         dim3 gg((unsigned)cdiv(bs, 32), (unsigned)cdiv(bs, 32), (unsigned)nE);
@@ -917,10 +915,10 @@ extern "C" ss_status_t ss_get_edge_blocks(ss_handle_t h, int edge, ss_cplx* out_
     return SS_OK;
 }
 
-extern "C" ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx* peer_iface_dev, const ss_cplx* S_couple_dev,
+extern "C" ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx* iface_dev, const ss_cplx* S_couple_dev,
                                           const ss_cplx* H_couple_dev, void* cuda_stream) {
-    if (!h || part < 0 || part > 1 || !peer_iface_dev || !S_couple_dev || !H_couple_dev) return SS_ERR_INVALID_ARG;
-    if (!h->launched || h->swept_cols != 3 || h->offload || h->part >= 0) return SS_ERR_NOT_READY;
+    if (!h || part < 0 || part > 1 || !iface_dev || !S_couple_dev || !H_couple_dev) return SS_ERR_INVALID_ARG;
+    if (!h->launched || h->swept_cols != 3 || h->offload) return SS_ERR_NOT_READY;
     const int nb = h->nb, bs = h->bs, nE = h->n_energy;
     const long long B2 = (long long)bs * bs, sE = slot_stride_e(h);
     cudaStream_t user = (cudaStream_t)cuda_stream, main = h->main_stream;
@@ -928,13 +926,12 @@ extern "C" ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx
     cudaEventRecord(h->ev_in, user);
     cudaStreamWaitEvent(main, h->ev_in, 0);
     Ctx ctx; ctx.st = main; ctx.variant = h->gemm_variant;
-    const cplx* peer = (const cplx*)peer_iface_dev;
-    // interface blocks (pointer of energy 0, energy stride): QT_h, PT_h of the top half, QB_1, PB_1 of the bottom half
-    const cplx* own[2];
-    edge_ptrs(h, part == 0 ? 1 : 0, own);
-    const cplx *QTh = part == 0 ? own[0] : peer, *PTh = part == 0 ? own[1] : peer + B2;
-    const cplx *QB1 = part == 1 ? own[0] : peer, *PB1 = part == 1 ? own[1] : peer + B2;
-    const long long sT = part == 0 ? sE : 2 * B2, sB = part == 1 ? sE : 2 * B2;
+    // interface blocks, gathered by the caller: iface[e][0] = (QT_h, PT_h), the LAST block of both columns of the top
+    // partition; iface[e][1] = (QB_1, PB_1), the FIRST block of both columns of the bottom partition.  (In a merge of
+    // partitions that are themselves spread over several GPUs, most ranks own neither.)
+    const cplx* ifc = (const cplx*)iface_dev;
+    const cplx *QTh = ifc, *PTh = ifc + B2, *QB1 = ifc + 2 * B2, *PB1 = ifc + 3 * B2;
+    const long long sT = 4 * B2, sB = 4 * B2;
     cplx *U = h->gam_l, *Lc = h->gam_r, *W1 = h->g1n, *V1 = h->w1, *W2 = h->w2;
     auto gemm = [&](double alpha, const cplx* A, long long sA, const cplx* B, long long sB_, double beta, cplx* C, long long sC, int ldc) {
         GemmArgs g = gemm_std(bs, bs, bs, alpha, bp_strided(A, sA), bs, bp_strided(B, sB_), bs, beta, bp_strided(C, sC), ldc);
@@ -1007,13 +1004,13 @@ extern "C" ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx
     return SS_OK;
 }
 
-extern "C" ss_status_t ss_post_partition(ss_handle_t h, const ss_cplx* peer_corner_dev, const ss_cplx* Sigma_L,
+extern "C" ss_status_t ss_post_partition(ss_handle_t h, const ss_cplx* corners_dev, const ss_cplx* Sigma_L,
                                          const ss_cplx* Sigma_R, const ss_cplx* Inj_first, const ss_cplx* Inj_last, int nrhs,
                                          ss_cplx* X_rows, void* cuda_stream) {
-    if (!h || !peer_corner_dev || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
+    if (!h || !corners_dev || !Sigma_L || !Sigma_R || nrhs < 0) return SS_ERR_INVALID_ARG;
     if (nrhs > 0 && (!Inj_first || !X_rows)) return SS_ERR_INVALID_ARG;
     if (!h->launched || h->part < 0) return SS_ERR_NOT_READY;
-    return run_phases(h, nullptr, PH_POST, 3, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X_rows, peer_corner_dev, cuda_stream);
+    return run_phases(h, nullptr, PH_POST, 3, Sigma_L, Sigma_R, Inj_first, Inj_last, nrhs, X_rows, corners_dev, cuda_stream);
 }
 
 extern "C" ss_status_t ss_post_column(ss_handle_t h, int column, const ss_cplx* peer_corner_dev, const ss_cplx* Sigma_L,

@@ -130,61 +130,94 @@ class LibraryColumnEngine:
 
 
 # ---------------------------------------------------------------------------------------------------------
-# SURVEY.md 8(f2), second half: ONE energy batch on TWO GPUs, the device split along the transport axis
+# SURVEY.md 8(f2), second half: ONE energy batch on 2^k GPUs, the device split along the transport axis
 # ---------------------------------------------------------------------------------------------------------
-# PAPER.md L167 ("horizontal split into two halves"), L169 (SPIKE): rank 0 of a pair owns the top h blocks of the device,
-# rank 1 the other nb - h, each only ITS slices of H and S.  Per rank: sweep of the sub-device (first / last block column of
-# A_T^-1 resp. A_B^-1); exchange of the two interface blocks (top: last block of both columns, bottom: first); the
-# SPIKE-style merge (two bs x bs interface systems, solved redundantly; include/splitsolve.h has the equations) turns the
-# local columns into the rank's rows of the global Q, P; exchange of the two outer corner blocks; corner system and T(E)
-# redundantly, X for the own rows.  X ends up distributed by rows (no reduction).  Bytes over the link per energy:
-# 2 x 2 bs^2 x 16 each way.
+# PAPER.md L167 ("horizontal split into two halves"), L169 (SPIKE: "power of 2" partitions, merged recursively): every rank
+# of a team owns a contiguous run of blocks and only ITS slices of H and S.  Per rank: sweep of the sub-device (first / last
+# block column of its own inverse); then log2(world) merge levels: at level l teams of 2^(l+1) ranks join their top and
+# bottom halves through the two bs x bs interface systems of include/splitsolve.h (ss_merge_partition) -- every rank of the
+# team needs the LAST block of both columns held by the last rank of the top half and the FIRST block held by the first rank of
+# the bottom half, solves the interface systems redundantly and updates its own rows; finally the corner blocks (first
+# rank's first, last rank's last) go to everybody, the corner system and T(E) are computed redundantly and every rank forms
+# X for its own rows.  X ends up distributed by rows (no reduction).  What crosses the link: per level and rank 4 blocks per
+# energy in an all-gather (every rank contributes its two edge block pairs), i.e. world * 4 bs^2 * 16 B received.
 #
-# `engine` (per rank): sweep(); edge(edge) -> tensor [n_energy, 2, bs, bs]; merge(part, peer_iface);
-#                      post(peer_corner) -> (X_rows tensor, T numpy).
+# `engine` (per rank): sweep(); edges() -> tensor [2, n_energy, 2, bs, bs] (first / last block of the first and last
+# column); merge(part, iface [n_energy, 2, 2, bs, bs], boundary) with boundary = global index h of the first block of the
+# bottom half (the coupling blocks are S_upper[h-1], H_upper[h-1]); post(corners [n_energy, 2, 2, bs, bs]) -> (X_rows, T).
 
 def split_blocks(nb: int):
     """Blocks of the top half: h = ceil(nb / 2); the bottom half gets the rest (both >= 1 for nb >= 2)."""
     return (nb + 1) // 2
 
 
-def _exchange(mine, rank, group):
+def partition_bounds(nb: int, world: int, lo: int = 0):
+    """[(lo, hi)) block ranges of `world` = 2^k partitions by recursive halving (the merge tree splits the same way)."""
+    if world < 1 or world & (world - 1):
+        raise ValueError("the number of partitions must be a power of 2 (PAPER.md L169)")
+    if world == 1:
+        return [(lo, lo + nb)]
+    h = split_blocks(nb)
+    return partition_bounds(h, world // 2, lo) + partition_bounds(nb - h, world // 2, lo + h)
+
+
+def merge_plan(nb: int, world: int, rank: int):
+    """The merge levels of `rank`: list of (part, rank of the top half's last partition, rank of the bottom half's first
+    partition, boundary block index)."""
+    bounds = partition_bounds(nb, world)
+    plan = []
+    size = 2
+    while size <= world:
+        r0 = (rank // size) * size
+        mid = r0 + size // 2
+        plan.append((0 if rank < mid else 1, mid - 1, mid, bounds[mid][0]))
+        size *= 2
+    return plan
+
+
+def _all_gather(t, group):
     import torch
     import torch.distributed as dist
-    mine = mine.contiguous()
-    both = [torch.empty_like(mine), torch.empty_like(mine)]
-    dist.all_gather([torch.view_as_real(t) for t in both], torch.view_as_real(mine), group=group)
-    return both[1 - (rank & 1)]
+    t = t.contiguous()
+    out = [torch.empty_like(t) for _ in range(dist.get_world_size(group))]
+    dist.all_gather([torch.view_as_real(x) for x in out], torch.view_as_real(t), group=group)
+    return out
 
 
-def spatial_split_solve(engine, rank: int, group=None):
-    """Runs the two-partition split on this rank (part = rank & 1) and returns (X_rows of this half, T)."""
-    part = rank & 1
+def spatial_split_solve(engine, nb: int, rank: int, world: int = 2, group=None):
+    """Runs the spatial split on this rank of a team of `world` = 2^k ranks (rank = index inside the team) and returns
+    (X_rows of this rank's blocks, T)."""
+    import torch
     engine.sweep()
-    peer_iface = _exchange(engine.edge(1 if part == 0 else 0), rank, group)
-    engine.merge(part, peer_iface)
-    peer_corner = _exchange(engine.edge(0 if part == 0 else 1), rank, group)
-    return engine.post(peer_corner)
+    for part, top_last, bottom_first, boundary in merge_plan(nb, world, rank):
+        edges = _all_gather(engine.edges(), group)                       # [world] x [2, nE, 2, bs, bs]
+        iface = torch.stack([edges[top_last][1], edges[bottom_first][0]], dim=1)      # [nE, 2, 2, bs, bs]
+        engine.merge(part, iface, boundary)
+    edges = _all_gather(engine.edges(), group)
+    corners = torch.stack([edges[0][0], edges[world - 1][1]], dim=1)
+    return engine.post(corners)
 
 
 class LibraryPartitionEngine:
     """The CUDA library behind spatial_split_solve: a SplitSolve handle created for THIS rank's sub-device (with its
-    slices of H and S registered), the coupling blocks S_{h,h+1}, H_{h,h+1} and the (replicated) boundary inputs."""
+    slices of H and S registered), `couple(h)` returning the device tensors (S_upper[h-1], H_upper[h-1]) of a boundary,
+    and the (replicated) boundary inputs."""
 
-    def __init__(self, ss, E, S_couple, H_couple, Sigma_L, Sigma_R, Inj_first, Inj_last=None):
-        self.ss, self.E = ss, E
-        self.couple = (S_couple, H_couple)
+    def __init__(self, ss, E, couple, Sigma_L, Sigma_R, Inj_first, Inj_last=None):
+        self.ss, self.E, self.couple = ss, E, couple
         self.args = (Sigma_L, Sigma_R, Inj_first, Inj_last)
 
     def sweep(self):
         self.ss.sweep_partition(self.E)
 
-    def edge(self, edge):
-        return self.ss.edge_blocks(edge)
+    def edges(self):
+        import torch
+        return torch.stack([self.ss.edge_blocks(0), self.ss.edge_blocks(1)])
 
-    def merge(self, part, peer_iface):
-        self.ss.merge_partition(part, peer_iface.contiguous(), *self.couple)
+    def merge(self, part, iface, boundary):
+        S_c, H_c = self.couple(boundary)
+        self.ss.merge_partition(part, iface.contiguous(), S_c, H_c)
 
-    def post(self, peer_corner):
-        X = self.ss.post_partition(peer_corner.contiguous(), *self.args)
+    def post(self, corners):
+        X = self.ss.post_partition(corners.contiguous(), *self.args)
         return X, self.ss.transmission()

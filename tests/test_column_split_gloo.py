@@ -92,20 +92,17 @@ def test_column_split_world2_matches_dense_oracle(tmp_path):
 
 
 # ------------------------------------------------------------------------------------------------------
-# spatial split (two halves of the device, SPIKE-style merge): sharding.spatial_split_solve on gloo
+# spatial split (2^k partitions of the device, SPIKE-style merges): sharding.spatial_split_solve on gloo
 # ------------------------------------------------------------------------------------------------------
 class OraclePartitionEngine:
     """CPU stand-in for the library's partition calls.  Sub-device columns from oracle/stepwise.py on the rank's slices of H, S;
     the merge written out in numpy from the interface equations (include/splitsolve.h, ss_merge_partition); the corner system
     from the four corner blocks."""
 
-    def __init__(self, p, part):
-        h = sharding.split_blocks(p.nb)
-        self.p, self.part, self.h = p, part, h
-        lo, hi = (0, h) if part == 0 else (h, p.nb)
+    def __init__(self, p, lo, hi):
+        self.p = p
         self.Hd, self.Sd = p.H_diag[lo:hi], p.S_diag[lo:hi]
         self.Hu, self.Su = p.H_upper[lo:hi - 1], p.S_upper[lo:hi - 1]
-        self.Hc, self.Sc = p.H_upper[h - 1], p.S_upper[h - 1]                 # coupling blocks (h, h+1)
 
     def sweep(self):
         from oracle import stepwise
@@ -113,20 +110,18 @@ class OraclePartitionEngine:
         self.Q = np.stack([stepwise.algorithm1_first_column(p.E[e], self.Hd, self.Hu, self.Sd, self.Su)[0] for e in range(p.n_energy)])
         self.P = np.stack([stepwise.algorithm1_last_column(p.E[e], self.Hd, self.Hu, self.Sd, self.Su)[0] for e in range(p.n_energy)])
 
-    def edge(self, edge):
-        i = -1 if edge else 0
-        return torch.from_numpy(np.ascontiguousarray(np.stack([self.Q[:, i], self.P[:, i]], axis=1)))
+    def edges(self):
+        e = [np.stack([self.Q[:, i], self.P[:, i]], axis=1) for i in (0, -1)]
+        return torch.from_numpy(np.ascontiguousarray(np.stack(e)))
 
-    def merge(self, part, peer):
-        p, peer = self.p, peer.numpy()
+    def merge(self, part, iface, boundary):
+        p, iface = self.p, iface.numpy()
+        Hc, Sc = p.H_upper[boundary - 1], p.S_upper[boundary - 1]
         for e in range(p.n_energy):
-            U = p.E[e] * self.Sc - self.Hc
-            L = p.E[e] * self.Sc.conj().T - self.Hc.conj().T
+            U = p.E[e] * Sc - Hc
+            L = p.E[e] * Sc.conj().T - Hc.conj().T
             one = np.eye(p.bs)
-            if part == 0:
-                QTh, PTh, QB1, PB1 = self.Q[e, -1], self.P[e, -1], peer[e, 0], peer[e, 1]
-            else:
-                QTh, PTh, QB1, PB1 = peer[e, 0], peer[e, 1], self.Q[e, 0], self.P[e, 0]
+            QTh, PTh, QB1, PB1 = iface[e, 0, 0], iface[e, 0, 1], iface[e, 1, 0], iface[e, 1, 1]
             a = np.linalg.solve(one - PTh @ U @ QB1 @ L, QTh)
             b = -QB1 @ L @ a
             b2 = np.linalg.solve(one - QB1 @ L @ PTh @ U, PB1)
@@ -139,15 +134,12 @@ class OraclePartitionEngine:
                 Qn = -self.Q[e] @ (L @ a)
             self.Q[e], self.P[e] = Qn, Pn
 
-    def post(self, peer):
+    def post(self, corners):
         from oracle import dense
-        p, bs, peer = self.p, self.p.bs, peer.numpy()
+        p, bs, c = self.p, self.p.bs, corners.numpy()
         Xs, Ts = [], []
         for e in range(p.n_energy):
-            if self.part == 0:
-                q1, p1, qn, pn = self.Q[e, 0], self.P[e, 0], peer[e, 0], peer[e, 1]
-            else:
-                q1, p1, qn, pn = peer[e, 0], peer[e, 1], self.Q[e, -1], self.P[e, -1]
+            q1, p1, qn, pn = c[e, 0, 0], c[e, 0, 1], c[e, 1, 0], c[e, 1, 1]
             R = np.eye(2 * bs, dtype=np.complex128)
             R[:bs, :bs] -= p.Sigma_L[e] @ q1
             R[:bs, bs:] -= p.Sigma_L[e] @ p1
@@ -167,25 +159,28 @@ def _spatial_worker(rank, world, port, out_dir, nb):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         p = inputs.random_problem(4, nb, 2, 3, seed=43, inj_last=True)
-        X, T = sharding.spatial_split_solve(OraclePartitionEngine(p, rank & 1), rank)
+        lo, hi = sharding.partition_bounds(nb, world)[rank]
+        X, T = sharding.spatial_split_solve(OraclePartitionEngine(p, lo, hi), nb, rank, world)
         np.save(os.path.join(out_dir, f"X_{rank}.npy"), X.numpy())
         np.save(os.path.join(out_dir, f"T_{rank}.npy"), T)
     finally:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("nb", [2, 5, 6])
-def test_spatial_split_world2_matches_dense_oracle(tmp_path, nb):
-    """The two halves' X rows stacked equal the dense oracle's X; T(E) is complete on both ranks; odd nb (uneven halves) and
-    the smallest device (one block per half) included."""
+@pytest.mark.parametrize("nb,world", [(2, 2), (5, 2), (6, 2), (4, 4), (9, 4)])
+def test_spatial_split_matches_dense_oracle(tmp_path, nb, world):
+    """The partitions' X rows stacked equal the dense oracle's X; T(E) is complete on every rank.  Two partitions (one merge)
+    and four (two merge levels), uneven partitions, and the smallest devices (one block per partition)."""
     from oracle import dense
     port = _free_port()
-    mp.spawn(_spatial_worker, args=(2, port, str(tmp_path), nb), nprocs=2, join=True)
+    mp.spawn(_spatial_worker, args=(world, port, str(tmp_path), nb), nprocs=world, join=True)
     p = inputs.random_problem(4, nb, 2, 3, seed=43, inj_last=True)
     Xo, To = dense.solve_all(p)
-    X = np.concatenate([np.load(tmp_path / "X_0.npy"), np.load(tmp_path / "X_1.npy")], axis=1)
+    X = np.concatenate([np.load(tmp_path / f"X_{r}.npy") for r in range(world)], axis=1)
     assert X.shape == Xo.shape
     assert np.abs(X - Xo).max() <= 1e-10 * np.abs(Xo).max()
-    for rank in range(2):
+    for rank in range(world):
         assert np.abs(np.load(tmp_path / f"T_{rank}.npy") - To).max() <= 1e-10 * np.abs(To).max()
-    assert sharding.split_blocks(2) == 1 and sharding.split_blocks(5) == 3 and sharding.split_blocks(6) == 3
+    assert sharding.partition_bounds(9, 4) == [(0, 3), (3, 5), (5, 7), (7, 9)]
+    with pytest.raises(ValueError):
+        sharding.partition_bounds(9, 3)

@@ -763,38 +763,45 @@ def test_offload_columns_repeated_solves_and_column_split(lib):
 # library's partition calls, both "ranks" emulated on one GPU (two handles on the two sub-devices, exchanges by tensor
 # copies); the 2-rank orchestration runs in tests/test_column_split_gloo.py
 # ------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("bs,nb,n_e,nrhs,inj_last,groups", [(16, 8, 4, 4, False, 4), (150, 5, 2, 21, True, 2), (70, 4, 3, 9, True, 1),
-                                                            (200, 7, 2, 33, False, 2)])
-def test_spatial_split_calls_vs_oracle(lib, bs, nb, n_e, nrhs, inj_last, groups):
+@pytest.mark.parametrize("bs,nb,n_e,nrhs,inj_last,groups,world", [(16, 8, 4, 4, False, 4, 2), (150, 5, 2, 21, True, 2, 2),
+                                                                  (70, 4, 3, 9, True, 1, 2), (200, 7, 2, 33, False, 2, 2),
+                                                                  (16, 8, 2, 4, True, 2, 4), (70, 11, 2, 9, False, 1, 4)])
+def test_spatial_split_calls_vs_oracle(lib, bs, nb, n_e, nrhs, inj_last, groups, world):
+    """2 or 4 partitions (one or two merge levels), every "rank" a handle on its sub-device, the all-gathers done by hand
+    following sharding.merge_plan."""
     from paper_1812_01396_b200 import sharding
     p = inputs.random_problem(bs, nb, n_e, nrhs, seed=44, inj_last=inj_last)
-    h = sharding.split_blocks(nb)
+    bounds = sharding.partition_bounds(nb, world)
     sl, sr, i1, i2 = dev(p.Sigma_L), dev(p.Sigma_R), dev(p.Inj_first), dev(p.Inj_last)
-    Sc, Hc = dev(p.S_upper[h - 1]), dev(p.H_upper[h - 1])
-    halves = []
-    for part, (lo, hi) in enumerate(((0, h), (h, nb))):
+    ranks = []
+    for lo, hi in bounds:
         ss = lib.SplitSolve(hi - lo, bs, n_e)
         ss.set_option("stream_groups", groups)
         ss.set_hamiltonian(dev(p.H_diag[lo:hi]), dev(p.H_upper[lo:hi - 1]), dev(p.S_diag[lo:hi]), dev(p.S_upper[lo:hi - 1]))
         with pytest.raises(lib.SplitSolveError):                   # merge before sweep
-            ss.merge_partition(part, torch.zeros((n_e, 2, bs, bs), dtype=torch.complex128, device="cuda"), Sc, Hc)
+            ss.merge_partition(0, torch.zeros((n_e, 2, 2, bs, bs), dtype=torch.complex128, device="cuda"), sl, sr)
         ss.sweep_partition(p.E)
-        halves.append(ss)
-    iface = [halves[0].edge_blocks(1), halves[1].edge_blocks(0)]
-    for part in range(2):
-        halves[part].merge_partition(part, iface[1 - part], Sc, Hc)
-    # after the merge each half holds its rows of the global inverse block columns
+        ranks.append(ss)
+    plans = [sharding.merge_plan(nb, world, r) for r in range(world)]
+    for level in range(len(plans[0])):
+        edges = [torch.stack([ss.edge_blocks(0), ss.edge_blocks(1)]) for ss in ranks]       # the all-gather
+        for r, ss in enumerate(ranks):
+            part, top_last, bottom_first, h = plans[r][level]
+            iface = torch.stack([edges[top_last][1], edges[bottom_first][0]], dim=1).contiguous()
+            ss.merge_partition(part, iface, dev(p.S_upper[h - 1]), dev(p.H_upper[h - 1]))
+    # after the merges every partition holds its rows of the global inverse block columns
     for e in range(n_e):
         Q, P = dense.inverse_columns(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
-        for part, (lo, hi) in enumerate(((0, h), (h, nb))):
-            q, pp = halves[part].inverse_columns(e)
-            assert residual.rel_frobenius(q.cpu().numpy(), Q[lo:hi]) <= TOL_X, (e, part)
-            assert residual.rel_frobenius(pp.cpu().numpy(), P[lo:hi]) <= TOL_X, (e, part)
-    corner = [halves[0].edge_blocks(0), halves[1].edge_blocks(1)]
-    parts = [halves[part].post_partition(corner[1 - part], sl, sr, i1, i2) for part in range(2)]
-    Ts = [halves[part].transmission() for part in range(2)]
+        for r, (lo, hi) in enumerate(bounds):
+            q, pp = ranks[r].inverse_columns(e)
+            assert residual.rel_frobenius(q.cpu().numpy(), Q[lo:hi]) <= TOL_X, (e, r)
+            assert residual.rel_frobenius(pp.cpu().numpy(), P[lo:hi]) <= TOL_X, (e, r)
+    corners = torch.stack([ranks[0].edge_blocks(0), ranks[-1].edge_blocks(1)], dim=1).contiguous()
+    parts = [ss.post_partition(corners, sl, sr, i1, i2) for ss in ranks]
+    Ts = [ss.transmission() for ss in ranks]
     X = torch.cat(parts, dim=1).cpu().numpy()
-    assert np.array_equal(Ts[0], Ts[1])
+    for T in Ts[1:]:
+        assert np.array_equal(Ts[0], T)
     check_against_oracle(p, dict(X=X, T=Ts[0]))
-    for ss in halves:
+    for ss in ranks:
         ss.close()
