@@ -77,6 +77,10 @@ def parse():
                     "even rank, bottom half on the odd one, SPIKE-style merge (SURVEY 8(f2), PAPER.md L167, L169)")
     ap.add_argument("--real-energies", action="store_true", help="variant of the workload with Im E = 0 and the energy grid moved "
                     "above the spectrum ([3.5, 4.5]: A definite), for the Hermitian modes of SURVEY 8(f1) (--option hermitian=1|2)")
+    ap.add_argument("--emulate-split", default=None, choices=["column", "spatial"], help="ONE GPU: run the per-rank work of the "
+                    "two-GPU splits of SURVEY 8(f2) rank after rank (two handles), time each rank's phases with CUDA events and "
+                    "print the per-rank critical path; the exchanges are device copies here, their NVLink time is estimated "
+                    "from the bytes (see profiles/r02_split_emulation.md)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the second block (C3) of the default C4 line")
@@ -583,6 +587,67 @@ def kernel_density(args):
           f"rel err {err:.1e}")
 
 
+def emulate_split(args, cfg):
+    """Per-rank work of the 2-GPU splits, on one GPU (the ranks run one after the other, so nothing waits on anything)."""
+    import torch
+    from paper_1812_01396_b200 import binding, build, sharding
+    build.build()
+    nE, bs, nb, m = cfg.n_energy, cfg.bs, cfg.nb, cfg.nrhs
+    p = inputs.random_problem(bs, nb, 1, 1, seed=cfg.seed, threads=os.cpu_count() or 1)
+    E = inputs.energy_grid(nE, cfg.e_lo, cfg.e_hi, cfg.eta)
+    d = {k: torch.from_numpy(getattr(p, k)).cuda() for k in ("H_diag", "H_upper", "S_diag", "S_upper")}
+    sl = torch.from_numpy(np.stack([inputs.sigma_block(cfg.seed, e, bs, "L") for e in range(nE)])).cuda()
+    sr = torch.from_numpy(np.stack([inputs.sigma_block(cfg.seed, e, bs, "R") for e in range(nE)])).cuda()
+    inj = torch.from_numpy(np.stack([inputs.inj_block(cfg.seed, e, bs, m) for e in range(nE)])).cuda()
+    spatial = args.emulate_split == "spatial"
+    bounds = sharding.partition_bounds(nb, 2) if spatial else [(0, nb), (0, nb)]
+    hs = []
+    for lo, hi in bounds:
+        ss = binding.SplitSolve(hi - lo, bs, nE)
+        ss.set_hamiltonian(d["H_diag"][lo:hi].contiguous(), d["H_upper"][lo:hi - 1].contiguous(), d["S_diag"][lo:hi].contiguous(),
+                           d["S_upper"][lo:hi - 1].contiguous())
+        hs.append(ss)
+
+    def timed(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); e0.record(); out = fn(); e1.record(); torch.cuda.synchronize()
+        return out, e0.elapsed_time(e1)
+
+    res = []
+    for rep in range(args.warmup + args.steps):
+        t = [dict(), dict()]
+        if spatial:
+            hcut = bounds[1][0]
+            Sc, Hc = d["S_upper"][hcut - 1].contiguous(), d["H_upper"][hcut - 1].contiguous()
+            for r in range(2):
+                _, t[r]["sweep"] = timed(lambda: hs[r].sweep_partition(E))
+            edges = [torch.stack([ss.edge_blocks(0), ss.edge_blocks(1)]) for ss in hs]
+            iface = torch.stack([edges[0][1], edges[1][0]], dim=1).contiguous()
+            for r in range(2):
+                _, t[r]["merge"] = timed(lambda: hs[r].merge_partition(r, iface, Sc, Hc))
+            corners = torch.stack([hs[0].edge_blocks(0), hs[1].edge_blocks(1)], dim=1).contiguous()
+            for r in range(2):
+                _, t[r]["post"] = timed(lambda: (hs[r].post_partition(corners, sl, sr, inj), hs[r].transmission()))
+            link = 2 * nE * 4 * bs * bs * 16                       # two all-gathers of 4 blocks per energy and rank
+        else:
+            for r in range(2):
+                _, t[r]["sweep"] = timed(lambda: hs[r].sweep_column(E, r))
+            cb = [hs[r].corner_blocks(r) for r in range(2)]
+            t[0]["merge"] = t[1]["merge"] = 0.0
+            for r in range(2):
+                _, t[r]["post"] = timed(lambda: (hs[r].post_column(r, cb[1 - r], sl, sr, inj), hs[r].transmission()))
+            link = nE * 2 * bs * bs * 16 + nE * nb * bs * m * 16   # corner all-gather + sum-all-reduce of the X shares
+        if rep >= args.warmup:
+            res.append(t)
+    per_rank = [{k: float(np.mean([t[r][k] for t in res])) for k in ("sweep", "merge", "post")} for r in range(2)]
+    crit = max(sum(x.values()) for x in per_rank)
+    link_ms = link / 770e9 * 1e3
+    print(json.dumps({"emulate_split": args.emulate_split, "workload": cfg.name, "per_rank_ms": per_rank,
+                      "critical_path_ms": crit, "link_bytes_per_rank": link, "link_ms_at_770GBps": link_ms,
+                      "solves_per_s_two_gpus_estimate": nE / ((crit + link_ms) * 1e-3),
+                      "note": "ranks run one after the other on ONE GPU; exchanges are device copies; not a 2-GPU measurement"}), flush=True)
+
+
 def main():
     args = parse()
     cfg = inputs.CONFIGS[args.workload]
@@ -594,6 +659,9 @@ def main():
         return
     if args.kernel:
         (kernel_gemm if args.kernel == "gemm" else kernel_density)(args)
+        return
+    if args.emulate_split:
+        emulate_split(args, cfg)
         return
     if args.impl == "reference":
         run_reference(args, cfg)
