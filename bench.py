@@ -81,6 +81,9 @@ def parse():
                     "two-GPU splits of SURVEY 8(f2) rank after rank (two handles), time each rank's phases with CUDA events and "
                     "print the per-rank critical path; the exchanges are device copies here, their NVLink time is estimated "
                     "from the bytes (see profiles/r02_split_emulation.md)")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"], help="N > 1: torch.distributed backend.  'gloo' is "
+                    "for exercising the N > 1 code paths on a box with fewer GPUs than ranks (ranks share GPUs; every collective "
+                    "is a host-level call, no kernel waits for another rank's): a functional check, never a measurement")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the second block (C3) of the default C4 line")
@@ -430,8 +433,8 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
                    "convention": "LAPACK (complex multiply-add = 8 flops), closed form ss_flops; *_executed = x" + str(ratio) +
                    " (3M: 6 real flops per complex multiply-add)"},
         "roofline": {"bound": "tensor", "kernel": kern,
-                     "achieved": gemm_tf * ratio, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
-                     "frac": gemm_tf * ratio / FP64_PEAK_NOMINAL_TFLOPS,
+                     "achieved": gemm_tf * ratio if gemm_n else None, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                     "frac": gemm_tf * ratio / FP64_PEAK_NOMINAL_TFLOPS if gemm_n else None,
                      "flops_convention": "achieved = real FP64 flops the kernel executes (3M: 6 M N K per complex GEMM) per second, "
                      "summed over every GEMM launch of one step; achieved_lapack = the same launches at 8 M N K",
                      "achieved_lapack": gemm_tf, "executed_over_lapack": ratio,
@@ -440,13 +443,16 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
                      "peak_measured_dmma_microbench is the library's DMMA microbenchmark on this GPU",
                      "gemm_launches": gemm_n, "gemm_share_of_step": gemm_ms / gemm_ref_ms,
                      "gemm_flops_share": gemm_fl / (flops_step * (steps if serial else 1)),
-                     "measured_in": "timed region (single stream)" if serial else
+                     "measured_in": "not collected (--split column / spatial runs time the step only)" if column_split else
+                     "timed region (single stream)" if serial else
                      "one extra step with stream_groups=1 right after the timed region (kernels of different stream "
                      f"groups overlap in the timed region); that serial step took {gemm_ref_ms:.1f} ms"},
         "gpu_launches": int(launches * steps),
         "clocks": clocks.summary(),
         "T_first_energy": float(T_all[0]),
     }
+    if column_split:                                      # a pair of GPUs shares one shard of energies
+        out["config"].update({"n_energy_per_gpu": nE / 2, "parallelism": f"{args.split} split over GPU pairs x energy-parallel x{e_world}"})
     if e2e:
         out["e2e"] = e2e
     return out
@@ -462,9 +468,14 @@ def run_ours(args, cfg):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    if args.dist_backend == "gloo":
+        local %= torch.cuda.device_count()                # functional check: ranks may share a GPU
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.dist_backend == "gloo":
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     build.build()
     binding.load()
     if args.gemm_variant is not None:
@@ -490,6 +501,8 @@ def run_ours(args, cfg):
             "clocks": r["clocks"], "T_first_energy": r["T_first_energy"],
         }
         line["roofline"]["peak_measured_dmma_microbench"] = peak_measured
+        if world > 1 and args.dist_backend != "nccl":
+            line["dist_backend"] = args.dist_backend + " (ranks may share GPUs: functional check of the N > 1 path, NOT a measurement)"
         if "e2e" in r:
             line["e2e"] = r["e2e"]
         if also:
