@@ -318,8 +318,7 @@ def _read_fingerprint(name):
     """tests/golden/c{3,4}_fingerprint.txt, written by tests/golden/make_golden_large.py from oracle/banded.py (Tier B)."""
     import os
     path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"{name.lower()}_fingerprint.txt")
-    if not os.path.exists(path):
-        return None                                   # no Tier B result stored for this config: residual certificate only
+    assert os.path.exists(path), f"{path} is missing (both full-size configs have a stored Tier B result)"
     fp = dict(xcol={}, x=[], g=[])
     with open(path) as f:
         for line in f:
