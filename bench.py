@@ -192,10 +192,31 @@ def oracle_sample(cfg, repeats=1):
     return dt, scale, desc
 
 
+def full_size_oracle_record(cfg):
+    """The one NOT extrapolated oracle time there is for C3 / C4: the run that wrote the Tier B fingerprint of one full energy
+    point (tests/golden/make_golden_large.py: banded LU of the whole matrix, 16 columns of X and the last block column of
+    T^-1), read from that file's header.  Measured once on the build container, not on this box: context, not a timing."""
+    import re
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "tests", "golden", f"{cfg.name.lower()}_fingerprint.txt")
+    try:
+        head = open(path).readline() + open(path).readlines()[1]
+    except (OSError, IndexError):
+        return None
+    m = re.search(r"in (\d+) s on (\d+) host cores", head)
+    if not m:
+        return None
+    return {"seconds_one_energy": int(m.group(1)), "cores": int(m.group(2)), "kind": "oracle/banded.py, full device, no extrapolation",
+            "source": os.path.relpath(path, os.path.dirname(os.path.abspath(__file__))) + " header (build container, not this box)"}
+
+
 def cpu_baseline(cfg):
     dt, scale, desc = oracle_sample(cfg)
-    return {"value": 1.0 / (dt * scale), "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": desc,
-            "sample_seconds": dt, "extrapolated": scale != 1.0, "scale": scale}
+    out = {"value": 1.0 / (dt * scale), "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": desc,
+           "sample_seconds": dt, "extrapolated": scale != 1.0, "scale": scale}
+    rec = full_size_oracle_record(cfg)
+    if rec:
+        out["full_size_record"] = rec
+    return out
 
 
 def run_reference(args, cfg):
