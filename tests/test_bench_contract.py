@@ -47,3 +47,15 @@ def test_reference_sample_shrinks_with_the_number_of_repeats():
     # cost model of oracle_sample: LU of the truncated matrix at 100 GFLOP/s; 23 repeats of C4's 8192^2 sample exceed 200 s
     assert 23 * (8.0 / 3.0) * (2 * 4096) ** 3 / 1e11 > 200.0 > 6 * (8.0 / 3.0) * (2 * 4096) ** 3 / 1e11
     assert bench.parse.__module__ == "bench"
+
+
+def test_full_size_oracle_record_comes_from_the_fingerprint_headers():
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1812_01396_b200 import inputs
+    for name in ("C3", "C4"):
+        rec = bench.full_size_oracle_record(inputs.CONFIGS[name])
+        head = open(os.path.join(ROOT, "tests", "golden", f"{name.lower()}_fingerprint.txt")).readlines()[1]
+        assert rec is not None and f"in {rec['seconds_one_energy']} s on {rec['cores']} host cores" in head
+        assert "not this box" in rec["source"]
+    assert bench.full_size_oracle_record(inputs.CONFIGS["C0"]) is None    # no stored full-size run: nothing is made up
