@@ -289,6 +289,42 @@ ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB_dev, int ld, long long
                              long long strideX, int* ipiv_dev, int* info_dev, int batch, void* work_dev, size_t work_bytes,
                              void* cuda_stream);
 
+/* ss_zgesv_batched for callers that are not in a position to allocate device memory.
+ *
+ * Who that is: code that is handed device pointers by a host application and owns no allocator of its own (a plug-in
+ * inside a transport code whose GPU memory was carved up at start-up, a Fortran/C driver that only forwards pointers);
+ * code running after the whole HBM has been given away (H, S and the block columns of a large device, or another
+ * framework's memory pool, leave nothing for a cudaMalloc to find); and code inside a latency-critical loop, where
+ * cudaMalloc / cudaFree stall the whole device while they run.  ss_zgesv_batched serves them only if somebody else has
+ * set aside ss_lu_workspace_bytes(n, batch) of scratch beforehand; this variant brings its scratch with it.
+ *
+ * The scratch (block inverses of the factors, row-move buffer, permutation lists) is ONE fixed array of
+ * SS_NOALLOC_SCRATCH_BYTES that is part of the library image: every GPU on which the library's kernels get loaded holds
+ * that many bytes from then until the process exits, whether or not this function is ever called.  The function itself
+ * calls no cudaMalloc, cudaFree, or any routine that allocates; the caller passes inputs and outputs only.
+ *
+ * Arguments, layout, results and asynchrony are those of ss_zgesv_batched without (work_dev, work_bytes); the results are
+ * the same bits, because the same kernels run in the same order.  Differences the caller has to know about:
+ *   - Size limit: ss_lu_workspace_bytes(n, batch) must not exceed SS_NOALLOC_SCRATCH_BYTES, otherwise the call does
+ *     nothing and returns SS_ERR_INVALID_ARG (ss_strerror: "invalid argument").  16 MiB covers, for instance, n = 1024
+ *     with batch 1, n = 512 with batch 3, n = 256 with batch 10, n = 128 with batch 21.  Check with ss_lu_workspace_bytes.
+ *   - The device that is current at the call must be the one AB_dev, X_dev, ipiv_dev, info_dev and cuda_stream belong to:
+ *     each device has its own copy of the array.
+ *   - First call on a device: the function looks up where that device keeps its copy of the array (one
+ *     cudaGetSymbolAddress, which also makes the runtime load the library's kernels onto that device) and remembers the
+ *     answer.  Make that first call during set-up, before any stream capture is begun; later calls on the device only
+ *     enqueue kernels and one memset of info_dev.
+ *   - All calls on one device share the one array, and it keeps whatever the previous call left in it.  Nothing in it needs
+ *     to start at zero (every part is written within a call before that call reads it), so nothing is cleared.  Two calls
+ *     whose GPU work can overlap -- different streams without an event between them, or two host threads -- overwrite each
+ *     other's scratch and give wrong results without any error: keep all calls of one device on one stream, or order them
+ *     yourself.  The same goes for two processes only in the sense that each has its own copy; they do not interfere.
+ * Errors: SS_ERR_INVALID_ARG (arguments as for ss_zgesv_batched, or the size limit), SS_ERR_CUDA (the address look-up or a
+ * launch failed).  Singular matrices are reported through info_dev as usual. */
+#define SS_NOALLOC_SCRATCH_BYTES (16u << 20)
+ss_status_t ss_zgesv_batched_noalloc(int n, int nrhs, ss_cplx* AB_dev, int ld, long long stride, ss_cplx* X_dev, int ldx,
+                                     long long strideX, int* ipiv_dev, int* info_dev, int batch, void* cuda_stream);
+
 /* Carrier density from the solution ("charge and current densities can be directly
  * derived from ... c(E)"):  rho[i] = sum_e w[e] * sum_c |X[e][i][c]|^2,  i = 0..n-1.
  *   X_dev [n_energy][n][nrhs] (the output of ss_solve, n = nb*bs), w_dev [n_energy] doubles (occupation x energy

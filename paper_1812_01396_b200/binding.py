@@ -54,6 +54,8 @@ SIGNATURES = {
                                   c_void_p]),
     "ss_zgesv_batched": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong, c_void_p,
                                  c_void_p, c_int, c_void_p, c_size_t, c_void_p]),
+    "ss_zgesv_batched_noalloc": (c_int, [c_int, c_int, c_void_p, c_int, c_longlong, c_void_p, c_int, c_longlong, c_void_p,
+                                         c_void_p, c_int, c_void_p]),
     "ss_fp64_peak_tflops": (c_int, [c_double, POINTER(c_double)]),
     "ss_density": (c_int, [c_void_p, c_int, c_longlong, c_int, c_void_p, c_void_p, c_void_p]),
     "ss_bond_current": (c_int, [c_void_p, c_void_p, c_int, c_void_p]),
@@ -354,6 +356,29 @@ def zgesv_batched(AB, n):
     _check(load().ss_zgesv_batched(n, nrhs, _dev(AB, "AB"), ncols, n * ncols, _dev(X, "X"), nrhs, n * nrhs,
                                    ipiv.data_ptr(), info.data_ptr(), batch, work.data_ptr(), work.numel(), _stream()),
            "ss_zgesv_batched")
+    return X, ipiv, info
+
+
+NOALLOC_SCRATCH_BYTES = 16 << 20      # SS_NOALLOC_SCRATCH_BYTES of include/splitsolve.h
+
+
+def zgesv_batched_noalloc(AB, X, ipiv, info, n):
+    """ss_zgesv_batched_noalloc: zgesv_batched for callers that cannot allocate device memory (they were only handed
+    pointers, the HBM is fully spoken for, or a cudaMalloc stall is not affordable where they run).  Nothing is allocated
+    here either: the caller passes every buffer -- AB [batch, n, n + nrhs] (overwritten), X [batch, n, nrhs] out, ipiv
+    [batch, n] int32 out, info [batch] int32 out, all CUDA tensors on the current device -- and the scratch is the library's
+    built-in array of NOALLOC_SCRATCH_BYTES, which limits the size (load().ss_lu_workspace_bytes(n, batch) must fit, else
+    SplitSolveError "invalid argument") and is shared by all calls on the device: calls whose GPU work could overlap must
+    be ordered by the caller.  Make the first call on a device during set-up, before any stream capture."""
+    import torch
+    batch, rows, ncols = AB.shape
+    nrhs = ncols - n
+    assert rows == n and tuple(X.shape) == (batch, n, nrhs)
+    for t, shape in ((ipiv, (batch, n)), (info, (batch,))):
+        if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and tuple(t.shape) == shape):
+            raise TypeError(f"expected a contiguous CUDA int32 tensor of shape {shape}")
+    _check(load().ss_zgesv_batched_noalloc(n, nrhs, _dev(AB, "AB"), ncols, n * ncols, _dev(X, "X"), nrhs, n * nrhs,
+                                           ipiv.data_ptr(), info.data_ptr(), batch, _stream()), "ss_zgesv_batched_noalloc")
     return X, ipiv, info
 
 

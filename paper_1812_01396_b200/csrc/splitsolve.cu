@@ -4,6 +4,7 @@
 
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "sweep.cuh"
@@ -1306,6 +1307,54 @@ extern "C" ss_status_t ss_zgesv_batched(int n, int nrhs, ss_cplx* AB, int ld, lo
                                         void* stream) {
     if (nrhs < 0 || (nrhs > 0 && (!X || ldx < nrhs))) return SS_ERR_INVALID_ARG;
     return lu_common(n, nrhs, n + nrhs, AB, ld, stride, X, ldx, sX, ipiv, info, batch, work, work_bytes, stream);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// ss_zgesv_batched for callers that cannot allocate device memory (plug-ins that are only handed pointers, runs whose HBM
+// is fully spoken for, latency-critical loops that cannot afford cudaMalloc's device-wide stall): the LU scratch is this
+// fixed array inside the library image instead of a caller-owned buffer.  Every device that loads the library carries it
+// until the process ends.  Nothing here allocates.
+//
+// ss_noalloc_scratch is a DEVICE symbol.  In host code its name is only a host-side shadow the runtime uses as a look-up
+// key -- it is not an address the GPU can use: a kernel given `ss_noalloc_scratch` (or &ss_noalloc_scratch[0]) from host
+// code would fault, or scribble over host memory on systems where the GPU can reach it.  The device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current (each device has its own copy at its own address).
+// ---------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char ss_noalloc_scratch[SS_NOALLOC_SCRATCH_BYTES];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static std::mutex g_noalloc_mu;
+static void* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};    // device address of ss_noalloc_scratch, per device ordinal
+
+// Device address of the current device's copy of the scratch array; looked up on the first call per device.
+static ss_status_t noalloc_scratch(void** out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return SS_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, ss_noalloc_scratch);
+        if (e != cudaSuccess || !p) { cudaGetLastError(); return SS_ERR_CUDA; }
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return SS_OK;
+}
+
+extern "C" ss_status_t ss_zgesv_batched_noalloc(int n, int nrhs, ss_cplx* AB, int ld, long long stride, ss_cplx* X, int ldx,
+                                                long long sX, int* ipiv, int* info, int batch, void* stream) {
+    if (nrhs < 0 || (nrhs > 0 && (!X || ldx < nrhs))) return SS_ERR_INVALID_ARG;
+    if (n < 1 || batch < 1) return SS_ERR_INVALID_ARG;
+    // the size limit is checked first, from host arithmetic alone: an oversized request touches neither the device nor the array
+    const size_t need = ss_lu_workspace_bytes(n, batch);
+    if (need == 0 || need > (size_t)SS_NOALLOC_SCRATCH_BYTES) return SS_ERR_INVALID_ARG;
+    void* work = nullptr;
+    ss_status_t s = noalloc_scratch(&work);
+    if (s != SS_OK) return s;
+    // same host driver, same kernels, same order as ss_zgesv_batched: only where the scratch lives differs.  The scratch is
+    // not cleared: the block inverses, the permutation lists and the row-move buffer are each written before they are read.
+    return lu_common(n, nrhs, n + nrhs, AB, ld, stride, X, ldx, sX, ipiv, info, batch, work, (size_t)SS_NOALLOC_SCRATCH_BYTES, stream);
 }
 
 extern "C" ss_status_t ss_density(const ss_cplx* X, int n_energy, long long n, int nrhs, const double* w, double* rho,
