@@ -502,3 +502,34 @@ def test_schur_complements_are_hermitian_at_real_energy_and_match_the_dense_defi
     p2 = tiny(5, 4, eta=1e-3)
     D2 = stepwise.schur_complements_first_column(p2.E[0], p2.H_diag, p2.H_upper, p2.S_diag, p2.S_upper)
     assert np.abs(D2[0] - D2[0].conj().T).max() >= 1e-4
+
+
+# --------------------------------------------------------------------------------------------
+# why the GPU parity tests assert 1000x looser tolerances at Im E = 0 (tests/test_parity_gpu.py, ragged-size test):
+# the loss of digits at real energies inside the band belongs to the METHOD (Eq. 11-13 split A = E S - H from the
+# self-energies; A alone is nearly singular at the closed device's resonances), not to the CUDA kernels.
+# The paper's own sequence of steps evaluated in numpy (oracle/stepwise.py, LAPACK LU with partial pivoting at every
+# "Solve") shows it on the same generator and seeds the GPU test draws from.
+# --------------------------------------------------------------------------------------------
+def test_method_loses_digits_at_real_energies_inside_the_band_in_numpy_too():
+    worst = {}
+    for eta in (0.0, 1e-3):
+        bwd, relx = [], []
+        for it in range(12):
+            bs, nb = [16, 33, 64, 96, 128][it % 5], 2 + it % 4
+            p = inputs.random_problem(bs, nb, 3, 5, seed=2000 + it, inj_last=True, eta=eta)
+            for e in range(p.n_energy):
+                Q, _ = stepwise.algorithm1_first_column(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+                P, _ = stepwise.algorithm1_last_column(p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper)
+                _, _, x = stepwise.four_steps(Q, P, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], p.Inj_last[e])
+                a = (p.E[e], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[e], p.Sigma_R[e], p.Inj_first[e], p.Inj_last[e])
+                bwd.append(residual.backward_error(*a, x))
+                relx.append(residual.rel_frobenius(x, dense.solve_energy(*a)["X"]))
+        worst[eta] = (max(bwd), max(relx))
+    # Im E = 1e-3 (the BASELINE.json configs): the north_star tolerances hold with two orders of magnitude to spare
+    assert worst[1e-3][0] <= 1e-13 and worst[1e-3][1] <= 1e-10
+    # Im E = 0: the same steps lose at least an order of magnitude (measured here: 1.1e-12 against 1.7e-14) ...
+    assert worst[0.0][0] > 10.0 * worst[1e-3][0]
+    assert worst[0.0][1] > 10.0 * worst[1e-3][1]
+    # ... and stay within the 1000x looser bounds the GPU tests assert at real energies
+    assert worst[0.0][0] <= 1e3 * 1e-12 and worst[0.0][1] <= 1e3 * 1e-8
