@@ -175,12 +175,15 @@ ss_status_t ss_transmission(ss_handle_t h, double* T_host);
  * [nb][bs][bs]: Q_first[i] = (A^-1)_{i+1,1}, Q_last[i] = (A^-1)_{i+1,nb}.  Valid until the next ss_solve. */
 ss_status_t ss_inverse_columns(ss_handle_t h, int energy, const ss_cplx** Q_first_dev, const ss_cplx** Q_last_dev);
 
-/* Copies the same two block columns into caller-owned device buffers [nb][bs][bs] (either may be NULL),
- * ordered on the stream of the last ss_solve. */
+/* Copies the same two block columns into caller-owned device buffers [nb][bs][bs] (either may be NULL).  Synchronises: waits
+ * for the handle's last solve, and the copies are complete on return.  With option "hermitian" = 2 the solve is checked
+ * first (and redone on the general path if its growth limit was exceeded), so an error of ss_synchronize can be returned. */
 ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cplx* Q_first_out_dev, ss_cplx* Q_last_out_dev);
 
-/* Location of the first exactly-zero pivot of the last ss_solve (-1s if none): energy index, 1-based block
- * index i of Alg. 1 (0 = the corner system R), column 0 = first-column sweep / 1 = mirror sweep. Synchronises. */
+/* Location of the first exactly-zero pivot (or column without a finite candidate) of the last ss_solve (-1s if none): energy
+ * index, 1-based block index i of Alg. 1 (0 = the corner system R; -2 = an interface system of ss_merge_partition, column then
+ * 0 for the system of a, 1 for that of b'), column 0 = first-column sweep / 1 = mirror sweep.  Records of the sweep come
+ * before those of the corner system and of the merges, and survive later merge levels.  Synchronises. */
 ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int* column);
 
 /* Closed-form flop count of steps a1-a7 per energy point (LAPACK convention: complex multiply-add = 8 flops;
@@ -260,10 +263,13 @@ ss_status_t ss_zgemm_batched(int M, int N, int K, double alpha, const ss_cplx* A
                              const ss_cplx* B_dev, int ldb, long long strideB, double beta, ss_cplx* C_dev, int ldc,
                              long long strideC, int batch, void* cuda_stream);
 
-/* The same product with SUM PLANES: the 3M arithmetic needs re + im of every operand element; A_sum_dev / B_sum_dev (doubles,
+/* EXPERIMENT, not used by the solve path (profiles/r02_gemm_sumplane.md: bit-identical, slower); kept for bench.py --sumplane.
+ * The same product with SUM PLANES: the 3M arithmetic needs re + im of every operand element; A_sum_dev / B_sum_dev (doubles,
  * same leading dimensions and batch strides as A / B, both or neither) supply them, so that the kernel stages them beside
- * the operands instead of adding per fragment on the FP64 pipe; C_sum_dev (or NULL) receives re + im of every element of C,
- * for use as an operand's sum plane later.  Needs K, N, lda, ldb and the strides even to take effect (else ignored). */
+ * the operands instead of adding per fragment on the FP64 pipe.  They take effect only where the software-pipelined 3M
+ * kernel runs (GEMM variant 3, or variant 1 with K >= 768) and K, N, lda, ldb and the strides are even; everywhere else
+ * they are ignored and the plain product runs -- C holds the same bits either way.  C_sum_dev (or NULL) receives re + im of
+ * every element of C under every 3M variant (1..5); under variant 0 (4M) a non-NULL C_sum_dev is SS_ERR_INVALID_ARG. */
 ss_status_t ss_zgemm_batched_sums(int M, int N, int K, double alpha, const ss_cplx* A_dev, const double* A_sum_dev, int lda,
                                   long long strideA, const ss_cplx* B_dev, const double* B_sum_dev, int ldb, long long strideB,
                                   double beta, ss_cplx* C_dev, double* C_sum_dev, int ldc, long long strideC, int batch,
@@ -343,12 +349,16 @@ ss_status_t ss_bond_current(ss_handle_t h, const ss_cplx* X_dev, int nrhs, doubl
  * FP64 peak"):  0 = 4M (four real products per complex product, 64x64 tile);  1 = 3M, the default (three real products,
  * P1 = Ar Br, P2 = Ai Bi, P3 = (Ar+Ai)(Br+Bi); 6 instead of 8 real flops per complex multiply-add; rounding differs,
  * normwise error stays O(u)), 64x32 CTA tile, kernel chosen by K (3 CTAs/SM for K < 768, software-pipelined main loop at
- * 2 CTAs/SM from K = 768);  2 / 3 = those two 3M kernels for every K.  The process-wide default (initially 1) applies to
- * handles created afterwards and to the handle-less building blocks above. */
+ * 2 CTAs/SM from K = 768);  2 / 3 = those two 3M kernels for every K;  4 / 5 = EXPERIMENTS (measured, not adopted:
+ * profiles/r02_gemm_tma.md): variant 3's main loop with the operand tiles staged by TMA at 2 / 3 CTAs per SM, for uniformly
+ * strided batches of whole matrices only -- any other operand layout, and a tensor map that cannot be encoded, silently take
+ * variant 3.  Anything outside 0..5 is SS_ERR_INVALID_ARG.  The process-wide default (initially 1) applies to handles created
+ * afterwards and to the handle-less building blocks above. */
 ss_status_t ss_set_default_gemm_variant(int variant);
 
-/* Tile rows per raster group of the GEMM kernels (1..64, default 16; process-wide): the CTAs of that many tile rows run
- * side by side and share the B column tiles in L2.  Tuning knob; profiles/r02_gemm_tma.md has the DRAM traffic it controls. */
+/* TUNING KNOB for bench.py --raster, not part of the stable interface: tile rows per raster group of the GEMM kernels (1..64,
+ * default 16; process-wide): the CTAs of that many tile rows run side by side and share the B column tiles in L2;
+ * profiles/r02_gemm_tma.md has the DRAM traffic it controls. */
 ss_status_t ss_set_gemm_raster(int tile_rows);
 int ss_get_default_gemm_variant(void);
 

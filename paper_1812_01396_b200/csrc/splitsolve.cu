@@ -126,7 +126,7 @@ static WsSizes ws_sizes(int nb, int bs, int nE, int nrhs, int slots_per_chain = 
     w.tpart = (size_t)nE * TRACE_PARTS * sizeof(double);
     w.T = (size_t)nE * sizeof(double);
     w.ipiv = (size_t)3 * nE * 2 * bs * sizeof(int);
-    w.info = (size_t)6 * nE * sizeof(int);                     // 3 nE zero-pivot records, 2 nE growth monitors, nE single-column sweeps
+    w.info = (size_t)8 * nE * sizeof(int);                     // 3 nE zero-pivot records, 2 nE growth monitors, nE single-column sweeps, 2 nE merge records
     w.perm = (size_t)nE * perm_ints_per_energy(bs) * sizeof(int);
     return w;
 }
@@ -716,7 +716,7 @@ static cudaError_t enqueue_solve(ss_handle_t h, cudaStream_t stream, int phases,
     const size_t nEs = (size_t)h->n_energy;
     if (phases & PH_SWEEP) {
         if (cudaMemcpyAsync(h->E_dev, h->E_pinned, sizeof(cplx) * nEs, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
-            cudaMemsetAsync(h->info, 0, sizeof(int) * 6 * nEs, stream) != cudaSuccess)
+            cudaMemsetAsync(h->info, 0, sizeof(int) * 8 * nEs, stream) != cudaSuccess)
             return cudaErrorUnknown;
     } else if (cudaMemsetAsync(h->info + 2 * nEs, 0, sizeof(int) * nEs, stream) != cudaSuccess) {   // the corner's records
         return cudaErrorUnknown;
@@ -957,9 +957,11 @@ extern "C" ss_status_t ss_merge_partition(ss_handle_t h, int part, const ss_cplx
     gemm(-1.0, PTh, sT, W2, B2, 1.0, h->aug, s_aug_e, ldg);
     gemm(-1.0, W1, B2, V1, B2, 1.0, h->aug + (long long)bs * ldg, s_aug_e, ldg);
     LuWork w2;                                                            // the sweep's scratch: all of it is free now
-    w2.tinv = h->tinv; w2.ipiv = h->ipiv; w2.ipiv_stride = 2 * bs; w2.info = h->info;   // zero pivots reported like a sweep's
+    w2.tinv = h->tinv; w2.ipiv = h->ipiv; w2.ipiv_stride = 2 * bs; w2.info = h->info + 6 * (size_t)nE;
+    // zero pivots of the interface systems go to the merge's own records [6 nE, 8 nE): the sweep's records [0, 2 nE) stay
+    // readable, and since a record is written by compare-and-swap against 0 and cleared only by the next sweep, the first
+    // failure of ANY merge level survives the levels after it (check_info, ss_last_info: block = -2)
     w2.perm = h->perm; w2.tmp = h->aop; w2.tmp_elems = B2;
-    cudaMemsetAsync(h->info, 0, sizeof(int) * 2 * (size_t)nE, ctx.st);
     lu_factor(ctx, aug, ldg, bs, 2 * bs, 2 * nE, w2, 0);
     cplx *av = h->aop, *bpv = h->aop + B2;                                // a (chain 0) and b' (chain 1) per energy
     back_substitute(ctx, aug, ldg, bs, bs, bp_chain(av, bpv, 2 * B2), bs, 2 * nE, w2);
@@ -1025,7 +1027,7 @@ extern "C" ss_status_t ss_post_column(ss_handle_t h, int column, const ss_cplx* 
 }
 
 static ss_status_t check_info(ss_handle_t h) {
-    const int nE = h->n_energy, n = 6 * nE;
+    const int nE = h->n_energy, n = 8 * nE;
     int* host = (int*)malloc(sizeof(int) * (size_t)n);
     if (!host) return SS_ERR_ALLOC;
     cudaError_t e = cudaMemcpy(host, h->info, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost);
@@ -1083,7 +1085,7 @@ extern "C" ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int*
     if (!h->solved) return SS_ERR_NOT_READY;
     *energy = *block = *column = -1;
     if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
-    const int nE = h->n_energy, n = 6 * nE;
+    const int nE = h->n_energy, n = 8 * nE;
     int* host = (int*)malloc(sizeof(int) * (size_t)n);
     if (!host) return SS_ERR_ALLOC;
     if (cudaMemcpy(host, h->info, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost) != cudaSuccess) {
@@ -1092,7 +1094,9 @@ extern "C" ss_status_t ss_last_info(ss_handle_t h, int* energy, int* block, int*
     const int info_stride = 2 * h->bs + 2;
     for (int i = 0; i < n; i++) {
         if (!host[i] || (i >= 3 * nE && i < 5 * nE)) continue;     // [3 nE, 5 nE) are the growth monitors
-        if (i < 2 * nE || i >= 5 * nE) {
+        if (i >= 6 * nE) {                                         // interface system of an ss_merge_partition
+            *energy = (i - 6 * nE) >> 1; *column = (i - 6 * nE) & 1; *block = -2;
+        } else if (i < 2 * nE || i >= 5 * nE) {
             const bool single = i >= 5 * nE;                       // ss_sweep_column: one record per energy
             int s = (host[i] - 1) / info_stride;
             *energy = single ? i - 5 * nE : i >> 1;
@@ -1120,6 +1124,14 @@ extern "C" ss_status_t ss_inverse_columns(ss_handle_t h, int energy, const ss_cp
 extern "C" ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cplx* Q_out, ss_cplx* P_out) {
     if (!h || energy < 0 || energy >= h->n_energy) return SS_ERR_INVALID_ARG;
     if (!h->launched || h->swept_cols != 3) return SS_ERR_NOT_READY;        // both block columns swept (ss_solve, ss_sweep_partition)
+    // The columns are complete once the handle's last work is (ev[2]); waiting for it on the host makes the copies below
+    // independent of which stream that work was joined to.  A no-pivot solve (mode 2) may still be discarded and redone:
+    // decide that first, so that the columns returned are the ones the solve stands by.
+    if (cudaEventSynchronize(h->ev[2]) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (h->mode == 2) {
+        ss_status_t c = check_info(h);
+        if (c != SS_OK) return c;
+    }
     const size_t B2 = (size_t)h->bs * h->bs, bytes = sizeof(cplx) * (size_t)h->nb * B2;
     const cplx *q, *p;
     cudaMemcpyKind kind = cudaMemcpyDeviceToDevice;
@@ -1132,6 +1144,7 @@ extern "C" ss_status_t ss_copy_inverse_columns(ss_handle_t h, int energy, ss_cpl
     }
     if (Q_out && cudaMemcpyAsync(Q_out, q, bytes, kind, h->last_stream) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
     if (P_out && cudaMemcpyAsync(P_out, p, bytes, kind, h->last_stream) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }
+    if (cudaStreamSynchronize(h->last_stream) != cudaSuccess) { cudaGetLastError(); return SS_ERR_CUDA; }   // complete on return
     return SS_OK;
 }
 
@@ -1269,6 +1282,7 @@ extern "C" ss_status_t ss_zgemm_batched_sums(int M, int N, int K, double alpha, 
                                              double beta, ss_cplx* C, double* C_sum, int ldc, long long sC, int batch, void* stream) {
     if (M < 0 || N < 0 || K < 0 || batch < 0 || !C || (K > 0 && (!A || !B))) return SS_ERR_INVALID_ARG;
     if (lda < K || ldb < N || ldc < N) return SS_ERR_INVALID_ARG;
+    if (C_sum && g_default_variant == GV_4M) return SS_ERR_INVALID_ARG;   // only the 3M kernels' epilogue writes a sum plane
     GemmArgs g = gemm_std(M, N, K, alpha, bp_strided((const cplx*)(A ? A : C), sA), lda, bp_strided((const cplx*)(B ? B : C), sB), ldb,
                           beta, bp_strided((cplx*)C, sC), ldc);
     if (A_sum && B_sum) { g.shA_c = (const cplx*)A; g.shA_d = A_sum; g.shB_c = (const cplx*)B; g.shB_d = B_sum; }

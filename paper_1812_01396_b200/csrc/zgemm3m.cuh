@@ -587,7 +587,11 @@ static cudaError_t gemm_launch(const GemmArgs& a, int batch, int cfg, int epi, c
         // TMA tensor maps describe uniformly strided batches of whole matrices; anything else takes the cp.async kernel
         const bool ok = !a.A.two && !a.B.two && a.A.n_in >= batch && a.B.n_in >= batch && a.K > 0 &&
                         (batch <= 1 || (a.A.s_in > 0 && a.B.s_in > 0));
-        if (ok) return variant == GV_3M_TMA3 ? gemm3m_epi<C3_64x32tma3>(a, batch, epi, st) : gemm3m_epi<C3_64x32tma>(a, batch, epi, st);
+        if (ok) {
+            cudaError_t e = variant == GV_3M_TMA3 ? gemm3m_epi<C3_64x32tma3>(a, batch, epi, st) : gemm3m_epi<C3_64x32tma>(a, batch, epi, st);
+            if (e != cudaErrorInvalidValue) return e;     // cudaErrorInvalidValue = the tensor maps could not be encoded (nothing was
+            cudaGetLastError();                           // launched): take the cp.async kernel instead of failing the product
+        }
         variant = GV_3M_PF;
     }
     if (variant == GV_3M_PF) {

@@ -231,14 +231,19 @@ __device__ __forceinline__ void st_async_16(unsigned remote_addr, unsigned long 
 // IMPLICIT for the whole panel (no row moves until the end), with the position bookkeeping of LAPACK's sequential swaps.
 // Per inner block:
 //  (1) the 16 active columns of the own row -> registers;
-//  (2) 16 pivot steps WITHOUT any CTA or cluster barrier: every warp finds its candidate (three redux.sync on the bit
-//      pattern of |re|+|im| and the position), leaves the candidate row in its CTA's shared memory, and lane c pushes the
-//      16-byte key into CTA c's shared memory (st.shared::cluster) followed by an mbarrier arrive with release semantics
-//      at cluster scope; every thread waits on its own CTA's mbarrier (8 warps x csize arrivals per step, acquire at
-//      cluster scope), every warp reduces the keys, pulls the winning row out of the winner CTA's shared memory
-//      (ld.shared::cluster) and applies the rank-1 update to the rows in its registers.  Candidate rows and keys are
-//      double-buffered by step parity: a warp can be at most one step ahead of the slowest warp of the cluster, because
-//      the barrier of step j+1 cannot complete without that warp's arrival.
+//  (2) 16 pivot steps WITHOUT any CTA or cluster barrier, two message hops each, both by st.async with mbarrier
+//      transaction counts (no arrive, no release/acquire pair, no remote load):
+//        keys: every warp finds its candidate (warp arg-max of |re|+|im| with the position), stages that row in its own
+//              shared memory, and lane c pushes the warp's 16-byte key into CTA c's key array (st.async.shared::cluster,
+//              completing 16 transaction bytes on CTA c's key barrier of the step's parity); thread 0 of every CTA has
+//              armed that barrier with expect_tx = 16 x (8 warps x csize) bytes, every thread waits on its own CTA's;
+//        row:  every warp reduces the keys (per lane over its keys, then redux.sync max / min on the bit pattern); the
+//              warp holding the winner PUSHES its staged row, the pivot's reciprocal and the row number to every CTA's
+//              row buffer (st.async again, expect_tx = one row message on the row barrier of that parity); every thread
+//              waits on its own CTA's row barrier and applies the rank-1 update to the row in its registers -- column
+//              j+1 at once, the rest deferred into the wait of the next step (software pipelining).
+//      Keys, row messages and both barriers are double-buffered by step parity: a warp can be at most one step ahead of
+//      the slowest warp of the cluster, because the key barrier of step j+1 cannot complete without that warp's key.
 //  (3) the pivot rows' remaining panel columns are read by every CTA, U12 = L11^-1 A12 is solved redundantly in shared
 //      memory (one thread per column), the owners write it back;
 //  (4) rank-16 update of the own row's remaining panel columns with the multipliers still in registers (four columns
@@ -437,7 +442,7 @@ lu_panel_kernel(BPtr Ab, int ld, int j0, int m, int nbw, int* __restrict__ ipiv,
                 const bool singular = !have || zero_piv;
                 if (crank == 0 && tid == 0) {
                     ipiv[(long long)z * ipiv_stride + j0 + q] = j0 + gp;
-                    if (zero_piv) atomicCAS(&info[z], 0, info_base + j0 + q + 1);
+                    if (singular) atomicCAS(&info[z], 0, info_base + j0 + q + 1);   // exact zero, or every candidate NaN (no key)
                 }
                 pend = false;
                 if (!done) {

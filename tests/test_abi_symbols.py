@@ -108,6 +108,16 @@ def test_host_side_argument_logic_without_a_device(libpath):
     assert binding.get_default_gemm_variant() == d
     assert lib.ss_zgemm_batched(-1, 1, 1, 1.0, None, 1, 0, None, 1, 0, 0.0, None, 1, 0, 1, None) == binding.SS_ERR_INVALID_ARG
     assert lib.ss_zgetrf_batched(0, 0, None, 0, 0, None, None, 1, None, 0, None) == binding.SS_ERR_INVALID_ARG
+    # a C sum plane cannot be honoured by the 4M kernel: refused before anything is launched (fake non-NULL pointers)
+    try:
+        assert lib.ss_set_default_gemm_variant(0) == binding.SS_OK
+        assert lib.ss_zgemm_batched_sums(8, 8, 8, 1.0, 4096, None, 8, 64, 4096, None, 8, 64, 0.0, 4096, 4096, 8, 64, 1, None) \
+            == binding.SS_ERR_INVALID_ARG
+    finally:
+        lib.ss_set_default_gemm_variant(d)
+    # the no-allocation LU: the size limit is host arithmetic and comes before any device access
+    assert lib.ss_zgesv_batched_noalloc(1024, 4, 4096, 1028, 0, 4096, 4, 0, 4096, 4096, 2, None) == binding.SS_ERR_INVALID_ARG
+    assert lib.ss_zgesv_batched_noalloc(0, 0, None, 0, 0, None, 0, 0, None, None, 1, None) == binding.SS_ERR_INVALID_ARG
     assert lib.ss_lu_workspace_bytes(0, 1) == 0 and lib.ss_lu_workspace_bytes(300, 2) >= 2 * 2 * 3 * 128 * 128 * 16
     assert lib.ss_lu_workspace_bytes(300, 4) > lib.ss_lu_workspace_bytes(300, 2) > lib.ss_lu_workspace_bytes(100, 2)
 

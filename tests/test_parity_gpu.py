@@ -146,6 +146,46 @@ def test_zgetrf_factors_and_pivots(lib, n):
         assert np.abs(np.tril(LU[z], -1)).max() <= np.sqrt(2.0) + 1e-12
 
 
+@pytest.mark.parametrize("n,nrhs", [(4200, 0), (4480, 48), (8192, 0)])
+def test_zgetrf_panels_of_more_than_4096_rows(lib, n, nrhs):
+    """Panels with more than 4096 rows leave the fused cluster panel kernel (csrc/zgetrf.cuh lu_panel: 16-column leaf
+    kernel, row swaps, 16-row triangular solve, rank-16 GEMM per inner block; perm_build with (2n + 1) ints of shared
+    memory).  On the hot path only the 2bs x 2bs corner system of a5 at bs > 2048 gets there (config C4), so it is pinned
+    here as a building block: n = 4200 takes that route for its first panel only, 4480 for its first three (and carries
+    right-hand sides through the interchanges and both triangular solves), 8192 = the largest n the LU accepts, for all
+    its first 32.  Checks: P A = L U from the in-place factors and LAPACK-style sequential interchanges, j <= ipiv[j] < n,
+    |L_ij| <= sqrt 2 (pivot metric |re| + |im| against the modulus), and A X = B.  The reference products are torch's
+    (cuBLAS) complex128 matmul on the same GPU: independent of the library under test, and n = 8192 stays within seconds."""
+    A = inputs.complex_gaussian(3, 75, n, (1, n, n), 1.0)
+    B = inputs.complex_gaussian(3, 76, n, (1, n, nrhs), 1.0) if nrhs else None
+    if nrhs:
+        X, ipiv, info = lib.zgesv_batched(AB := dev(np.concatenate([A, B], axis=2)), n)
+    else:
+        ipiv, info = lib.zgetrf_batched(AB := dev(A.copy()), n)
+    assert int(info.abs().max()) == 0
+    piv = ipiv.cpu().numpy()[0]
+    assert (piv >= np.arange(n)).all() and (piv < n).all()
+    order = np.arange(n)                                   # row of A that ends up in row r after the interchanges
+    for j in range(n):
+        if piv[j] != j:
+            order[[j, piv[j]]] = order[[piv[j], j]]
+    assert len(np.unique(order)) == n
+    Ad = dev(A[0])
+    LU = AB[0, :, :n]
+    L = torch.tril(LU, -1) + torch.eye(n, dtype=torch.complex128, device="cuda")
+    U = torch.triu(LU)
+    err = torch.linalg.norm(Ad[torch.from_numpy(order).cuda()] - L @ U) / torch.linalg.norm(Ad)
+    assert float(err) <= 1e-13 * n ** 0.5, float(err)      # Frobenius: the sum of n^2 entries, each O(sqrt(n) u |A|)
+    assert float(torch.tril(LU, -1).abs().max()) <= np.sqrt(2.0) + 1e-12
+    assert float(torch.diagonal(LU).abs().min()) > 0.0
+    if nrhs:
+        Bd = dev(B[0])
+        res = torch.linalg.norm(Ad @ X[0] - Bd) / (torch.linalg.norm(Ad) * torch.linalg.norm(X[0]) + torch.linalg.norm(Bd))
+        assert float(res) <= 1e-13, float(res)
+        want = np.linalg.solve(A[0], B[0])
+        assert np.linalg.norm(X[0].cpu().numpy() - want) <= 1e-8 * np.linalg.norm(want)
+
+
 def test_zgesv_needs_pivoting(lib):
     """A matrix whose leading entries are zero: no-pivot LU (the paper's zgesv_nopiv, L186) would divide by zero."""
     n = 48
