@@ -38,24 +38,37 @@ FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 EXECUTED_RATIO = {False: 1.0, True: 0.75}
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant GEMM kernel: read from the committed summary of
 # the `ncu --set full` capture (profiles/*_gemm_traffic.csv: kernel,M,N,K,batch,dram_bytes_read,dram_bytes_write,source)
-TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_gemm_traffic.csv")
+TRAFFIC_CSVS = [os.path.join(ROOT, "profiles", f) for f in ("r03_gemm_traffic.csv", "r02_gemm_traffic.csv")]
 
 
-def ncu_traffic(is3m: bool):
-    """(bytes per launch, note) of the dominant GEMM kernel from the committed ncu summary, or (None, why)."""
+def ncu_traffic(is3m: bool, bs: int, batch: int):
+    """(bytes per launch, over-fetch ratio, note) of the dominant GEMM launch of the timed workload -- M = N = K = bs, `batch`
+    chains per launch (two chains per energy of a stream group) -- from the committed ncu summaries, or (None, None, why).
+    Rows are matched by (kernel, M, N, K) and then by batch; a row of another batch size is used only when there is none of
+    the same, and the note says so.  over-fetch = captured DRAM bytes / algorithmic bytes of the CAPTURED launch."""
     want = "zgemm3m_kernel" if is3m else "zgemm_kernel"
-    try:
-        with open(TRAFFIC_CSV) as f:
-            rows = [ln.strip().split(",") for ln in f if ln.strip() and not ln.startswith("#")]
-        for r in rows[1:]:
-            if r[0] == want:
-                M, N, K, batch = (int(x) for x in r[1:5])
-                rd, wr = float(r[5]), float(r[6])
-                return rd + wr, (f"{os.path.relpath(TRAFFIC_CSV, ROOT)}: {r[0]} {M}x{N}x{K} x{batch}, read {rd:.3g} + write {wr:.3g} B "
-                                 f"per launch (algorithmic {16.0 * (M * K + K * N + M * N) * batch:.3g} B); capture {r[7]}")
-    except OSError:
-        pass
-    return None, f"no ncu summary for {want} in profiles/"
+    rows = []
+    for path in TRAFFIC_CSVS:
+        try:
+            with open(path) as f:
+                for ln in f:
+                    r = ln.strip().split(",")
+                    if len(r) >= 8 and r[0] == want:
+                        rows.append((r, path))
+        except OSError:
+            pass
+    same = [(r, p) for r, p in rows if tuple(int(x) for x in r[1:4]) == (bs, bs, bs)]
+    if not same:
+        return None, None, f"no ncu capture of {want} at {bs}^3 in profiles/ (captured: {sorted({r[1] for r, _ in rows})})"
+    exact = [(r, p) for r, p in same if int(r[4]) == batch]
+    r, path = (exact or same)[0]
+    M, N, K, b = (int(x) for x in r[1:5])
+    rd, wr = float(r[5]), float(r[6])
+    alg = 16.0 * (M * K + K * N + M * N) * b
+    note = (f"{os.path.relpath(path, ROOT)}: {r[0]} {M}x{N}x{K} x{b}, read {rd:.4g} + write {wr:.4g} B per launch, algorithmic "
+            f"{alg:.4g} B, over-fetch {(rd + wr) / alg:.2f}x; capture {','.join(r[7:])}" +
+            ("" if exact else f"; NOTE: the timed step launches batch {batch}, no capture of that batch size is committed"))
+    return rd + wr, (rd + wr) / alg, note
 
 
 def parse():
@@ -87,10 +100,10 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the second block (C3) of the default C4 line")
-    ap.add_argument("--kernel", default=None, choices=["gemm", "density"], help="time ONE kernel alone through its C-ABI "
+    ap.add_argument("--kernel", default=None, choices=["gemm", "density", "lu"], help="time ONE kernel alone through its C-ABI "
                     "entry point instead of the hot path (tuning, and the command of the ncu --set full captures in profiles/)")
     ap.add_argument("--dims", type=int, nargs="*", default=[], help="--kernel gemm: M N K batch [reps]; --kernel density: "
-                    "n_energy n nrhs [reps]")
+                    "n_energy n nrhs [reps]; --kernel lu: n batch [reps]")
     ap.add_argument("--beta", type=float, default=0.0, help="--kernel gemm: C = A B + beta C (1 = the in-place update form)")
     ap.add_argument("--sumplane", action="store_true", help="--kernel gemm: pass re + im planes of A and B (ss_zgemm_batched_sums)")
     ap.add_argument("--raster", type=int, default=None, help="--kernel gemm: tile rows per raster group (library default 16)")
@@ -159,7 +172,13 @@ def config_dict(cfg, world):
             "small workload: inputs fit L2 (launch-bound config)"}
 
 
-def oracle_sample(cfg, repeats=1):
+REFERENCE_BUDGET_S = 150.0     # --impl reference: host seconds the timed oracle repetitions may take in total
+
+
+_sample_inputs = {}
+
+
+def oracle_sample(cfg):
     """Times the oracle, as it stands, on a bounded sample of the workload: ONE energy point of the same generator
     with the device truncated to nb_s blocks (nb_s = 2 for bs >= 1024, else min(nb, 4)), solved by the plain definition
     (LU of the full matrix: oracle/dense.py when the truncated matrix is <= 8192 rows -- with 2 blocks the band of the
@@ -167,19 +186,19 @@ def oracle_sample(cfg, repeats=1):
     form that fits the host) costs 64 nb bs^3 flops for the factorisation, linear in nb, so the per-energy time is
     EXTRAPOLATED by nb / nb_s and flagged as such; `--calibrate-oracle` measures that ratio on C2, and the full-size
     Tier B times of one energy point of C3 / C4 are in the headers of tests/golden/c{3,4}_fingerprint.txt.
-    `repeats` = how many times the caller will time the sample (--impl reference: warm-up + steps): when repeats x the
-    estimated cost of a sample (LU flops at 100 GFLOP/s) exceeds 200 s, the blocks of the sample are halved too (bs_s = bs/2
-    or bs/4; cost ~ bs^3, the extrapolation factor says so), so that the whole run stays within a few minutes.
+    The sample depends on the workload ONLY (never on --steps / --warmup), so the cpu_baseline of the CUDA arm and the
+    --impl reference arm time the same thing and their values differ by timing noise alone; the reference arm bounds its
+    run time by capping how often it repeats the sample (REFERENCE_BUDGET_S), not by shrinking it.
     Returns (sample seconds, scale, description)."""
     from oracle import banded, dense
     nb_s = 2 if cfg.bs >= 1024 else min(cfg.nb, 4)
     bs_s = cfg.bs
-    while bs_s > 256 and repeats * (8.0 / 3.0) * (nb_s * bs_s) ** 3 / 1e11 > 200.0:
-        bs_s //= 2
-    if cfg.kind == "chain":
-        p = inputs.perfect_chain_problem(bs_s, nb_s, 1)
-    else:
-        p = inputs.random_problem(bs_s, nb_s, 1, cfg.nrhs, seed=cfg.seed, threads=os.cpu_count() or 1)
+    if cfg.name not in _sample_inputs:
+        if cfg.kind == "chain":
+            _sample_inputs[cfg.name] = inputs.perfect_chain_problem(bs_s, nb_s, 1)
+        else:
+            _sample_inputs[cfg.name] = inputs.random_problem(bs_s, nb_s, 1, cfg.nrhs, seed=cfg.seed, threads=os.cpu_count() or 1)
+    p = _sample_inputs[cfg.name]
     solver = dense if bs_s * nb_s <= 8192 else banded
     t0 = time.perf_counter()
     solver.solve_energy(p.E[0], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[0], p.Sigma_R[0], p.Inj_first[0], None)
@@ -190,6 +209,14 @@ def oracle_sample(cfg, repeats=1):
             f"oracle/{'dense' if solver is dense else 'banded'}.py LU of the full matrix; solves/s EXTRAPOLATED to the full device "
             f"by x{scale:g} (cost linear in nb" + (", cubic in bs" if bs_s != cfg.bs else "") + "; see profiles/r02_oracle_scaling.md)")
     return dt, scale, desc
+
+
+def reference_repetitions(first_seconds, warmup, steps, budget=REFERENCE_BUDGET_S):
+    """How many times --impl reference repeats the (fixed) sample: warm-up + steps if that fits the budget at the pace of the
+    first repetition, else as many as fit (at least one; at least two when a warm-up was asked for and two fit)."""
+    want = warmup + steps
+    fit = int(budget / max(first_seconds, 1e-9))
+    return max(1, min(want, fit))
 
 
 def full_size_oracle_record(cfg):
@@ -219,6 +246,26 @@ def cpu_baseline(cfg):
     return out
 
 
+def cpu_baseline_full(cfg):
+    """The oracle on the WHOLE device of `cfg`, one energy point, X for the workload's Inj columns: oracle/banded.py, LU with
+    partial pivoting of the full matrix in band storage.  Nothing is truncated and nothing is extrapolated.  T(E) is NOT
+    computed (want_G = False): it needs the last block column of the inverse, 2 bs more right-hand sides, which takes the C2
+    sample from 16 s to 122 s on the box's 16 cores (profiles/r03_bench.md) -- so the sample is LESS work than one energy
+    point of a GPU step, and says so.  Used for C2; C3 / C4 would take 40 min / 4 h per energy point
+    (tests/golden/c{3,4}_fingerprint.txt headers)."""
+    from oracle import banded
+    p = inputs.random_problem(cfg.bs, cfg.nb, 1, cfg.nrhs, seed=cfg.seed, threads=os.cpu_count() or 1)
+    t0 = time.perf_counter()
+    banded.solve_energy(p.E[0], p.H_diag, p.H_upper, p.S_diag, p.S_upper, p.Sigma_L[0], p.Sigma_R[0], p.Inj_first[0], None,
+                        want_G=False)
+    dt = time.perf_counter() - t0
+    return {"value": 1.0 / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+            "sample": f"1 of {cfg.n_energy} energy points of {cfg.name}, the full device (nb={cfg.nb}, bs={cfg.bs}, nrhs={cfg.nrhs}), "
+                      "X only (no T(E): less work than the GPU step's energy point), oracle/banded.py LU of the full matrix in band "
+                      "storage; not truncated, not extrapolated",
+            "sample_seconds": dt, "extrapolated": False, "scale": 1.0}
+
+
 def run_reference(args, cfg):
     """--impl reference: the oracle, as it stands, on the host cores.  Each step is the bounded sample of oracle_sample;
     `ms_per_step` is what was actually timed, `value` the solves/s extrapolated to the full device (flagged)."""
@@ -226,14 +273,21 @@ def run_reference(args, cfg):
     if rank != 0:
         return
     times, desc, scale = [], "", 1.0
-    for i in range(args.warmup + args.steps):
-        dt, scale, desc = oracle_sample(cfg, repeats=args.warmup + args.steps)
-        if i >= args.warmup:
+    dt, scale, desc = oracle_sample(cfg)                                  # the first repetition sizes the run
+    total = reference_repetitions(dt, args.warmup, args.steps)
+    n_warm = min(args.warmup, max(0, total - 1), 1 if total < args.warmup + args.steps else args.warmup)
+    if n_warm == 0:
+        times.append(dt)
+    for i in range(1, total):
+        dt, scale, desc = oracle_sample(cfg)
+        if i >= n_warm:
             times.append(dt)
     mean = sum(times) / max(1, len(times))
     val = 1.0 / (mean * scale) if mean > 0 else 0.0
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * mean, "ms_per_step_is": "the timed sample (one truncated energy point)",
+            "warmup": args.warmup, "steps_timed": len(times), "warmup_run": n_warm,
+            "gpus_used": 0, "n_gpus_is": "the N of the run this line is paired with; the oracle runs on the host cores of rank 0 only",
+            "ms_per_step": 1e3 * mean, "ms_per_step_is": "the timed sample (one truncated energy point)",
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128 (f64 re/im)", "data": "synthetic",
             "config": config_dict(cfg, max(1, args.gpus)),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": desc,
@@ -438,17 +492,22 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
         e2e = {"value": nE * world * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "steps": n_e2e}
         del Xh, Th
+    T_first = float(T_all[0])
     ss.close()
     del X, devt, host
     torch.cuda.empty_cache()
 
     ratio = EXECUTED_RATIO[is3m]
-    traffic, traffic_note = ncu_traffic(is3m)
+    # dominant launch of the timed step: bs^3 with two chains (first / last column sweep) per energy of a stream group
+    dom_batch = 2 * ((nE + min(groups, nE) - 1) // min(groups, nE))
+    traffic, overfetch, traffic_note = ncu_traffic(is3m, bs, dom_batch)
     kern = ("zgemm3m_kernel" if is3m else "zgemm_kernel") + f" [{binding.GEMM_VARIANTS[variant]}] (DMMA.8x8x4, mma.sync f64)"
     out = {
         "value": value, "ms_per_step": ms_step, "steps": steps, "warmup": warmup,
         "config": config_dict(cfg, world), "launch": {"stream_groups": groups, "split": ("spatial pairs" if spatial_split else "column pairs") if column_split else "energy"},
-        "tflops": {"whole_solve": flops_step / (ms_step * 1e-3) / 1e12, "sweep_a1_a4": sweep_tf,
+        "tflops": {"whole_solve": flops_step / (ms_step * 1e-3) / 1e12,
+                   "whole_solve_executed_frac_of_fp64_peak": flops_step / (ms_step * 1e-3) / 1e12 * ratio / FP64_PEAK_NOMINAL_TFLOPS,
+                   "sweep_a1_a4": sweep_tf,
                    "sweep_executed": sweep_tf * ratio, "sweep_executed_frac_of_fp64_peak": sweep_tf * ratio / FP64_PEAK_NOMINAL_TFLOPS,
                    "flops_per_step": flops_step,
                    "convention": "LAPACK (complex multiply-add = 8 flops), closed form ss_flops; *_executed = x" + str(ratio) +
@@ -459,10 +518,12 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
                      "flops_convention": "achieved = real FP64 flops the kernel executes (3M: 6 M N K per complex GEMM) per second, "
                      "summed over every GEMM launch of one step; achieved_lapack = the same launches at 8 M N K",
                      "achieved_lapack": gemm_tf, "executed_over_lapack": ratio,
-                     "traffic": traffic, "traffic_note": traffic_note,
+                     "traffic": traffic, "traffic_overfetch": overfetch, "traffic_note": traffic_note,
+                     "dominant_launch": f"{bs}x{bs}x{bs} x{dom_batch}",
                      "peak_source": "148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (no FP64 entry in MEASURED_PEAKS.json); "
                      "peak_measured_dmma_microbench is the library's DMMA microbenchmark on this GPU",
                      "gemm_launches": gemm_n, "gemm_share_of_step": gemm_ms / gemm_ref_ms,
+                     "ms_per_step_serial": None if (serial or column_split) else gemm_ref_ms,
                      "gemm_flops_share": gemm_fl / (flops_step * (steps if serial else 1)),
                      "measured_in": "not collected (--split column / spatial runs time the step only)" if column_split else
                      "timed region (single stream)" if serial else
@@ -470,7 +531,7 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
                      f"groups overlap in the timed region); that serial step took {gemm_ref_ms:.1f} ms"},
         "gpu_launches": int(launches * steps),
         "clocks": clocks.summary(),
-        "T_first_energy": float(T_all[0]),
+        "T_first_energy": T_first,
     }
     if column_split:                                      # a pair of GPUs shares one shard of energies
         out["config"].update({"n_energy_per_gpu": nE / 2, "parallelism": f"{args.split} split over GPU pairs x energy-parallel x{e_world}"})
@@ -479,14 +540,35 @@ def measure(args, cfg, world, rank, local, steps, warmup, want_e2e, want_clocks=
     return out
 
 
+def launch_ranks(n: int) -> int:
+    """Re-executes this command line under torch.distributed.run with n ranks on this node (rendezvous on 127.0.0.1, a free
+    port); rank r binds GPU r (LOCAL_RANK).  NCCL's own logging is left as the environment has it (NCCL_DEBUG is passed
+    through), so a scaling run can count ranks and transports.  Returns the launcher's exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd).returncode
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
     from paper_1812_01396_b200 import binding, build
 
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        # started without torchrun: start the N ranks here (one per GPU) and let rank 0 print the line
+        if args.dist_backend != "gloo" and torch.cuda.device_count() < args.gpus:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: only {torch.cuda.device_count()} CUDA device(s) visible "
+                             "(--dist-backend gloo lets ranks share GPUs for a functional check)")
+        raise SystemExit(launch_ranks(args.gpus))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != max(1, args.gpus):
+        raise SystemExit(f"bench.py --gpus {args.gpus} was started with WORLD_SIZE={world}: the two must agree")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
     if args.dist_backend == "gloo":
@@ -512,6 +594,18 @@ def run_ours(args, cfg):
         also = {"C3": {k: a[k] for k in ("value", "ms_per_step", "steps", "warmup", "config", "launch", "tflops", "roofline", "gpu_launches",
                                          "clocks")}}
         also["C3"]["unit"] = UNIT
+        # the three small configurations (launch-latency-bound): every BASELINE.json config in one driver line
+        for name in ("C2", "C1", "C0"):
+            c = inputs.CONFIGS[name]
+            a = measure(args, c, world, rank, local, max(1, min(args.steps, 5)), 3, want_e2e=False)
+            also[name] = {k: a[k] for k in ("value", "ms_per_step", "steps", "warmup", "config", "launch", "tflops", "gpu_launches",
+                                            "T_first_energy")}
+            also[name]["unit"] = UNIT
+            also[name]["launches_per_step"] = a["gpu_launches"] // max(1, a["steps"])
+        if not args.no_cpu_baseline:
+            # the one configuration whose FULL-size oracle run fits a bench run: GPU and oracle timed in the same run, same
+            # box, same (whole) device -- the un-extrapolated counterpart of the flagged cpu_baseline of C4 / C3
+            also["C2"]["cpu_baseline"] = cpu_baseline_full(inputs.CONFIGS["C2"])
 
     if rank == 0:
         line = {
@@ -621,6 +715,38 @@ def kernel_density(args):
           f"rel err {err:.1e}")
 
 
+def kernel_lu(args):
+    """ss_zgetrf_batched alone (a2 of the sweep: `batch` chains of an n x n pivoted LU, the shape one block step of a
+    stream group factors): best-of-reps CUDA-event time, TFLOP/s at (8/3) n^3 per matrix.  The command of the
+    `ncu --set full -k regex:lu_panel` capture under profiles/ (the latency-bound panel kernel is its second kernel)."""
+    import torch
+    from paper_1812_01396_b200 import binding, build
+    build.build()
+    a = args.dims
+    n, batch = (a + [2048, 16][len(a):])[:2]
+    reps = a[2] if len(a) > 2 else 5
+    g = torch.Generator(device="cuda").manual_seed(0)
+    A0 = torch.randn((batch, n, n), dtype=torch.complex128, device="cuda", generator=g)
+    A = A0.clone()
+    for _ in range(2):
+        A.copy_(A0)
+        ipiv, info = binding.zgetrf_batched(A, n)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = 1e30
+    for _ in range(reps):
+        A.copy_(A0)
+        e0.record()
+        ipiv, info = binding.zgetrf_batched(A, n)
+        e1.record()
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    assert int(info.abs().max()) == 0
+    tf = 8.0 / 3.0 * n ** 3 * batch / best / 1e9
+    print(f"zgetrf n={n} batch={batch}: {best:.3f} ms  {tf:.2f} TFLOP/s (LAPACK conv., (8/3) n^3)  "
+          f"{(n + 127) // 128} panel launches of lu_panel_kernel per factorisation", flush=True)
+
+
 def emulate_split(args, cfg):
     """Per-rank work of the 2-GPU splits, on one GPU (the ranks run one after the other, so nothing waits on anything)."""
     import torch
@@ -692,7 +818,7 @@ def main():
         calibrate_oracle()
         return
     if args.kernel:
-        (kernel_gemm if args.kernel == "gemm" else kernel_density)(args)
+        {"gemm": kernel_gemm, "density": kernel_density, "lu": kernel_lu}[args.kernel](args)
         return
     if args.emulate_split:
         emulate_split(args, cfg)

@@ -28,25 +28,38 @@ def test_reference_arm_line():
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
 
 
-def test_both_arms_spell_config_the_same():
+def test_reference_arm_config_is_config_dict_of_the_workload():
+    """Both arms build `config` with bench.config_dict (the driver compares the two lines): the reference arm's printed
+    config must be exactly that function's value for the workload (the CUDA arm passes the same function's value through)."""
     sys.path.insert(0, ROOT)
     import bench
     from paper_1812_01396_b200 import inputs
-    src = open(os.path.join(ROOT, "bench.py")).read()
-    assert src.count('"config": config_dict(cfg,') >= 2                  # reference arm and CUDA arm
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "C0", "--steps", "1",
+                          "--warmup", "0"], capture_output=True, text=True, cwd=ROOT, timeout=300)
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["config"] == bench.config_dict(inputs.CONFIGS["C0"], 1)
+    assert line["steps_timed"] == 1 and line["warmup_run"] == 0 and line["gpus_used"] == 0
     d = bench.config_dict(inputs.CONFIGS["C4"], 1)
     assert d["workload"] == "C4" and d["bs"] == 4096 and d["nb"] == 24 and d["n_energy_per_gpu"] == 4 and d["nrhs"] == 512
     assert "L2" in d["l2"]
 
 
-def test_reference_sample_shrinks_with_the_number_of_repeats():
+def test_reference_sample_does_not_depend_on_the_number_of_repeats():
+    """the two arms of one driver call must quote the same baseline.  The oracle sample is a function of the
+    workload only; the reference arm keeps its run time bounded by repeating it fewer times, never by shrinking it."""
     sys.path.insert(0, ROOT)
     import bench
-    src = open(os.path.join(ROOT, "bench.py")).read()
-    assert "repeats=args.warmup + args.steps" in src
-    # cost model of oracle_sample: LU of the truncated matrix at 100 GFLOP/s; 23 repeats of C4's 8192^2 sample exceed 200 s
-    assert 23 * (8.0 / 3.0) * (2 * 4096) ** 3 / 1e11 > 200.0 > 6 * (8.0 / 3.0) * (2 * 4096) ** 3 / 1e11
-    assert bench.parse.__module__ == "bench"
+    from paper_1812_01396_b200 import inputs
+    import inspect
+    assert list(inspect.signature(bench.oracle_sample).parameters) == ["cfg"]
+    _, scale1, desc1 = bench.oracle_sample(inputs.CONFIGS["C0"])
+    _, scale2, desc2 = bench.oracle_sample(inputs.CONFIGS["C0"])
+    assert (scale1, desc1) == (scale2, desc2) and scale1 == 2.0
+    # repetitions: all of warm-up + steps when they fit the budget at the first repetition's pace, else what fits, >= 1
+    assert bench.reference_repetitions(0.01, 3, 20) == 23
+    assert bench.reference_repetitions(13.5, 3, 20, budget=150.0) == 11
+    assert bench.reference_repetitions(500.0, 3, 20, budget=150.0) == 1
+    assert bench.reference_repetitions(13.5, 3, 20, budget=150.0) == bench.reference_repetitions(13.5, 1, 50, budget=150.0)
 
 
 def test_full_size_oracle_record_comes_from_the_fingerprint_headers():
